@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py -- ms per chunk compression step (all layers) and KV tok/s of the OmniMem hot path on B200.
+
+A "step" is one `omnimem_compress_chunk` call: all five stages (score, AVBA budgets, select, compact) over every
+layer of one synthetic chunk.  Default workload = BASELINE.json configs[1] (Qwen2.5-Omni-7B-shaped, bf16).
+`value` = KV tokens processed per second = Nk / t_step (Nk = cached + new rows per layer), whole job over N GPUs.
+Multi-GPU: the path does not shard in this repo (replicas only) -> N independent replicas,
+weak scaling, no data-path collective.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_07577_b200 import inputs as I  # noqa: E402
+
+
+# ------------------------------------------------------------------------------------------------ accounting
+def algorithmic_work(wl: I.Workload, n_v: int, n_a: int) -> dict:
+    """flops of ONE scoring pass over the causal pairs, and minimum HBM bytes."""
+    Nc, Nn = n_v + n_a, wl.Nn
+    Nk = Nc + Nn
+    pairs = Nn * Nc + Nn * (Nn + 1) // 2                  # visible (q, k) pairs per query head (R3)
+    f_pass = 2.0 * wl.D * wl.Hq * wl.L * pairs
+    es = wl.elem_bytes
+    qb, kb = wl.L * wl.Hq * Nn * wl.D * es, wl.L * wl.Hkv * Nk * wl.D * es
+    keep = min(wl.budget, Nk)
+    score_b = 2 * (qb + kb) + 2 * wl.L * wl.Hq * Nn * 4 + wl.L * wl.Hkv * Nk * 4
+    cos_b = kb + wl.L * wl.Hkv * Nk * 4
+    fin_b = 3 * wl.L * wl.Hkv * Nk * 4
+    sel_b = wl.L * wl.Hkv * (Nk + keep) * 4
+    comp_b = 2 * 2 * wl.L * wl.Hkv * keep * wl.D * es + wl.L * wl.Hkv * keep * 4
+    return dict(Nk=Nk, pairs=pairs, f_pass=f_pass, exps_pass=pairs * wl.Hq * wl.L,
+                bytes=dict(score=score_b, cosine=cos_b, finalize=fin_b, select=sel_b, compact=comp_b,
+                           total=score_b + cos_b + fin_b + sel_b + comp_b))
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=p["hbm_gbs"], tf_burst=p["bf16_tflops"], tf_sust=p.get("bf16_tflops_sustained", p["bf16_tflops"]),
+                    src="measured")
+    return dict(hbm_gbs=6650.0, tf_burst=1590.0, tf_sust=1400.0, src="fallback")   # B200_PROFILING.md fallback
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index: int, period: float = 0.05):
+        self.index, self.period, self.samples, self.reasons = index, period, [], set()
+        self.max_mhz, self._stop, self._thr, self.ok = None, threading.Event(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def _loop(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake": 0x80}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample_seconds(wl: I.Workload, layer: int, heads) -> float:
+    """Time the fp64 oracle (as it stands, on the host cores) on a bounded sample of the workload: all five stages of
+    `layer` restricted to the KV heads in `heads` (and their query groups).  Returns seconds."""
+    from oracle import ref
+    x = I.layer_inputs(wl, layer)
+    G = wl.G
+    hs = list(heads)
+    qs = [h * G + g for h in hs for g in range(G)]
+    cache = torch.zeros(1, len(hs), wl.cache_cap, wl.D, dtype=wl.torch_dtype)
+    cacheV = torch.zeros_like(cache)
+    nc = wl.n_v + wl.n_a
+    cache[0, :, :nc], cacheV[0, :, :nc] = x["cacheK"][hs], x["cacheV"][hs]
+    p = ref.RefParams(L=1, Hq=len(qs), Hkv=len(hs), D=wl.D, cache_cap=wl.cache_cap, Nn_v=wl.Nn_v, Nn_a=wl.Nn_a,
+                      sim_stride_v=wl.sim_stride_v, sim_stride_a=wl.sim_stride_a)
+    n_v, n, B = np.array([wl.n_v], np.int32), np.array([nc], np.int32), np.array([wl.budget], np.int32)
+    chunkK, chunkV, Q = x["chunkK"][hs][None].contiguous(), x["chunkV"][hs][None].contiguous(), x["Q"][qs][None].contiguous()
+    t0 = time.perf_counter()
+    ref.compress_chunk(p, cache, cacheV, n_v, n, chunkK, chunkV, Q, B)      # widening to fp64 is part of the oracle's step
+    return time.perf_counter() - t0
+
+
+def run_reference(args, wl: I.Workload, rank: int, world: int):
+    """--impl reference: the oracle timed on the host cores; each step = one (layer, KV head) unit, scaled to the step."""
+    if rank != 0:
+        return
+    from oracle import ref
+    work = algorithmic_work(wl, wl.n_v, wl.n_a)
+    units = wl.L * wl.Hkv
+    for i in range(args.warmup):
+        oracle_sample_seconds(wl, 0, [i % wl.Hkv])
+    ts = [oracle_sample_seconds(wl, (i // wl.Hkv) % wl.L, [i % wl.Hkv]) for i in range(args.steps)]
+    t_step = float(np.mean(ts)) * units
+    val = work["Nk"] / t_step
+    cores = ref.num_threads()
+    sample = f"one (layer, KV head) unit of {units} per step, all five stages, scaled x{units}"
+    print(json.dumps({
+        "impl": "reference", "metric": "kv_tokens_per_s", "value": val, "unit": "KV tok/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "KV tok/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "KV tok/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
+    import torch.distributed as dist
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    eng = OmniMem.for_workload(wl, device=str(dev))
+    t_gen = time.perf_counter()
+    x = I.full_inputs(wl, pin=True)                      # chunk tensors in pinned host memory (e2e source)
+    t_gen = time.perf_counter() - t_gen
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    dst = eng.new_cache()
+    host_chunk = Chunk(x["chunkK"], x["chunkV"], x["Q"], wl.Nn_v, wl.Nn_a)
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
+    host_M_v = torch.zeros(wl.L, dtype=torch.int32).pin_memory()
+    host_M_a = torch.zeros(wl.L, dtype=torch.int32).pin_memory()
+    work = algorithmic_work(wl, wl.n_v, wl.n_a)
+    peaks = measured_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing (inputs already in HBM), per-stage events inside the timed region
+    eng.set_profiling(True)
+    for _ in range(args.warmup):
+        eng.compress_chunk(src, chunk, B, dst)
+    barrier()
+    stage_sum = {}
+    launches = 0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            eng.compress_chunk(src, chunk, B, dst)
+            ms, nl = eng.stage_ms()                      # waits on this step's own events (adds ~us per 10s of ms)
+            launches += nl
+            for k, v in ms.items():
+                stage_sum[k] = stage_sum.get(k, 0.0) + v
+        ev1.record()
+        barrier()
+    t_total = ev0.elapsed_time(ev1) / 1e3
+    clocks = clk.summary()
+    eng.set_profiling(False)
+
+    # ---- end to end through the C ABI with HOST buffers (H2D of the chunk + D2H of the budgets inside the region)
+    h2d = d2h = 0
+    for _ in range(2):
+        h2d, d2h = eng.compress_chunk_host(src, host_chunk, chunk, B, dst, host_M_v, host_M_a)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        eng.compress_chunk_host(src, host_chunk, chunk, B, dst, host_M_v, host_M_a)
+    torch.cuda.synchronize(dev)
+    t_e2e = time.perf_counter() - t0
+
+    if world > 1:
+        tt = torch.tensor([t_total, t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)          # max over ranks (reporting only; no data-path collective)
+        t_total, t_e2e = float(tt[0]), float(tt[1])
+    if rank != 0:
+        return
+    t_step = t_total / args.steps
+    stage_ms = {k: v / args.steps for k, v in stage_sum.items()}
+    dom = "colsum" if stage_ms.get("colsum", 0) >= stage_ms.get("lse", 0) else "lse"
+    t_dom = stage_ms[dom] / 1e3
+    achieved = work["f_pass"] / t_dom / 1e12 if t_dom > 0 else 0.0
+    t_roof = max(2 * work["f_pass"] / (peaks["tf_sust"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
+    out = {
+        "metric": "kv_tokens_per_s", "value": world * work["Nk"] / t_step, "unit": "KV tok/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype, "data": "synthetic",
+        "config": {"workload": wl.name, "L": wl.L, "Hq": wl.Hq, "Hkv": wl.Hkv, "D": wl.D, "cache_rows": wl.n_v + wl.n_a,
+                   "chunk_rows": wl.Nn, "budget": wl.budget, "parallelism": f"replicas x{world}",
+                   "l2": "inputs larger than L2 (Q+K+V per step >> 126 MB); no flush", "gen_s": round(t_gen, 1)},
+        "clocks": clocks,
+        "e2e": {"value": world * work["Nk"] / (t_e2e / args.steps), "unit": "KV tok/s", "ms_per_step": t_e2e / args.steps * 1e3,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": launches,
+        "stage_ms": stage_ms,
+        "roofline": {"bound": "tensor", "kernel": f"score_tc_kernel<{2 if dom == 'colsum' else 1}> ({dom})",
+                     "achieved": achieved, "peak": peaks["tf_sust"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sust"],
+                     "peak_source": f"{peaks['src']} bf16 sustained (kernel timed inside the step)",
+                     "frac_of_burst": achieved / peaks["tf_burst"], "traffic": NCU_TRAFFIC_BYTES.get(dom),
+                     "algorithmic_flops_per_launch": work["f_pass"], "exps_per_launch": work["exps_pass"]},
+        "step_roofline": {"t_roof_ms": t_roof * 1e3, "frac_two_pass": t_roof / t_step,
+                          "frac_one_pass_normalised": t_roof / 2 / t_step, "bytes": work["bytes"]["total"],
+                          "flops_two_pass": 2 * work["f_pass"]},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import ref
+        secs = oracle_sample_seconds(wl, 0, [0, 1][: wl.Hkv])
+        nunits = min(2, wl.Hkv)
+        t_cpu = secs * wl.L * wl.Hkv / nunits
+        out["cpu_baseline"] = {"value": work["Nk"] / t_cpu, "unit": "KV tok/s", "cores": ref.num_threads(), "kind": "oracle",
+                               "ms_per_step": t_cpu * 1e3,
+                               "sample": f"layer 0, KV heads 0-{nunits - 1} of {wl.Hkv} (all five stages, {secs:.1f} s), "
+                                         f"scaled x{wl.L * wl.Hkv // nunits}"}
+    print(json.dumps(out), flush=True)
+
+
+# per-launch DRAM bytes of the scoring kernels from the committed ncu --set full capture (profiles/); None = not captured
+NCU_TRAFFIC_BYTES = {"colsum": None, "lse": None}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[i-1]; 2 = the config the metric is quoted on")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    wl = I.CONFIGS[args.config]
+    rank, local_rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        run_reference(args, wl, rank, world)
+        return
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    try:
+        run_ours(args, wl, rank, local_rank, world)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,190 @@
+/*
+ * omnimem.h -- C ABI of the B200-native OmniMem per-chunk KV-cache compression step.
+ *
+ * What it computes (arxiv/paper_2606_07577; "P:<n>" = line of PAPER.md, "R<k>" = reading listed in DESIGN.md):
+ * each time a chunk of visual + audio tokens is appended to every layer's KV cache (Eq.3) the cache is
+ * pruned back to a fixed budget (Eq.4-5) by
+ *   1. importance   a_k  = sum over the chunk's queries of softmax attention on key k      (Eq.6)
+ *   2. redundancy   s_k  = mean cosine similarity with the adjacent positions               (Eq.7)
+ *   3. AVBA         C_m  = H[abar_m](1 - sbar_m)/log K_m  ->  w_v, w_a  ->  M_v, M_a        (Eq.9-12)
+ *                   C^(l), B^(l) = Softmax(C/T)[l] (optional per-layer totals)              (Eq.13-14)
+ *   4. select       top-M_m of psi_k = a_k^lambda (1 - s_k) per (layer, KV head, modality)  (Eq.8)
+ *   5. compact      gather of the kept K/V rows into the fixed-budget cache
+ *
+ * Conventions
+ *   - All pointers are DEVICE pointers unless a comment says HOST.  The caller owns every buffer; the library
+ *     allocates no device memory after omnimem_create, frees nothing of the caller's and never synchronises the host
+ *     (except omnimem_compress_chunk_host, see there).
+ *   - Every call enqueues work on `stream` (a cudaStream_t passed as void*) and returns at once.
+ *   - Return value: OMNIMEM_OK or a negative omnimem_status.  Argument errors are detected before any launch.
+ *     No C++ exception crosses this boundary.  There is no CPU fallback: on a device that is not sm_100
+ *     omnimem_create returns OMNIMEM_UNSUPPORTED.
+ *   - Layout of a cache (one per model, "two separate KV caches" of P:56-58 Eq.2 pooled in one buffer):
+ *     k, v are [L, Hkv, cache_cap, D] contiguous; for layer l rows [0, n_v[l]) are the visual cache, rows
+ *     [n_v[l], n[l]) the audio cache, the same for every KV head of the layer.
+ *   - Layout of a chunk: k, v are [L, Hkv, Nn, D], q is [L, Hq, Nn, D], Nn = Nn_v + Nn_a, visual rows first (R25).
+ *     Query head j reads KV head j / (Hq/Hkv) (R5).
+ *   - Logical key order seen by the attention of Eq.1/Eq.6 (ONE joint softmax, R2):
+ *     cached visual, cached audio, new visual, new audio.  Causal inside the chunk (R3): chunk key t is visible to
+ *     chunk query i iff t <= i; cached keys are visible to every query.
+ *   - Segment-local index t of modality m (the appended sequence K~_m of Eq.3, length K_m = n_m + Nn_m):
+ *     t < n_m -> cache row off_m + t (off_v = 0, off_a = n_v);  else chunk row coff_m + (t - n_m) (coff_v = 0,
+ *     coff_a = Nn_v).  Per-modality arrays are [L, Hkv, seg_cap_m] fp32 with seg_cap_m = cache_cap + max_chunk_m
+ *     (omnimem_seg_cap); entries at t >= K_m are unspecified.
+ */
+#ifndef OMNIMEM_H_
+#define OMNIMEM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define OMNIMEM_API __attribute__((visibility("default")))
+#else
+#define OMNIMEM_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  OMNIMEM_OK = 0,
+  OMNIMEM_INVALID_ARG = -1,        /* NULL where a pointer is required, negative size, aliasing dst == src ...  */
+  OMNIMEM_UNSUPPORTED = -2,        /* dtype / head_dim / device architecture not supported                        */
+  OMNIMEM_WORKSPACE_TOO_SMALL = -3,
+  OMNIMEM_CUDA_ERROR = -4,         /* details: omnimem_last_cuda_error                                           */
+  OMNIMEM_CAPACITY = -5            /* chunk larger than max_chunk_*, or budget larger than cache_cap              */
+} omnimem_status;
+
+enum { OMNIMEM_FP32 = 0, OMNIMEM_BF16 = 1 };
+
+typedef struct omnimem_ctx omnimem_ctx; /* opaque: config, device properties, TMA descriptors, timing events */
+
+typedef struct {
+  int32_t n_layers, n_q_heads, n_kv_heads; /* L, Hq, Hkv; Hq % Hkv == 0                                              */
+  int32_t head_dim;                        /* D in {64, 128}                                                         */
+  int32_t dtype;                           /* OMNIMEM_FP32 (SIMT fp32 path) or OMNIMEM_BF16 (tcgen05 path when D=128) */
+  int32_t cache_cap;                       /* rows per (layer, kv head) of each cache buffer (>= every budget)       */
+  int32_t max_chunk_v, max_chunk_a;        /* capacity of a chunk per modality                                       */
+  float softmax_scale;                     /* c of z = c <q,k>; 0 => 1/sqrt(head_dim) (R4)                           */
+  float lambda;                            /* Eq.8; paper default 0.02; 0 = cosine-only ablation     */
+  float ratio_r;                           /* Eq.11-12 prior visual:audio ratio; paper default 5             */
+  float temperature;                       /* Eq.14 T; paper default 0.2                                     */
+  int32_t budget_min, budget_max;          /* Eq.14 clamp [B_min, B_max]; 0,0 => no clamp                    */
+  int32_t causal;                          /* 1 = causal inside the chunk (R3, default), 0 = every key visible       */
+  int32_t sim_source;                      /* Eq.7 vectors: 0 = value rows (default), 1 = key rows            */
+  int32_t sim_stride_v, sim_stride_a;      /* neighbour distance of Eq.7 per modality; 1 = paper literal (R11)       */
+  int32_t score_path;                      /* 0 = auto (tcgen05 for bf16 D=128, SIMT otherwise), 1 = force SIMT      */
+} omnimem_config;
+
+typedef struct {     /* one pooled KV cache */
+  void* k;           /* [L, Hkv, cache_cap, D] dtype                                          */
+  void* v;           /* [L, Hkv, cache_cap, D] dtype                                          */
+  int32_t* n_v;      /* [L] visual rows valid per layer                                       */
+  int32_t* n;        /* [L] total rows valid per layer (visual + audio), n[l] <= cache_cap    */
+} omnimem_cache;
+
+typedef struct {     /* one chunk, modality-blocked */
+  const void* k;     /* [L, Hkv, Nn, D]                                                       */
+  const void* v;     /* [L, Hkv, Nn, D]                                                       */
+  const void* q;     /* [L, Hq, Nn, D]  queries = the chunk's tokens                          */
+  const float* lse;  /* optional [L, Hq, Nn]: natural-log LSE of the scaled, masked logits of Eq.1 as produced by the
+                        model's own attention forward; NULL => computed here (score pass 1)                        */
+  int32_t Nn_v, Nn_a; /* HOST ints: rows of each modality in this chunk                       */
+} omnimem_chunk;
+
+typedef struct {     /* outputs of the scoring stages; any pointer may be NULL except where noted */
+  float *a_v, *a_a;      /* Eq.6 importance per modality segment  [L, Hkv, seg_cap_m]  (required)  */
+  float *s_v, *s_a;      /* Eq.7 redundancy                                             (required)  */
+  float *psi_v, *psi_a;  /* Eq.8 score, fp32: the public array that selection consumes  (required)  */
+  float* lse_out;        /* [L, Hq, Nn] LSE computed by pass 1 (natural log) or NULL                */
+  float* row_entropy;    /* [L, Hq, Nn] -sum_k p ln p per query row (diagnostic, R16) or NULL       */
+  double* stats;         /* [L, 8]: Hn_v, Hn_a, sbar_v, sbar_a, C_v, C_a, Hn_all, sbar_all (required) */
+} omnimem_scores;
+
+/* ---- life cycle ---------------------------------------------------------------------------------------------- */
+/* HOST pointers.  Validates the config, queries the current CUDA device, creates timing events.  *out is set only
+ * on success.  Errors: INVALID_ARG (NULL, non-positive sizes, Hq % Hkv != 0, strides < 1), UNSUPPORTED (dtype,
+ * head_dim, device is not compute capability 10.x), CUDA_ERROR. */
+OMNIMEM_API int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out);
+OMNIMEM_API int omnimem_destroy(omnimem_ctx* ctx);
+/* Bytes of device scratch every call below needs at this ctx's capacities; the caller allocates it once
+ * (256-byte aligned) and passes it to each call.  Contents need not persist between calls. */
+OMNIMEM_API size_t omnimem_workspace_bytes(const omnimem_ctx* ctx);
+/* Row stride of the per-modality arrays: cache_cap + max_chunk_m (m = 0 visual, 1 audio). */
+OMNIMEM_API int32_t omnimem_seg_cap(const omnimem_ctx* ctx, int32_t modality);
+OMNIMEM_API const char* omnimem_strerror(int status);              /* static string                                     */
+OMNIMEM_API const char* omnimem_last_cuda_error(const omnimem_ctx* ctx); /* cudaGetErrorString of the last CUDA failure  */
+
+/* ---- stage 1-3a: importance, redundancy, psi, AVBA statistics (Eq.6-10, Eq.13) ------------------------------- */
+/* src, chunk, out: HOST structs holding DEVICE pointers.  Launches: [LSE pass unless chunk->lse] -> column-sum pass
+ * -> cosine pass -> finalize (psi, partial statistics) -> statistics.  Errors: INVALID_ARG, CAPACITY (Nn_v > max_chunk_v,
+ * Nn_a > max_chunk_a), WORKSPACE_TOO_SMALL, CUDA_ERROR.  An empty chunk (Nn = 0) yields a = 0 and stats from s only. */
+OMNIMEM_API int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, omnimem_scores* out,
+                  void* ws, size_t ws_bytes, void* stream);
+
+/* ---- stage 3b: budgets (Eq.11-12; Eq.13-14 when layer_budget == NULL) ---------------------------------------- */
+/* stats [L,8] as written by omnimem_score; n_v, n [L]; layer_budget [L] int32 per-layer totals B^(l) (the paper
+ * fixes them offline) or NULL => B^(l) = Softmax_l(C^(l)/T) * total_budget, clamped to [budget_min,
+ * budget_max], integerised by largest remainder (R19, R20).  Out: M_v, M_a [L] with M_v + M_a = min(B^(l), K_v + K_a),
+ * M_m <= K_m (R22); layer_budget_out [L] or NULL receives the totals used. */
+OMNIMEM_API int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const int32_t* n_v, const int32_t* n, int32_t Nn_v,
+                     int32_t Nn_a, const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
+                     int32_t* layer_budget_out, void* stream);
+
+/* ---- stage 4: segmented top-M (Eq.4-5) ---------------------------------------------------------------- */
+/* psi_m [L, Hkv, seg_cap_m] fp32 (finite); per (l, h, m) writes the segment-local indices of the M_m[l] largest
+ * psi to idx_m[l, h, 0:M_m[l]) in ASCENDING index order; among equal psi the lowest index wins (R23).
+ * idx_m are [L, Hkv, cache_cap] int32; entries at >= M_m[l] are left untouched. */
+OMNIMEM_API int omnimem_select(omnimem_ctx* ctx, const float* psi_v, const float* psi_a, const int32_t* n_v, const int32_t* n,
+                   int32_t Nn_v, int32_t Nn_a, const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a,
+                   void* ws, size_t ws_bytes, void* stream);
+
+/* ---- stage 5: prune / gather-compaction ---------------------------------------------------------- */
+/* dst[l,h,0:M_v] = visual rows idx_v, dst[l,h,M_v:M_v+M_a] = audio rows idx_a, K and V, byte-exact;
+ * dst->n_v[l] = M_v[l], dst->n[l] = M_v[l] + M_a[l].  dst buffers must not alias src's (INVALID_ARG if
+ * dst->k == src->k or dst->v == src->v): the caller ping-pongs two caches. */
+OMNIMEM_API int omnimem_compact(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* idx_v,
+                    const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a, omnimem_cache* dst, void* stream);
+
+/* ---- the fused step: stages 1-5 for all layers, one stream, no host synchronisation ------------------------------- */
+/* layer_budget [L] device int32 (required).  opt_out NULL => scores live in ws; opt_idx_* NULL => indices live in ws.
+ * opt_M_v / opt_M_a [L] or NULL.  When opt_out is NULL, layers with nothing to evict (n[l] + Nn <= layer_budget[l])
+ * skip the scoring passes: their rows are appended unchanged. */
+OMNIMEM_API int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk,
+                           const int32_t* layer_budget, omnimem_cache* dst, omnimem_scores* opt_out,
+                           int32_t* opt_idx_v, int32_t* opt_idx_a, int32_t* opt_M_v, int32_t* opt_M_a, void* ws,
+                           size_t ws_bytes, void* stream);
+
+/* ---- the fused step fed from HOST memory (end-to-end entry) --------------------------------------------------- */
+/* host_chunk->k/v/q (and ->lse if non-NULL) are HOST pointers (pinned memory for full copy speed) with the chunk
+ * layout above; dev_chunk holds DEVICE staging buffers of the same shapes (caller-owned).  Copies the chunk to the
+ * device, runs omnimem_compress_chunk, copies M_v, M_a (and dst n_v, n) back to the HOST arrays host_M_v, host_M_a
+ * [L] (pinned) and synchronises `stream` before returning.  Returns the byte counts moved through
+ * h2d_bytes / d2h_bytes (HOST, may be NULL). */
+OMNIMEM_API int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
+                                const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,
+                                int32_t* host_M_v, int32_t* host_M_a, int64_t* h2d_bytes, int64_t* d2h_bytes,
+                                void* ws, size_t ws_bytes, void* stream);
+
+/* ---- per-stage device timing (CUDA events on `stream`, recorded inside the calls above when enabled) ---------- */
+enum {
+  OMNIMEM_STAGE_LSE = 0,      /* score pass 1 */
+  OMNIMEM_STAGE_COLSUM = 1,   /* score pass 2 */
+  OMNIMEM_STAGE_COSINE = 2,
+  OMNIMEM_STAGE_FINALIZE = 3, /* psi + statistics */
+  OMNIMEM_STAGE_ALLOCATE = 4,
+  OMNIMEM_STAGE_SELECT = 5,
+  OMNIMEM_STAGE_COMPACT = 6,
+  OMNIMEM_N_STAGES = 7
+};
+OMNIMEM_API int omnimem_set_profiling(omnimem_ctx* ctx, int32_t enabled);
+/* HOST out[OMNIMEM_N_STAGES]: milliseconds of each stage in the most recent call (0 for stages that did not run);
+ * synchronises on the recorded events.  launches_out (HOST, may be NULL): kernels launched by that call. */
+OMNIMEM_API int omnimem_get_stage_ms(omnimem_ctx* ctx, float* out, int32_t* launches_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OMNIMEM_H_ */

@@ -275,8 +275,9 @@ int omnimem_ref_stats(const omnimem_ref_params* p, const int32_t* n_v, const int
 
 /* ---- O6b: per-layer totals (Eq.13-14) -- PARITY UNPINNED beyond invariants (R19, R20) ----
  * C^(l) = Hn_all (1 - sbar_all); pi = softmax_l(C/T); b_l = pi_l * total.
- * Clamp to [B_min,B_max] (if budget_max > 0): layers outside the range are fixed at the bound and the
- * remaining total is re-split over the free layers in proportion to pi, until nothing moves.
+ * Clamp to [B_min,B_max] (if budget_max > 0): layers beyond the bound on the side with the larger total violation
+ * are fixed at that bound and the remaining total is re-split over the free layers in proportion to pi, until
+ * nothing moves (so that sum_l B^(l) = total whenever L*B_min <= total <= L*B_max).
  * Integerise by largest remainder, ties -> lowest layer, never above B_max.  If the clamps make the
  * total unreachable every layer sits at the nearer bound. */
 int omnimem_ref_layer_budgets(const omnimem_ref_params* p, const double* stats, int64_t total,
@@ -306,11 +307,17 @@ int omnimem_ref_layer_budgets(const omnimem_ref_params* p, const double* stats, 
         else pfree += pi[l];
       }
       int moved = 0;
+      double below = 0.0, above = 0.0;
       for (int l = 0; l < L; ++l)
-        if (!fixed[l]) b[l] = pfree > 0.0 ? rem * pi[l] / pfree : 0.0;
+        if (!fixed[l]) {
+          b[l] = pfree > 0.0 ? rem * pi[l] / pfree : 0.0;
+          if (b[l] < lo) below += lo - b[l];
+          if (b[l] > hi) above += b[l] - hi;
+        }
+      /* fix only the side that violates more: fixing both at once could strand budget (sum invariant, R20) */
       for (int l = 0; l < L; ++l)
-        if (!fixed[l] && (b[l] < lo || b[l] > hi)) {
-          b[l] = b[l] < lo ? lo : hi;
+        if (!fixed[l] && ((above >= below && b[l] > hi) || (above < below && b[l] < lo))) {
+          b[l] = above >= below ? hi : lo;
           fixed[l] = 1;
           moved = 1;
         }

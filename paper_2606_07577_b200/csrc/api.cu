@@ -1,0 +1,396 @@
+// C ABI of the OmniMem compression step (include/omnimem.h): context, validation, workspace carving, launch order.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "common.cuh"
+
+using namespace omnimem;
+
+namespace {
+
+struct WsLayout {
+  size_t lse, cosn, partials, a_v, a_a, s_v, s_a, psi_v, psi_a, stats, M_v, M_a, idx_v, idx_a, total;
+};
+
+size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+WsLayout ws_layout(const omnimem_ctx* c) {
+  const omnimem_config& g = c->cfg;
+  const size_t L = g.n_layers, Hq = g.n_q_heads, Hkv = g.n_kv_heads;
+  const size_t Nn = (size_t)g.max_chunk_v + g.max_chunk_a;
+  WsLayout w{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  w.lse = take(L * Hq * ((Nn + 127) / 128 * 128) * sizeof(float));
+  w.cosn = take(L * Hkv * ((size_t)c->seg_cap_v + c->seg_cap_a) * sizeof(float));
+  w.partials = take(L * 2 * (size_t)c->fin_blocks * 3 * sizeof(double));
+  w.a_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
+  w.a_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
+  w.s_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
+  w.s_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
+  w.psi_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
+  w.psi_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
+  w.stats = take(L * 8 * sizeof(double));
+  w.M_v = take(L * sizeof(int32_t));
+  w.M_a = take(L * sizeof(int32_t));
+  w.idx_v = take(L * Hkv * (size_t)g.cache_cap * sizeof(int32_t));
+  w.idx_a = take(L * Hkv * (size_t)g.cache_cap * sizeof(int32_t));
+  w.total = off;
+  return w;
+}
+
+int fail_cuda(omnimem_ctx* c, cudaError_t e) {
+  c->last_err = e;
+  return OMNIMEM_CUDA_ERROR;
+}
+
+StepParams make_params(const omnimem_ctx* c, int Nn_v, int Nn_a, const int32_t* n_v, const int32_t* n,
+                       const int32_t* skip_budget) {
+  const omnimem_config& g = c->cfg;
+  StepParams p{};
+  p.L = g.n_layers; p.Hq = g.n_q_heads; p.Hkv = g.n_kv_heads; p.G = g.n_q_heads / g.n_kv_heads; p.D = g.head_dim;
+  p.cache_cap = g.cache_cap;
+  p.Nn_v = Nn_v; p.Nn_a = Nn_a; p.Nn = Nn_v + Nn_a;
+  p.seg_cap_v = c->seg_cap_v; p.seg_cap_a = c->seg_cap_a;
+  p.causal = g.causal;
+  p.stride_v = g.sim_stride_v; p.stride_a = g.sim_stride_a;
+  p.scale = c->scale;
+  p.scale_log2e = (float)((double)c->scale * 1.4426950408889634);
+  p.lambda = g.lambda;
+  p.n_v = n_v; p.n = n; p.skip_budget = skip_budget;
+  return p;
+}
+
+int check_chunk(const omnimem_ctx* c, const omnimem_chunk* ch, bool need_q) {
+  if (!ch) return OMNIMEM_INVALID_ARG;
+  if (ch->Nn_v < 0 || ch->Nn_a < 0) return OMNIMEM_INVALID_ARG;
+  if (ch->Nn_v > c->cfg.max_chunk_v || ch->Nn_a > c->cfg.max_chunk_a) return OMNIMEM_CAPACITY;
+  if (ch->Nn_v + ch->Nn_a > 0 && (!ch->k || !ch->v || (need_q && !ch->q))) return OMNIMEM_INVALID_ARG;
+  return OMNIMEM_OK;
+}
+int check_cache(const omnimem_cache* ca) {
+  return (ca && ca->k && ca->v && ca->n_v && ca->n) ? OMNIMEM_OK : OMNIMEM_INVALID_ARG;
+}
+
+struct StageTimer {
+  omnimem_ctx* c;
+  cudaStream_t st;
+  int stage;
+  StageTimer(omnimem_ctx* c_, cudaStream_t st_, int stage_) : c(c_), st(st_), stage(stage_) {
+    if (c->profiling) { cudaEventRecord(c->ev[2 * stage], st); c->ev_used[stage] = true; }
+  }
+  ~StageTimer() { if (c->profiling) cudaEventRecord(c->ev[2 * stage + 1], st); }
+};
+
+void begin_call(omnimem_ctx* c) {
+  c->launches = 0;
+  for (int s = 0; s < OMNIMEM_N_STAGES; ++s) c->ev_used[s] = false;
+}
+
+// stages 1-3a on already validated arguments
+int run_score(omnimem_ctx* c, const StepParams& p, StepBuffers& b, cudaStream_t st) {
+  cudaError_t e;
+  if (p.Nn > 0 && b.lse_in == nullptr) {
+    StageTimer t(c, st, OMNIMEM_STAGE_LSE);
+    e = c->use_tc ? launch_lse_tc(c, p, b, st, &c->launches) : launch_lse_simt(c, p, b, st, &c->launches);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+  }
+  {
+    StageTimer t(c, st, OMNIMEM_STAGE_COLSUM);
+    e = c->use_tc ? launch_colsum_tc(c, p, b, st, &c->launches) : launch_colsum_simt(c, p, b, st, &c->launches);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+  }
+  {
+    StageTimer t(c, st, OMNIMEM_STAGE_COSINE);
+    e = launch_cosine(c, p, b, st, &c->launches);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+  }
+  {
+    StageTimer t(c, st, OMNIMEM_STAGE_FINALIZE);
+    e = launch_finalize(c, p, b, st, &c->launches);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+  }
+  return OMNIMEM_OK;
+}
+
+void fill_buffers(const omnimem_ctx* c, const omnimem_cache* src, const omnimem_chunk* ch, const omnimem_scores* out,
+                  uint8_t* ws, const WsLayout& w, StepBuffers& b) {
+  b.cacheK = src->k; b.cacheV = src->v; b.chunkK = ch->k; b.chunkV = ch->v; b.Q = ch->q;
+  b.lse_in = ch->lse;
+  b.lse_out = out ? out->lse_out : nullptr;
+  b.lse = ch->lse ? const_cast<float*>(ch->lse) : (b.lse_out ? b.lse_out : (float*)(ws + w.lse));
+  b.lse2 = (float*)(ws + w.lse);
+  b.row_entropy = out ? out->row_entropy : nullptr;
+  b.a_v = out ? out->a_v : (float*)(ws + w.a_v);
+  b.a_a = out ? out->a_a : (float*)(ws + w.a_a);
+  b.s_v = out ? out->s_v : (float*)(ws + w.s_v);
+  b.s_a = out ? out->s_a : (float*)(ws + w.s_a);
+  b.psi_v = out ? out->psi_v : (float*)(ws + w.psi_v);
+  b.psi_a = out ? out->psi_a : (float*)(ws + w.psi_a);
+  b.cosn = (float*)(ws + w.cosn);
+  b.partials = (double*)(ws + w.partials);
+  b.stats = out ? out->stats : (double*)(ws + w.stats);
+}
+
+int check_scores(const omnimem_scores* o) {
+  return (o->a_v && o->a_a && o->s_v && o->s_a && o->psi_v && o->psi_a && o->stats) ? OMNIMEM_OK : OMNIMEM_INVALID_ARG;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* omnimem_strerror(int status) {
+  switch (status) {
+    case OMNIMEM_OK: return "ok";
+    case OMNIMEM_INVALID_ARG: return "invalid argument";
+    case OMNIMEM_UNSUPPORTED: return "unsupported dtype, head_dim or device (needs sm_100)";
+    case OMNIMEM_WORKSPACE_TOO_SMALL: return "workspace too small (see omnimem_workspace_bytes)";
+    case OMNIMEM_CUDA_ERROR: return "CUDA error (see omnimem_last_cuda_error)";
+    case OMNIMEM_CAPACITY: return "chunk or budget exceeds the context capacities";
+    default: return "unknown status";
+  }
+}
+
+int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
+  if (!cfg || !out) return OMNIMEM_INVALID_ARG;
+  const omnimem_config& g = *cfg;
+  if (g.n_layers <= 0 || g.n_q_heads <= 0 || g.n_kv_heads <= 0 || g.cache_cap <= 0 || g.max_chunk_v < 0 ||
+      g.max_chunk_a < 0 || g.n_q_heads % g.n_kv_heads != 0 || g.sim_stride_v < 1 || g.sim_stride_a < 1 ||
+      g.softmax_scale < 0.f || g.lambda < 0.f || g.ratio_r <= 0.f || g.temperature <= 0.f || g.budget_min < 0 ||
+      g.budget_max < g.budget_min || (g.sim_source != 0 && g.sim_source != 1) || g.n_kv_heads > 65535)
+    return OMNIMEM_INVALID_ARG;
+  if (g.dtype != OMNIMEM_FP32 && g.dtype != OMNIMEM_BF16) return OMNIMEM_UNSUPPORTED;
+  if (g.head_dim != 64 && g.head_dim != 128) return OMNIMEM_UNSUPPORTED;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return OMNIMEM_CUDA_ERROR;
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return OMNIMEM_CUDA_ERROR;
+  if (prop.major != 10) return OMNIMEM_UNSUPPORTED;  // no fallback: this library is sm_100a code only
+  omnimem_ctx* c = new (std::nothrow) omnimem_ctx();
+  if (!c) return OMNIMEM_INVALID_ARG;
+  c->cfg = g;
+  c->device = dev;
+  c->sm_count = prop.multiProcessorCount;
+  c->cc_major = prop.major;
+  c->cc_minor = prop.minor;
+  c->seg_cap_v = g.cache_cap + g.max_chunk_v;
+  c->seg_cap_a = g.cache_cap + g.max_chunk_a;
+  const int mx = c->seg_cap_v > c->seg_cap_a ? c->seg_cap_v : c->seg_cap_a;
+  c->fin_blocks = (mx + 255) / 256;
+  c->scale = g.softmax_scale > 0.f ? g.softmax_scale : (float)(1.0 / sqrt((double)g.head_dim));
+  c->use_tc = g.dtype == OMNIMEM_BF16 && g.head_dim == 128 && g.score_path == 0;
+  c->last_err = cudaSuccess;
+  c->profiling = false;
+  c->launches = 0;
+  c->encode_tiled = nullptr;
+  for (int i = 0; i < 2 * OMNIMEM_N_STAGES; ++i) {
+    e = cudaEventCreate(&c->ev[i]);
+    if (e != cudaSuccess) { delete c; return OMNIMEM_CUDA_ERROR; }
+  }
+  for (int s = 0; s < OMNIMEM_N_STAGES; ++s) c->ev_used[s] = false;
+  *out = c;
+  return OMNIMEM_OK;
+}
+
+int omnimem_destroy(omnimem_ctx* ctx) {
+  if (!ctx) return OMNIMEM_INVALID_ARG;
+  for (int i = 0; i < 2 * OMNIMEM_N_STAGES; ++i) cudaEventDestroy(ctx->ev[i]);
+  delete ctx;
+  return OMNIMEM_OK;
+}
+
+size_t omnimem_workspace_bytes(const omnimem_ctx* ctx) { return ctx ? ws_layout(ctx).total : 0; }
+
+int32_t omnimem_seg_cap(const omnimem_ctx* ctx, int32_t modality) {
+  if (!ctx) return 0;
+  return modality == 0 ? ctx->seg_cap_v : ctx->seg_cap_a;
+}
+
+const char* omnimem_last_cuda_error(const omnimem_ctx* ctx) {
+  return ctx ? cudaGetErrorString(ctx->last_err) : "no context";
+}
+
+int omnimem_set_profiling(omnimem_ctx* ctx, int32_t enabled) {
+  if (!ctx) return OMNIMEM_INVALID_ARG;
+  ctx->profiling = enabled != 0;
+  return OMNIMEM_OK;
+}
+
+int omnimem_get_stage_ms(omnimem_ctx* ctx, float* out, int32_t* launches_out) {
+  if (!ctx || !out) return OMNIMEM_INVALID_ARG;
+  for (int s = 0; s < OMNIMEM_N_STAGES; ++s) {
+    out[s] = 0.f;
+    if (ctx->profiling && ctx->ev_used[s]) {
+      cudaError_t e = cudaEventSynchronize(ctx->ev[2 * s + 1]);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&out[s], ctx->ev[2 * s], ctx->ev[2 * s + 1]);
+      if (e != cudaSuccess) return fail_cuda(ctx, e);
+    }
+  }
+  if (launches_out) *launches_out = ctx->launches;
+  return OMNIMEM_OK;
+}
+
+int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, omnimem_scores* out, void* ws,
+                  size_t ws_bytes, void* stream) {
+  if (!ctx || !out || !ws) return OMNIMEM_INVALID_ARG;
+  int rc = check_cache(src);
+  if (rc) return rc;
+  rc = check_chunk(ctx, chunk, true);
+  if (rc) return rc;
+  rc = check_scores(out);
+  if (rc) return rc;
+  const WsLayout w = ws_layout(ctx);
+  if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
+  begin_call(ctx);
+  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
+  StepBuffers b{};
+  fill_buffers(ctx, src, chunk, out, (uint8_t*)ws, w, b);
+  return run_score(ctx, p, b, (cudaStream_t)stream);
+}
+
+int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const int32_t* n_v, const int32_t* n, int32_t Nn_v,
+                     int32_t Nn_a, const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
+                     int32_t* layer_budget_out, void* stream) {
+  if (!ctx || !stats || !n_v || !n || !M_v || !M_a || Nn_v < 0 || Nn_a < 0) return OMNIMEM_INVALID_ARG;
+  if (!layer_budget && total_budget < 0) return OMNIMEM_INVALID_ARG;
+  if (Nn_v > ctx->cfg.max_chunk_v || Nn_a > ctx->cfg.max_chunk_a) return OMNIMEM_CAPACITY;
+  begin_call(ctx);
+  StepParams p = make_params(ctx, Nn_v, Nn_a, n_v, n, nullptr);
+  StageTimer t(ctx, (cudaStream_t)stream, OMNIMEM_STAGE_ALLOCATE);
+  cudaError_t e = launch_allocate(ctx, p, stats, layer_budget, total_budget, M_v, M_a, layer_budget_out,
+                                  (cudaStream_t)stream, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
+int omnimem_select(omnimem_ctx* ctx, const float* psi_v, const float* psi_a, const int32_t* n_v, const int32_t* n,
+                   int32_t Nn_v, int32_t Nn_a, const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a,
+                   void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (!ctx || !psi_v || !psi_a || !n_v || !n || !M_v || !M_a || !idx_v || !idx_a || Nn_v < 0 || Nn_a < 0)
+    return OMNIMEM_INVALID_ARG;
+  if (Nn_v > ctx->cfg.max_chunk_v || Nn_a > ctx->cfg.max_chunk_a) return OMNIMEM_CAPACITY;
+  begin_call(ctx);
+  StepParams p = make_params(ctx, Nn_v, Nn_a, n_v, n, nullptr);
+  StageTimer t(ctx, (cudaStream_t)stream, OMNIMEM_STAGE_SELECT);
+  cudaError_t e = launch_select(ctx, p, psi_v, psi_a, M_v, M_a, idx_v, idx_a, (cudaStream_t)stream, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
+int omnimem_compact(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* idx_v,
+                    const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a, omnimem_cache* dst, void* stream) {
+  if (!ctx || !idx_v || !idx_a || !M_v || !M_a) return OMNIMEM_INVALID_ARG;
+  int rc = check_cache(src);
+  if (rc) return rc;
+  rc = check_cache(dst);
+  if (rc) return rc;
+  rc = check_chunk(ctx, chunk, false);
+  if (rc) return rc;
+  if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
+  begin_call(ctx);
+  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
+  StageTimer t(ctx, (cudaStream_t)stream, OMNIMEM_STAGE_COMPACT);
+  cudaError_t e = launch_compact(ctx, p, src->k, src->v, chunk->k, chunk->v, idx_v, idx_a, M_v, M_a, dst->k, dst->v,
+                                 dst->n_v, dst->n, (cudaStream_t)stream, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
+int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk,
+                           const int32_t* layer_budget, omnimem_cache* dst, omnimem_scores* opt_out, int32_t* opt_idx_v,
+                           int32_t* opt_idx_a, int32_t* opt_M_v, int32_t* opt_M_a, void* ws, size_t ws_bytes,
+                           void* stream) {
+  if (!ctx || !layer_budget || !ws) return OMNIMEM_INVALID_ARG;
+  int rc = check_cache(src);
+  if (rc) return rc;
+  rc = check_cache(dst);
+  if (rc) return rc;
+  rc = check_chunk(ctx, chunk, true);
+  if (rc) return rc;
+  if (opt_out && (rc = check_scores(opt_out))) return rc;
+  if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
+  const WsLayout w = ws_layout(ctx);
+  if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = (cudaStream_t)stream;
+  uint8_t* wsb = (uint8_t*)ws;
+  begin_call(ctx);
+  // layers with nothing to evict skip scoring unless the caller asked for the scores
+  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, opt_out ? nullptr : layer_budget);
+  StepBuffers b{};
+  fill_buffers(ctx, src, chunk, opt_out, wsb, w, b);
+  rc = run_score(ctx, p, b, st);
+  if (rc) return rc;
+  int32_t* M_v = opt_M_v ? opt_M_v : (int32_t*)(wsb + w.M_v);
+  int32_t* M_a = opt_M_a ? opt_M_a : (int32_t*)(wsb + w.M_a);
+  int32_t* idx_v = opt_idx_v ? opt_idx_v : (int32_t*)(wsb + w.idx_v);
+  int32_t* idx_a = opt_idx_a ? opt_idx_a : (int32_t*)(wsb + w.idx_a);
+  cudaError_t e;
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_ALLOCATE);
+    e = launch_allocate(ctx, p, b.stats, layer_budget, 0, M_v, M_a, nullptr, st, &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_SELECT);
+    e = launch_select(ctx, p, b.psi_v, b.psi_a, M_v, M_a, idx_v, idx_a, st, &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_COMPACT);
+    e = launch_compact(ctx, p, src->k, src->v, chunk->k, chunk->v, idx_v, idx_a, M_v, M_a, dst->k, dst->v, dst->n_v,
+                       dst->n, st, &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  return OMNIMEM_OK;
+}
+
+int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
+                                const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,
+                                int32_t* host_M_v, int32_t* host_M_a, int64_t* h2d_bytes, int64_t* d2h_bytes, void* ws,
+                                size_t ws_bytes, void* stream) {
+  if (!ctx || !host_chunk || !dev_chunk || !host_M_v || !host_M_a || !ws) return OMNIMEM_INVALID_ARG;
+  int rc = check_chunk(ctx, host_chunk, true);
+  if (rc) return rc;
+  if (!dev_chunk->k || !dev_chunk->v || !dev_chunk->q || (host_chunk->lse && !dev_chunk->lse)) return OMNIMEM_INVALID_ARG;
+  const WsLayout w = ws_layout(ctx);
+  if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const omnimem_config& g = ctx->cfg;
+  const size_t es = g.dtype == OMNIMEM_FP32 ? 4 : 2;
+  const size_t Nn = (size_t)host_chunk->Nn_v + host_chunk->Nn_a;
+  const size_t kv_bytes = (size_t)g.n_layers * g.n_kv_heads * Nn * g.head_dim * es;
+  const size_t q_bytes = (size_t)g.n_layers * g.n_q_heads * Nn * g.head_dim * es;
+  const size_t lse_bytes = host_chunk->lse ? (size_t)g.n_layers * g.n_q_heads * Nn * sizeof(float) : 0;
+  cudaError_t e = cudaSuccess;
+  if (Nn > 0) {
+    e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->k), host_chunk->k, kv_bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->v), host_chunk->v, kv_bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->q), host_chunk->q, q_bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && lse_bytes)
+      e = cudaMemcpyAsync(const_cast<float*>(dev_chunk->lse), host_chunk->lse, lse_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  omnimem_chunk ch = *dev_chunk;
+  ch.Nn_v = host_chunk->Nn_v;
+  ch.Nn_a = host_chunk->Nn_a;
+  if (!host_chunk->lse) ch.lse = nullptr;
+  uint8_t* wsb = (uint8_t*)ws;
+  int32_t* M_v = (int32_t*)(wsb + w.M_v);
+  int32_t* M_a = (int32_t*)(wsb + w.M_a);
+  rc = omnimem_compress_chunk(ctx, src, &ch, layer_budget, dst, nullptr, nullptr, nullptr, M_v, M_a, ws, ws_bytes, stream);
+  if (rc) return rc;
+  const size_t mb = (size_t)g.n_layers * sizeof(int32_t);
+  e = cudaMemcpyAsync(host_M_v, M_v, mb, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(host_M_a, M_a, mb, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail_cuda(ctx, e);
+  if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? 2 * kv_bytes + q_bytes + lse_bytes : 0);
+  if (d2h_bytes) *d2h_bytes = (int64_t)(2 * mb);
+  return OMNIMEM_OK;
+}
+
+}  // extern "C"

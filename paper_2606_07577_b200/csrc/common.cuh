@@ -1,0 +1,109 @@
+// Shared declarations of the CUDA path (host context, kernel parameter block, segment maps).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/omnimem.h"
+
+namespace omnimem {
+
+// Kernel parameter block (by value).  Names follow include/omnimem.h and the paper's notation.
+struct StepParams {
+  int L, Hq, Hkv, G, D;
+  int cache_cap;
+  int Nn_v, Nn_a, Nn;        // this chunk
+  int seg_cap_v, seg_cap_a;  // row strides of the per-modality arrays
+  int causal;
+  int stride_v, stride_a;    // Eq.7 neighbour distance per modality
+  float scale;               // c
+  float scale_log2e;         // c * log2(e)
+  float lambda;
+  // device state
+  const int32_t* n_v;        // [L]
+  const int32_t* n;          // [L]
+  const int32_t* skip_budget;  // [L] or nullptr: layers with n[l] + Nn <= skip_budget[l] skip scoring
+};
+
+// Segment maps (include/omnimem.h "Conventions"; Eq.3 appended sequences).
+__host__ __device__ __forceinline__ int seg_len(const StepParams& p, int n_v, int n, int m) {
+  return m == 0 ? n_v + p.Nn_v : (n - n_v) + p.Nn_a;
+}
+// segment-local t -> row in cache (in_chunk = false) or chunk (in_chunk = true)
+__device__ __forceinline__ int seg_row(const StepParams& p, int n_v, int n, int m, int t, bool& in_chunk) {
+  const int n_m = m == 0 ? n_v : n - n_v;
+  if (t < n_m) {
+    in_chunk = false;
+    return (m == 0 ? 0 : n_v) + t;
+  }
+  in_chunk = true;
+  return (m == 0 ? 0 : p.Nn_v) + (t - n_m);
+}
+// logical key (cache row r < n, or chunk row) -> (modality, segment-local index)
+__device__ __forceinline__ void cache_row_to_seg(int n_v, int r, int& m, int& t) {
+  if (r < n_v) { m = 0; t = r; } else { m = 1; t = r - n_v; }
+}
+__device__ __forceinline__ void chunk_row_to_seg(const StepParams& p, int n_v, int n, int r, int& m, int& t) {
+  if (r < p.Nn_v) { m = 0; t = n_v + r; } else { m = 1; t = (n - n_v) + (r - p.Nn_v); }
+}
+__device__ __forceinline__ bool layer_skips_scoring(const StepParams& p, int l) {
+  return p.skip_budget != nullptr && p.n[l] + p.Nn <= p.skip_budget[l];
+}
+
+// Buffers of one step (device pointers).
+struct StepBuffers {
+  const void *cacheK, *cacheV, *chunkK, *chunkV, *Q;
+  const float* lse_in;   // caller-supplied natural-log LSE [L,Hq,Nn] or nullptr
+  float* lse;            // SIMT path: natural-log LSE read by pass 2 (== lse_in when supplied)
+  float* lse2;           // tcgen05 path: internal log2-domain LSE, rows padded to a multiple of 128
+  float* lse_out;        // caller's natural-log output or nullptr
+  float* row_entropy;    // or nullptr
+  float *a_v, *a_a, *s_v, *s_a, *psi_v, *psi_a;
+  float* cosn;           // [L,Hkv,seg_cap_v+seg_cap_a]: cos(x_t, x_{t+sigma})
+  double* partials;      // [L][2][nblk][3]
+  double* stats;         // [L,8]
+};
+
+struct TmaMaps;  // score_tc.cu
+
+}  // namespace omnimem
+
+struct omnimem_ctx {
+  omnimem_config cfg;
+  int device;
+  int sm_count;
+  int cc_major, cc_minor;
+  int seg_cap_v, seg_cap_a;
+  int fin_blocks;  // blocks per (layer, modality) of the finalize kernel
+  float scale;
+  bool use_tc;
+  cudaError_t last_err;
+  bool profiling;
+  cudaEvent_t ev[2 * OMNIMEM_N_STAGES];
+  bool ev_used[OMNIMEM_N_STAGES];
+  int launches;
+  void* encode_tiled;  // cuTensorMapEncodeTiled entry point
+};
+
+namespace omnimem {
+
+// launchers (each returns cudaGetLastError() after its launches; `launches` is incremented per kernel)
+cudaError_t launch_lse_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,
+                            int64_t total_budget, int32_t* M_v, int32_t* M_a, int32_t* layer_budget_out, cudaStream_t st,
+                            int* launches);
+cudaError_t launch_select(const omnimem_ctx* ctx, const StepParams& p, const float* psi_v, const float* psi_a,
+                          const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a, cudaStream_t st,
+                          int* launches);
+cudaError_t launch_compact(const omnimem_ctx* ctx, const StepParams& p, const void* srcK, const void* srcV,
+                           const void* chunkK, const void* chunkV, const int32_t* idx_v, const int32_t* idx_a,
+                           const int32_t* M_v, const int32_t* M_a, void* dstK, void* dstV, int32_t* dst_n_v,
+                           int32_t* dst_n, cudaStream_t st, int* launches);
+
+}  // namespace omnimem

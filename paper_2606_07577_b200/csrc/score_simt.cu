@@ -1,0 +1,186 @@
+// SIMT scoring kernels: score pass 1 (row LSE of Eq.1's softmax) and pass 2 (Eq.6 column sums).
+// Used for fp32 inputs (CFG1, 1e-5 tolerance: no tensor-core rounding allowed) and for bf16 shapes the
+// tcgen05 path does not cover (head_dim != 128).  One warp per query row (pass 1) / per key (pass 2).
+#include <math.h>
+
+#include "common.cuh"
+
+namespace omnimem {
+
+template <typename T> struct Vec16;
+template <> struct Vec16<float> {
+  static constexpr int N = 4;
+  __device__ static __forceinline__ void load(const float* p, float* o) {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+  }
+};
+template <> struct Vec16<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ static __forceinline__ void load(const __nv_bfloat16* p, float* o) {
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      o[2 * i] = __uint_as_float(w[i] << 16);
+      o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    }
+  }
+};
+__device__ __forceinline__ float to_float(float x) { return x; }
+__device__ __forceinline__ float to_float(__nv_bfloat16 x) { return __bfloat162float(x); }
+
+template <typename T>
+__device__ __forceinline__ float dot_row(const float* __restrict__ sx, const T* __restrict__ gy, int D) {
+  float acc = 0.f;
+  for (int d = 0; d < D; d += Vec16<T>::N) {
+    float y[Vec16<T>::N];
+    Vec16<T>::load(gy + d, y);
+#pragma unroll
+    for (int e = 0; e < Vec16<T>::N; ++e) acc = fmaf(sx[d + e], y[e], acc);
+  }
+  return acc;
+}
+
+// ---- pass 1: lse[l,j,i] = log sum_{k visible} exp(c <q_i, k_k>)   (softmax of P:54 Eq.1; needed by Eq.6) ----
+template <typename T, bool kEntropy>
+__global__ void __launch_bounds__(128) lse_simt_kernel(StepParams p, const T* __restrict__ cacheK,
+                                                       const T* __restrict__ chunkK, const T* __restrict__ Q,
+                                                       float* __restrict__ lse, float* __restrict__ rowH) {
+  extern __shared__ float sq[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long row = (long long)blockIdx.x * 4 + warp;
+  if (row >= (long long)p.L * p.Hq * p.Nn) return;
+  const int i = (int)(row % p.Nn);
+  const int j = (int)((row / p.Nn) % p.Hq);
+  const int l = (int)(row / ((long long)p.Nn * p.Hq));
+  if (layer_skips_scoring(p, l)) return;
+  const int h = j / p.G, D = p.D;
+  const T* q = Q + row * D;
+  float* myq = sq + warp * D;
+  for (int d = lane; d < D; d += 32) myq[d] = to_float(q[d]);
+  __syncwarp();
+  const int Nc = p.n[l];
+  const int nvis = p.causal ? Nc + i + 1 : Nc + p.Nn;
+  const T* kc = cacheK + (long long)(l * p.Hkv + h) * p.cache_cap * D;
+  const T* kn = chunkK + (long long)(l * p.Hkv + h) * p.Nn * D;
+  float m = -INFINITY, Z = 0.f, W = 0.f;
+  for (int k = lane; k < nvis; k += 32) {
+    const T* kr = k < Nc ? kc + (long long)k * D : kn + (long long)(k - Nc) * D;
+    const float z = p.scale * dot_row<T>(myq, kr, D);
+    if (z > m) {
+      const float r = expf(m - z);
+      Z = Z * r + 1.f;
+      if (kEntropy) W = W * r + z;
+      m = z;
+    } else {
+      const float e = expf(z - m);
+      Z += e;
+      if (kEntropy) W = fmaf(e, z, W);
+    }
+  }
+  float mm = m;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mm = fmaxf(mm, __shfl_xor_sync(0xffffffffu, mm, o));
+  const float r = (m == -INFINITY) ? 0.f : expf(m - mm);
+  Z *= r;
+  W *= r;
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    Z += __shfl_xor_sync(0xffffffffu, Z, o);
+    W += __shfl_xor_sync(0xffffffffu, W, o);
+  }
+  if (lane == 0) {
+    const float v = mm + logf(Z);
+    lse[row] = v;
+    if (kEntropy) rowH[row] = v - W / Z;  // -sum p ln p = lse - sum p z
+  }
+}
+
+// ---- pass 2: a[l,h,k] = sum_g sum_{i visible} exp(c <q_i, k_k> - lse[l,hG+g,i])   (Eq.6, R5) ----
+template <typename T>
+__global__ void __launch_bounds__(128) colsum_simt_kernel(StepParams p, const T* __restrict__ cacheK,
+                                                          const T* __restrict__ chunkK, const T* __restrict__ Q,
+                                                          const float* __restrict__ lse, float* __restrict__ a_v,
+                                                          float* __restrict__ a_a) {
+  extern __shared__ float sk[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int slots = p.cache_cap + p.Nn;  // logical key slots per (l,h): cache rows by capacity, then chunk rows
+  const long long item = (long long)blockIdx.x * 4 + warp;
+  if (item >= (long long)p.L * p.Hkv * slots) return;
+  const int kk = (int)(item % slots);
+  const int h = (int)((item / slots) % p.Hkv);
+  const int l = (int)(item / ((long long)slots * p.Hkv));
+  if (layer_skips_scoring(p, l)) return;
+  const int D = p.D, n_v = p.n_v[l], n = p.n[l];
+  int m, t, t_chunk = -1;
+  const T* kr;
+  if (kk < p.cache_cap) {
+    if (kk >= n) return;
+    kr = cacheK + ((long long)(l * p.Hkv + h) * p.cache_cap + kk) * D;
+    cache_row_to_seg(n_v, kk, m, t);
+  } else {
+    t_chunk = kk - p.cache_cap;
+    kr = chunkK + ((long long)(l * p.Hkv + h) * p.Nn + t_chunk) * D;
+    chunk_row_to_seg(p, n_v, n, t_chunk, m, t);
+  }
+  float* myk = sk + warp * D;
+  for (int d = lane; d < D; d += 32) myk[d] = to_float(kr[d]);
+  __syncwarp();
+  float acc = 0.f;
+  const int rows = p.G * p.Nn;
+  for (int rr = lane; rr < rows; rr += 32) {
+    const int g = rr / p.Nn, i = rr % p.Nn;
+    if (p.causal && t_chunk > i) continue;
+    const long long qrow = (long long)(l * p.Hq + h * p.G + g) * p.Nn + i;
+    const float z = p.scale * dot_row<T>(myk, Q + qrow * D, D);
+    acc += expf(z - lse[qrow]);
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) {
+    float* out = m == 0 ? a_v + (long long)(l * p.Hkv + h) * p.seg_cap_v : a_a + (long long)(l * p.Hkv + h) * p.seg_cap_a;
+    out[t] = acc;
+  }
+}
+
+template <typename T>
+static cudaError_t lse_simt_t(const StepParams& p, const StepBuffers& b, cudaStream_t st) {
+  const long long rows = (long long)p.L * p.Hq * p.Nn;
+  if (rows == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((rows + 3) / 4);
+  const size_t smem = 4 * p.D * sizeof(float);
+  if (b.row_entropy)
+    lse_simt_kernel<T, true><<<grid, 128, smem, st>>>(p, (const T*)b.cacheK, (const T*)b.chunkK, (const T*)b.Q, b.lse,
+                                                      b.row_entropy);
+  else
+    lse_simt_kernel<T, false><<<grid, 128, smem, st>>>(p, (const T*)b.cacheK, (const T*)b.chunkK, (const T*)b.Q, b.lse,
+                                                       nullptr);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_lse_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
+                            int* launches) {
+  if ((long long)p.L * p.Hq * p.Nn == 0) return cudaSuccess;
+  ++*launches;
+  return ctx->cfg.dtype == OMNIMEM_FP32 ? lse_simt_t<float>(p, b, st) : lse_simt_t<__nv_bfloat16>(p, b, st);
+}
+
+cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
+                               int* launches) {
+  const long long items = (long long)p.L * p.Hkv * (p.cache_cap + p.Nn);
+  if (items == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((items + 3) / 4);
+  const size_t smem = 4 * p.D * sizeof(float);
+  ++*launches;
+  if (ctx->cfg.dtype == OMNIMEM_FP32)
+    colsum_simt_kernel<float><<<grid, 128, smem, st>>>(p, (const float*)b.cacheK, (const float*)b.chunkK,
+                                                       (const float*)b.Q, b.lse, b.a_v, b.a_a);
+  else
+    colsum_simt_kernel<__nv_bfloat16><<<grid, 128, smem, st>>>(p, (const __nv_bfloat16*)b.cacheK,
+                                                               (const __nv_bfloat16*)b.chunkK,
+                                                               (const __nv_bfloat16*)b.Q, b.lse, b.a_v, b.a_a);
+  return cudaGetLastError();
+}
+
+}  // namespace omnimem

@@ -1,0 +1,504 @@
+// tcgen05 / TMEM / TMA scoring kernels for bf16, head_dim 128 (sm_100a only).
+//
+// Eq.6 needs the softmax row normaliser before the column sums, so the QK^T contraction runs twice:
+//   pass 1 (kPass == 1)  S  = Q K^T, M = 128 queries per sub-tile: each thread owns one query row of the TMEM
+//                        accumulator, keeps an online max / sum and writes lse2 = log2 sum_k 2^(c2 s_k).
+//   pass 2 (kPass == 2)  S^T = K Q^T, M = 128 keys per sub-tile: each thread owns one KEY row, the sum over
+//                        queries is thread-local: a_k = sum_{g,i} 2^(c2 s - lse2_i).  No atomics, no shuffles.
+// One CTA holds two stationary 128-row sub-tiles (A operand, 64 KB) and streams 128-row tiles of the other
+// operand (B, 32 KB stages) by TMA; one thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile) into a
+// double-buffered 128-column TMEM accumulator per sub-tile; two 4-warp softmax groups drain them with
+// tcgen05.ld 32x32b.  Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-7 / 8-11 = epilogue.
+#include <cuda.h>
+#include <math.h>
+
+#include "common.cuh"
+
+namespace omnimem {
+
+constexpr int kTile = 128;         // rows per operand tile (UMMA M and N)
+constexpr int kHeadDim = 128;      // D
+constexpr int kKBlock = 64;        // bf16 elements per 128-byte swizzle atom row
+constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16 KB K-blocks
+constexpr int kKBlockBytes = kTile * kKBlock * 2; // 16 KB
+constexpr int kStages = 4;
+constexpr int kThreads = 384;
+constexpr int kTmemCols = 512;
+constexpr size_t kSmemBytes = 1024 /*align slack*/ + 2 * kTileBytes + kStages * kTileBytes + 256 /*barriers*/;
+
+// ---- PTX wrappers -------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra WAIT_DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
+          "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc),
+      "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// UMMA shared-memory descriptor, K-major, 128-byte swizzle: 8-row groups are 1024 B apart (SBO), LBO unused,
+// descriptor version 1 (sm_100), layout type 2 (SWIZZLE_128B).
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
+  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)(1024u >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+// Instruction descriptor: D = f32 (bit 4), A = B = bf16 (bits 7, 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
+
+struct TcArgs {
+  StepParams p;
+  float* lse2;         // [L, Hq, lse_stride] log2-domain LSE (internal, padded rows hold +inf)
+  int lse_stride;
+  float* lse_nat;      // pass 1: optional natural-log output [L, Hq, Nn]
+  float* row_entropy;  // pass 1: optional [L, Hq, Nn]
+  float* a_v;          // pass 2 outputs
+  float* a_a;
+  int n_cache_pairs;   // pass 2: ceil(cache_cap / 256)
+};
+
+// What one CTA works on, computed identically by every role.
+struct Work {
+  int l, lhA;            // layer; outer TMA coordinate of the stationary operand
+  int rowA0;             // first row of sub-tile 0 in the stationary operand
+  bool a_chunk;          // pass 2: stationary keys come from the chunk (else cache)
+  bool sub_valid[2];
+  int ntiles;            // streamed tiles in this CTA's sequence
+  // pass 1
+  int n_cache_tiles, ntiles_sub[2], h;
+  // pass 2
+  int it0[2], tiles_per_g, hq0;
+};
+
+template <int kPass>
+__device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
+  const StepParams& p = a.p;
+  w.l = blockIdx.z;
+  if (layer_skips_scoring(p, w.l)) return false;
+  const int n = p.n[w.l];
+  if (kPass == 1) {
+    const int j = blockIdx.y;  // query head
+    w.h = j / p.G;
+    w.lhA = w.l * p.Hq + j;
+    w.rowA0 = blockIdx.x * 2 * kTile;
+    w.a_chunk = false;
+    w.n_cache_tiles = (n + kTile - 1) / kTile;
+    const int nct = (p.Nn + kTile - 1) / kTile;
+    w.ntiles = 0;
+    for (int s = 0; s < 2; ++s) {
+      const int r0 = w.rowA0 + s * kTile;
+      w.sub_valid[s] = r0 < p.Nn;
+      const int nc = p.causal ? min(nct, r0 / kTile + 1) : nct;  // R3: chunk key t visible iff t <= i
+      w.ntiles_sub[s] = w.sub_valid[s] ? w.n_cache_tiles + nc : 0;
+      w.ntiles = max(w.ntiles, w.ntiles_sub[s]);
+    }
+    return w.sub_valid[0];
+  } else {
+    const int h = blockIdx.y;  // KV head
+    w.h = h;
+    w.lhA = w.l * p.Hkv + h;
+    w.hq0 = w.l * p.Hq + h * p.G;
+    int valid_rows;
+    if ((int)blockIdx.x < a.n_cache_pairs) {
+      w.a_chunk = false;
+      w.rowA0 = blockIdx.x * 2 * kTile;
+      valid_rows = n;
+    } else {
+      w.a_chunk = true;
+      w.rowA0 = (blockIdx.x - a.n_cache_pairs) * 2 * kTile;
+      valid_rows = p.Nn;
+    }
+    const int nqt = (p.Nn + kTile - 1) / kTile;
+    for (int s = 0; s < 2; ++s) {
+      const int r0 = w.rowA0 + s * kTile;
+      w.sub_valid[s] = r0 < valid_rows;
+      w.it0[s] = (p.causal && w.a_chunk) ? r0 / kTile : 0;  // first query tile that can see this key sub-tile
+    }
+    w.tiles_per_g = nqt - w.it0[0];
+    w.ntiles = w.sub_valid[0] ? p.G * w.tiles_per_g : 0;
+    return w.sub_valid[0] && w.ntiles > 0;
+  }
+}
+
+template <int kPass>
+__device__ __forceinline__ bool sub_takes_tile(const Work& w, int s, int j) {
+  if (kPass == 1) return j < w.ntiles_sub[s];
+  if (!w.sub_valid[s]) return false;
+  const int it = w.it0[0] + j % w.tiles_per_g;
+  return it >= w.it0[s];
+}
+
+template <int kPass, bool kEntropy>
+__global__ void __launch_bounds__(kThreads, 1)
+score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapKc,
+                const __grid_constant__ CUtensorMap mapKn, const TcArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const StepParams& p = a.p;
+  Work w;
+  if (!make_work<kPass>(a, w)) return;  // uniform across the CTA
+
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  const uint32_t sA = smem_u32(smem);                    // [2 sub][2 kb][16 KB]
+  const uint32_t sB = sA + 2 * kTileBytes;               // [kStages][2 kb][16 KB]
+  const uint32_t bars = sB + kStages * kTileBytes;
+  const uint32_t bar_full = bars, bar_empty = bars + 8 * kStages, bar_a = bars + 16 * kStages;
+  const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 32;  // [sub*2+buf]
+  uint32_t* tmem_slot = (uint32_t*)(smem + 2 * kTileBytes + kStages * kTileBytes + 16 * kStages + 8 + 64);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+    mbar_init(bar_a, 1);
+    for (int i = 0; i < 4; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      const CUtensorMap* mA = kPass == 1 ? &mapQ : (w.a_chunk ? &mapKn : &mapKc);
+      const int nsub = w.sub_valid[1] ? 2 : 1;
+      mbar_expect_tx(bar_a, nsub * kTileBytes);
+      for (int s = 0; s < nsub; ++s)
+        for (int kb = 0; kb < 2; ++kb)
+          tma_load_3d(sA + s * kTileBytes + kb * kKBlockBytes, mA, kb * kKBlock, w.rowA0 + s * kTile, w.lhA, bar_a);
+      for (int j = 0; j < w.ntiles; ++j) {
+        const int stage = j % kStages;
+        mbar_wait(bar_empty + 8 * stage, ((j / kStages) & 1) ^ 1);
+        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
+        const CUtensorMap* mB;
+        int row0, lh;
+        if (kPass == 1) {
+          const bool cache = j < w.n_cache_tiles;
+          mB = cache ? &mapKc : &mapKn;
+          row0 = (cache ? j : j - w.n_cache_tiles) * kTile;
+          lh = w.l * p.Hkv + w.h;
+        } else {
+          mB = &mapQ;
+          row0 = (w.it0[0] + j % w.tiles_per_g) * kTile;
+          lh = w.hq0 + j / w.tiles_per_g;
+        }
+        for (int kb = 0; kb < 2; ++kb)
+          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      mbar_wait(bar_a, 0);
+      tc_fence_after();
+      int js[2] = {0, 0};
+      for (int j = 0; j < w.ntiles; ++j) {
+        const int stage = j % kStages;
+        mbar_wait(bar_full + 8 * stage, (j / kStages) & 1);
+        tc_fence_after();
+        for (int s = 0; s < 2; ++s) {
+          if (!sub_takes_tile<kPass>(w, s, j)) continue;
+          const int buf = js[s] & 1;
+          mbar_wait(bar_sempty + 8 * (s * 2 + buf), ((js[s] >> 1) & 1) ^ 1);
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)((s * 2 + buf) * kTile);
+#pragma unroll
+          for (int kk = 0; kk < kHeadDim / 16; ++kk) {
+            const uint32_t koff = (uint32_t)((kk >> 2) * kKBlockBytes + (kk & 3) * 32);
+            tc_mma_bf16(d_tmem, umma_desc_sw128(sA + s * kTileBytes + koff), umma_desc_sw128(sB + stage * kTileBytes + koff),
+                        kIdesc, kk > 0 ? 1u : 0u);
+          }
+          tc_commit(bar_sfull + 8 * (s * 2 + buf));
+          ++js[s];
+        }
+        tc_commit(bar_empty + 8 * stage);
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue groups =====================
+    const int s = (warp - 4) >> 2;       // sub-tile
+    const int q4 = warp & 3;             // TMEM lane quarter owned by this warp
+    const int r = q4 * 32 + lane;        // row of the sub-tile == TMEM lane
+    const float c2 = p.scale_log2e;
+    if (w.sub_valid[s]) {
+      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+      int js = 0;
+      if (kPass == 1) {
+        const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
+        const int n = p.n[w.l];
+        float m_run = -1e30f, Z = 0.f, W = 0.f;
+        for (int j = 0; j < w.ntiles_sub[s]; ++j, ++js) {
+          const int buf = js & 1;
+          // number of visible key columns of this tile for this row
+          int limit;
+          if (j < w.n_cache_tiles) limit = n - j * kTile;
+          else {
+            const int t0 = (j - w.n_cache_tiles) * kTile;
+            limit = p.Nn - t0;
+            if (p.causal) limit = min(limit, i - t0 + 1);
+          }
+          mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
+          tc_fence_after();
+          const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
+#pragma unroll 1
+          for (int c = 0; c < 4; ++c) {
+            uint32_t v[32];
+            tc_ld32(t_addr + c * 32, v);
+            tc_wait_ld();
+            float x[32];
+            const int lim_c = limit - c * 32;
+            if (lim_c >= 32) {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) x[e] = __uint_as_float(v[e]);
+            } else {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) x[e] = e < lim_c ? __uint_as_float(v[e]) : -INFINITY;
+            }
+            float mx[4] = {x[0], x[1], x[2], x[3]};
+#pragma unroll
+            for (int e = 4; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], x[e]);
+            const float cmax = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+            const float m_new = fmaxf(m_run, cmax * c2);
+            const float rs = ex2(m_run - m_new);
+            m_run = m_new;
+            float z[4] = {0.f, 0.f, 0.f, 0.f}, wz[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+              const float pe = ex2(fmaf(x[e], c2, -m_new));
+              z[e & 3] += pe;
+              if (kEntropy) wz[e & 3] = fmaf(pe, lim_c > e ? x[e] * c2 : 0.f, wz[e & 3]);
+            }
+            Z = fmaf(Z, rs, (z[0] + z[1]) + (z[2] + z[3]));
+            if (kEntropy) W = fmaf(W, rs, (wz[0] + wz[1]) + (wz[2] + wz[3]));
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));
+        }
+        // lse2 = log2 sum_k 2^(c2 s_k); padded rows (i >= Nn) publish +inf so that pass 2 adds nothing for them
+        const long long hq = (long long)w.lhA;
+        const float l2 = m_run + log2f(Z);
+        a.lse2[hq * a.lse_stride + i] = i < p.Nn ? l2 : INFINITY;
+        if (i < p.Nn) {
+          if (a.lse_nat) a.lse_nat[hq * p.Nn + i] = l2 * 0.6931471805599453f;
+          if (kEntropy && a.row_entropy) a.row_entropy[hq * p.Nn + i] = (l2 - W / Z) * 0.6931471805599453f;
+        }
+      } else {
+        const int krow = w.rowA0 + s * kTile + r;  // key row in cache or chunk
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int j = 0; j < w.ntiles; ++j) {
+          const int it = w.it0[0] + j % w.tiles_per_g;
+          if (it < w.it0[s]) continue;
+          const int g = j / w.tiles_per_g;
+          const int buf = js & 1;
+          // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column of this tile:
+          const int first = (p.causal && w.a_chunk) ? krow - it * kTile : 0;
+          const float4* l4 = reinterpret_cast<const float4*>(a.lse2 + (long long)(w.hq0 + g) * a.lse_stride + it * kTile);
+          mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
+          tc_fence_after();
+          const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
+#pragma unroll 1
+          for (int c = 0; c < 4; ++c) {
+            uint32_t v[32];
+            tc_ld32(t_addr + c * 32, v);
+            float ls[32];
+#pragma unroll
+            for (int e4 = 0; e4 < 8; ++e4) {
+              const float4 t4 = __ldg(l4 + c * 8 + e4);
+              ls[4 * e4] = t4.x; ls[4 * e4 + 1] = t4.y; ls[4 * e4 + 2] = t4.z; ls[4 * e4 + 3] = t4.w;
+            }
+            tc_wait_ld();
+            const int first_c = first - c * 32;
+            if (first_c <= 0) {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) acc[e & 3] += ex2(fmaf(__uint_as_float(v[e]), c2, -ls[e]));
+            } else {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) {
+                const float pe = ex2(fmaf(__uint_as_float(v[e]), c2, -ls[e]));
+                acc[e & 3] += e >= first_c ? pe : 0.f;
+              }
+            }
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));
+          ++js;
+        }
+        const int n_v = p.n_v[w.l], n = p.n[w.l];
+        const bool valid = w.a_chunk ? krow < p.Nn : krow < n;
+        if (valid) {
+          int m, t;
+          if (w.a_chunk) chunk_row_to_seg(p, n_v, n, krow, m, t); else cache_row_to_seg(n_v, krow, m, t);
+          float* out = m == 0 ? a.a_v + (long long)w.lhA * p.seg_cap_v : a.a_a + (long long)w.lhA * p.seg_cap_a;
+          out[t] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+  }
+}
+
+// natural-log LSE supplied by the caller -> internal log2-domain, padded layout
+__global__ void lse_to_log2_kernel(const float* __restrict__ lse_nat, float* __restrict__ lse2, int rows, int Nn, int stride) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)rows * stride) return;
+  const int i = (int)(idx % stride);
+  const long long r = idx / stride;
+  lse2[idx] = i < Nn ? lse_nat[r * Nn + i] * 1.4426950408889634f : INFINITY;
+}
+
+// ---- host side -------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static cudaError_t get_encode(omnimem_ctx* ctx, EncodeTiledFn* fn) {
+  if (!ctx->encode_tiled) {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (q != cudaDriverEntryPointSuccess || !f) return cudaErrorNotSupported;
+    ctx->encode_tiled = f;
+  }
+  *fn = (EncodeTiledFn)ctx->encode_tiled;
+  return cudaSuccess;
+}
+
+// [outer, rows, 128] bf16 row-major -> 3-D map, box = 64 x 128 x 1, 128-byte swizzle, zero fill out of bounds
+static cudaError_t make_map(EncodeTiledFn enc, CUtensorMap* m, const void* base, uint64_t rows, uint64_t outer) {
+  if (rows == 0 || outer == 0 || base == nullptr) { memset(m, 0, sizeof(*m)); return cudaSuccess; }
+  const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, outer};
+  const cuuint64_t strides[2] = {(cuuint64_t)kHeadDim * 2, rows * kHeadDim * 2};
+  const cuuint32_t box[3] = {(cuuint32_t)kKBlock, (cuuint32_t)kTile, 1};
+  const cuuint32_t es[3] = {1, 1, 1};
+  const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+struct Maps { CUtensorMap q, kc, kn; };
+
+static cudaError_t make_maps(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, Maps* m) {
+  EncodeTiledFn enc;
+  cudaError_t e = get_encode(const_cast<omnimem_ctx*>(ctx), &enc);
+  if (e != cudaSuccess) return e;
+  if ((e = make_map(enc, &m->q, b.Q, p.Nn, (uint64_t)p.L * p.Hq)) != cudaSuccess) return e;
+  if ((e = make_map(enc, &m->kc, b.cacheK, p.cache_cap, (uint64_t)p.L * p.Hkv)) != cudaSuccess) return e;
+  return make_map(enc, &m->kn, b.chunkK, p.Nn, (uint64_t)p.L * p.Hkv);
+}
+
+static TcArgs make_args(const StepParams& p, const StepBuffers& b) {
+  TcArgs a{};
+  a.p = p;
+  a.lse2 = b.lse2;
+  a.lse_stride = (p.Nn + kTile - 1) / kTile * kTile;
+  a.lse_nat = b.lse_out;
+  a.row_entropy = b.row_entropy;
+  a.a_v = b.a_v;
+  a.a_a = b.a_a;
+  a.n_cache_pairs = (p.cache_cap + 2 * kTile - 1) / (2 * kTile);
+  return a;
+}
+
+cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
+  if (p.Nn == 0) return cudaSuccess;
+  Maps m;
+  cudaError_t e = make_maps(ctx, p, b, &m);
+  if (e != cudaSuccess) return e;
+  const TcArgs a = make_args(p, b);
+  dim3 grid((p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hq, p.L);
+  ++*launches;
+  if (b.row_entropy) {
+    e = cudaFuncSetAttribute(score_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) return e;
+    score_tc_kernel<1, true><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
+  } else {
+    e = cudaFuncSetAttribute(score_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) return e;
+    score_tc_kernel<1, false><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
+  if (p.Nn == 0) {  // no queries: a = 0 everywhere
+    cudaError_t e = cudaMemsetAsync(b.a_v, 0, (size_t)p.L * p.Hkv * p.seg_cap_v * sizeof(float), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(b.a_a, 0, (size_t)p.L * p.Hkv * p.seg_cap_a * sizeof(float), st);
+    return e;
+  }
+  Maps m;
+  cudaError_t e = make_maps(ctx, p, b, &m);
+  if (e != cudaSuccess) return e;
+  const TcArgs a = make_args(p, b);
+  if (b.lse_in) {
+    const long long tot = (long long)p.L * p.Hq * a.lse_stride;
+    lse_to_log2_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(b.lse_in, b.lse2, p.L * p.Hq, p.Nn, a.lse_stride);
+    ++*launches;
+  }
+  dim3 grid(a.n_cache_pairs + (p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hkv, p.L);
+  e = cudaFuncSetAttribute(score_tc_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  ++*launches;
+  score_tc_kernel<2, false><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
+  return cudaGetLastError();
+}
+
+}  // namespace omnimem

@@ -1,0 +1,500 @@
+// Bandwidth / latency kernels of the step: adjacent cosine (Eq.7), finalize (Eq.8 psi + Eq.9-10/13 partial
+// statistics), statistics + budgets (Eq.9-14), segmented radix top-M (Eq.4-5), gather-compaction.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace omnimem {
+
+// ------------------------------------------------------------------------------------------------------------
+// Eq.7 (value rows per P:103, R8): cosn[t] = cos(x_t, x_{t+sigma}) inside the modality's appended sequence.
+// s_t is assembled from cosn[t] and cosn[t-sigma] in finalize.  kTPR threads (16 B each) cover one row.
+// ------------------------------------------------------------------------------------------------------------
+template <typename T> struct Row16;
+template <> struct Row16<float> {
+  static constexpr int N = 4;
+  __device__ static __forceinline__ void load(const float* p, float* o) {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+  }
+};
+template <> struct Row16<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ static __forceinline__ void load(const __nv_bfloat16* p, float* o) {
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      o[2 * i] = __uint_as_float(w[i] << 16);
+      o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    }
+  }
+};
+
+template <typename T, int kTPR>
+__global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __restrict__ cacheX,
+                                                     const T* __restrict__ chunkX, float* __restrict__ cosn) {
+  constexpr int kRows = 256 / kTPR;
+  const int items = p.seg_cap_v + p.seg_cap_a;
+  const long long item = (long long)blockIdx.x * kRows + threadIdx.x / kTPR;
+  const int sub = threadIdx.x % kTPR;
+  const long long total = (long long)p.L * p.Hkv * items;
+  bool active = item < total;
+  int l = 0, h = 0, m = 0, t = 0;
+  if (active) {
+    const int it = (int)(item % items);
+    h = (int)((item / items) % p.Hkv);
+    l = (int)(item / ((long long)items * p.Hkv));
+    m = it < p.seg_cap_v ? 0 : 1;
+    t = m == 0 ? it : it - p.seg_cap_v;
+  }
+  float dot = 0.f, nx = 0.f, ny = 0.f;
+  if (active) {
+    const int n_v = p.n_v[l], n = p.n[l];
+    const int sg = m == 0 ? p.stride_v : p.stride_a;
+    active = t + sg < seg_len(p, n_v, n, m);
+    if (active) {
+      bool cx, cy;
+      const int rx = seg_row(p, n_v, n, m, t, cx), ry = seg_row(p, n_v, n, m, t + sg, cy);
+      const long long lh = (long long)l * p.Hkv + h;
+      const T* x = (cx ? chunkX + (lh * p.Nn + rx) * p.D : cacheX + (lh * p.cache_cap + rx) * p.D) + sub * Row16<T>::N;
+      const T* y = (cy ? chunkX + (lh * p.Nn + ry) * p.D : cacheX + (lh * p.cache_cap + ry) * p.D) + sub * Row16<T>::N;
+      float xv[Row16<T>::N], yv[Row16<T>::N];
+      Row16<T>::load(x, xv);
+      Row16<T>::load(y, yv);
+#pragma unroll
+      for (int e = 0; e < Row16<T>::N; ++e) {
+        dot = fmaf(xv[e], yv[e], dot);
+        nx = fmaf(xv[e], xv[e], nx);
+        ny = fmaf(yv[e], yv[e], ny);
+      }
+    }
+  }
+#pragma unroll
+  for (int o = kTPR / 2; o; o >>= 1) {
+    dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    nx += __shfl_xor_sync(0xffffffffu, nx, o);
+    ny += __shfl_xor_sync(0xffffffffu, ny, o);
+  }
+  if (active && sub == 0) cosn[item] = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
+}
+
+cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
+                          int* launches) {
+  const void* cx = ctx->cfg.sim_source == 0 ? b.cacheV : b.cacheK;
+  const void* kx = ctx->cfg.sim_source == 0 ? b.chunkV : b.chunkK;
+  const long long total = (long long)p.L * p.Hkv * (p.seg_cap_v + p.seg_cap_a);
+  const int row_bytes = p.D * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2);
+  const int tpr = row_bytes / 16;
+  const unsigned grid = (unsigned)((total + 256 / tpr - 1) / (256 / tpr));
+  ++*launches;
+#define OMNIMEM_COS(T, TPR) cosine_kernel<T, TPR><<<grid, 256, 0, st>>>(p, (const T*)cx, (const T*)kx, b.cosn)
+  if (ctx->cfg.dtype == OMNIMEM_FP32) {
+    if (tpr == 16) OMNIMEM_COS(float, 16); else OMNIMEM_COS(float, 32);
+  } else {
+    if (tpr == 8) OMNIMEM_COS(__nv_bfloat16, 8); else OMNIMEM_COS(__nv_bfloat16, 16);
+  }
+#undef OMNIMEM_COS
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Finalize: s_t (Eq.7 mean over existing neighbours, clamp, R10/R12), psi = a^lambda (1-s) (Eq.8), and per-block
+// partial sums of A_t = sum_h a, A_t ln A_t and s for the AVBA statistics (Eq.9-10, 13; H = ln S - sum A ln A / S).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) finalize_kernel(StepParams p, const float* __restrict__ a_v,
+                                                       const float* __restrict__ a_a, const float* __restrict__ cosn,
+                                                       float* __restrict__ s_v, float* __restrict__ s_a,
+                                                       float* __restrict__ psi_v, float* __restrict__ psi_a,
+                                                       double* __restrict__ partials, int nblk) {
+  const int l = blockIdx.z, m = blockIdx.y, t = blockIdx.x * 256 + threadIdx.x;
+  const int n_v = p.n_v[l], n = p.n[l];
+  const int Km = seg_len(p, n_v, n, m);
+  const int cap = m == 0 ? p.seg_cap_v : p.seg_cap_a;
+  const int sg = m == 0 ? p.stride_v : p.stride_a;
+  const int items = p.seg_cap_v + p.seg_cap_a;
+  const bool skip = layer_skips_scoring(p, l);
+  double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+  if (t < Km && !skip) {
+    float A = 0.f, ssum = 0.f;
+    for (int h = 0; h < p.Hkv; ++h) {
+      const long long lh = (long long)l * p.Hkv + h;
+      const float* cs = cosn + lh * items + (m == 0 ? 0 : p.seg_cap_v);
+      float sum = 0.f;
+      int cnt = 0;
+      if (t + sg < Km) { sum += cs[t]; ++cnt; }
+      if (t - sg >= 0) { sum += cs[t - sg]; ++cnt; }
+      float s = cnt == 2 ? 0.5f * sum : sum;  // cnt == 0 -> 0 (R10)
+      s = fminf(1.f, fmaxf(-1.f, s));
+      const float a = (m == 0 ? a_v : a_a)[lh * cap + t];
+      (m == 0 ? s_v : s_a)[lh * cap + t] = s;
+      (m == 0 ? psi_v : psi_a)[lh * cap + t] = powf(a, p.lambda) * (1.f - s);
+      A += a;
+      ssum += s;
+    }
+    v0 = (double)A;
+    v1 = A > 0.f ? (double)A * log((double)A) : 0.0;
+    v2 = (double)ssum;
+  }
+  __shared__ double red[3][8];
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) { red[0][warp] = v0; red[1][warp] = v1; red[2][warp] = v2; }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    double acc = 0.0;
+    for (int w = 0; w < 8; ++w) acc += red[threadIdx.x][w];
+    partials[(((long long)l * 2 + m) * nblk + blockIdx.x) * 3 + threadIdx.x] = acc;
+  }
+}
+
+// stats[l] = {Hn_v, Hn_a, sbar_v, sbar_a, C_v, C_a, Hn_all, sbar_all}; one warp per layer, fixed summation order.
+__global__ void __launch_bounds__(32) stats_kernel(StepParams p, const double* __restrict__ partials, int nblk,
+                                                   double* __restrict__ stats) {
+  const int l = blockIdx.x, lane = threadIdx.x;
+  double S[2], Tl[2], Ss[2];
+  for (int m = 0; m < 2; ++m) {
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+    const double* pp = partials + ((long long)l * 2 + m) * nblk * 3;
+    for (int b = lane; b < nblk; b += 32) { v0 += pp[b * 3]; v1 += pp[b * 3 + 1]; v2 += pp[b * 3 + 2]; }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+      v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+      v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+    }
+    S[m] = v0; Tl[m] = v1; Ss[m] = v2;
+  }
+  if (lane == 0) {
+    const int n_v = p.n_v[l], n = p.n[l];
+    const int K[2] = {seg_len(p, n_v, n, 0), seg_len(p, n_v, n, 1)};
+    double Hn[2], sbar[2];
+    for (int m = 0; m < 2; ++m) {
+      double H = S[m] > 0.0 ? log(S[m]) - Tl[m] / S[m] : 0.0;
+      H = H < 0.0 ? 0.0 : H;
+      Hn[m] = (K[m] > 1 && S[m] > 0.0) ? fmin(1.0, H / log((double)K[m])) : 0.0;  // R15
+      sbar[m] = K[m] > 0 ? Ss[m] / ((double)K[m] * p.Hkv) : 0.0;                    // R17
+    }
+    const double Sall = S[0] + S[1], Tall = Tl[0] + Tl[1];
+    const int Kall = K[0] + K[1];
+    double Hall = Sall > 0.0 ? log(Sall) - Tall / Sall : 0.0;
+    Hall = Hall < 0.0 ? 0.0 : Hall;
+    double* st = stats + (long long)l * 8;
+    st[0] = Hn[0]; st[1] = Hn[1]; st[2] = sbar[0]; st[3] = sbar[1];
+    st[4] = Hn[0] * (1.0 - sbar[0]);  // Eq.9
+    st[5] = Hn[1] * (1.0 - sbar[1]);  // Eq.10
+    st[6] = (Kall > 1 && Sall > 0.0) ? fmin(1.0, Hall / log((double)Kall)) : 0.0;  // Eq.13, R18
+    st[7] = Kall > 0 ? (Ss[0] + Ss[1]) / ((double)Kall * p.Hkv) : 0.0;
+  }
+}
+
+cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
+                            int* launches) {
+  const int nblk = ctx->fin_blocks;
+  dim3 grid(nblk, 2, p.L);
+  finalize_kernel<<<grid, 256, 0, st>>>(p, b.a_v, b.a_a, b.cosn, b.s_v, b.s_a, b.psi_v, b.psi_a, b.partials, nblk);
+  stats_kernel<<<p.L, 32, 0, st>>>(p, b.partials, nblk, b.stats);
+  *launches += 2;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Budgets.  Eq.13-14 layer totals (only if layer_budget == nullptr; R19, R20) then Eq.11-12 modality split (R22).
+// ------------------------------------------------------------------------------------------------------------
+struct AllocParams {
+  double ratio_r, temperature;
+  long long total_budget, budget_min, budget_max;
+};
+
+__global__ void __launch_bounds__(128) allocate_kernel(StepParams p, AllocParams ap, const double* __restrict__ stats,
+                                                       const int32_t* __restrict__ layer_budget, int32_t* __restrict__ M_v,
+                                                       int32_t* __restrict__ M_a, int32_t* __restrict__ layer_budget_out) {
+  extern __shared__ double sm_alloc[];
+  const int L = p.L;
+  double* pi = sm_alloc;            // [L]
+  double* bl = sm_alloc + L;        // [L]
+  int* B = (int*)(sm_alloc + 2 * L);  // [L]
+  int* fixed = B + L;               // [L]
+  if (layer_budget != nullptr) {
+    for (int l = threadIdx.x; l < L; l += blockDim.x) B[l] = layer_budget[l];
+  } else if (threadIdx.x == 0) {
+    const bool clamp = ap.budget_max > 0;
+    const double lo = clamp ? (double)ap.budget_min : 0.0, hi = clamp ? (double)ap.budget_max : INFINITY;
+    double mx = -INFINITY, Z = 0.0;
+    for (int l = 0; l < L; ++l) {
+      pi[l] = stats[l * 8 + 6] * (1.0 - stats[l * 8 + 7]) / ap.temperature;  // C^(l)/T, Eq.13
+      mx = fmax(mx, pi[l]);
+      fixed[l] = 0;
+    }
+    for (int l = 0; l < L; ++l) Z += (pi[l] = exp(pi[l] - mx));
+    for (int l = 0; l < L; ++l) pi[l] /= Z;                                 // Eq.14 softmax over layers
+    if (clamp && (double)ap.total_budget >= hi * L) {
+      for (int l = 0; l < L; ++l) B[l] = (int)ap.budget_max;
+    } else if (clamp && (double)ap.total_budget <= lo * L) {
+      for (int l = 0; l < L; ++l) B[l] = (int)ap.budget_min;
+    } else {
+      for (int it = 0; it <= L; ++it) {  // fix violators at the bound, re-split the rest in proportion to pi
+        double rem = (double)ap.total_budget, pfree = 0.0;
+        for (int l = 0; l < L; ++l) { if (fixed[l]) rem -= bl[l]; else pfree += pi[l]; }
+        double below = 0.0, above = 0.0;
+        for (int l = 0; l < L; ++l)
+          if (!fixed[l]) {
+            bl[l] = pfree > 0.0 ? rem * pi[l] / pfree : 0.0;
+            below += bl[l] < lo ? lo - bl[l] : 0.0;
+            above += bl[l] > hi ? bl[l] - hi : 0.0;
+          }
+        bool moved = false;
+        const bool top = above >= below;  // clamp one side per round so that the total is preserved
+        for (int l = 0; l < L; ++l)
+          if (!fixed[l] && (top ? bl[l] > hi : bl[l] < lo)) { bl[l] = top ? hi : lo; fixed[l] = 1; moved = true; }
+        if (!moved) break;
+      }
+      long long sum = 0;
+      for (int l = 0; l < L; ++l) { B[l] = (int)floor(bl[l]); sum += B[l]; }
+      for (long long left = ap.total_budget - sum; left > 0; --left) {  // largest remainder, ties -> lowest layer
+        int best = -1;
+        double bf = -1.0;
+        for (int l = 0; l < L; ++l) {
+          const double fl = floor(bl[l]);
+          if ((double)B[l] <= fl && (double)B[l] + 1.0 <= hi && bl[l] - fl > bf) { bf = bl[l] - fl; best = l; }
+        }
+        if (best < 0) break;
+        B[best] += 1;
+      }
+    }
+  }
+  __syncthreads();
+  for (int l = threadIdx.x; l < L; l += blockDim.x) {
+    const int n_v = p.n_v[l], n = p.n[l];
+    const int Kv = seg_len(p, n_v, n, 0), Ka = seg_len(p, n_v, n, 1);
+    const int Bl = B[l] < 0 ? 0 : B[l];
+    if (layer_budget_out) layer_budget_out[l] = Bl;
+    if (Kv + Ka <= Bl) { M_v[l] = Kv; M_a[l] = Ka; continue; }
+    const double Cv = stats[l * 8 + 4], Ca = stats[l * 8 + 5];
+    const double den = ap.ratio_r * Cv + Ca;
+    const double wv = den > 0.0 ? ap.ratio_r * Cv / den : ap.ratio_r / (ap.ratio_r + 1.0);  // Eq.11
+    long long mv = (long long)floor(wv * (double)Bl + 0.5);
+    const long long lo = Bl - Ka > 0 ? Bl - Ka : 0, hi = Kv < Bl ? Kv : Bl;
+    mv = mv < lo ? lo : (mv > hi ? hi : mv);
+    M_v[l] = (int)mv;
+    M_a[l] = (int)(Bl - mv);
+  }
+}
+
+cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats,
+                            const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
+                            int32_t* layer_budget_out, cudaStream_t st, int* launches) {
+  AllocParams ap{(double)ctx->cfg.ratio_r, (double)ctx->cfg.temperature, (long long)total_budget,
+                 (long long)ctx->cfg.budget_min, (long long)ctx->cfg.budget_max};
+  const size_t smem = (size_t)p.L * (2 * sizeof(double) + 2 * sizeof(int));
+  allocate_kernel<<<1, 128, smem, st>>>(p, ap, stats, layer_budget, M_v, M_a, layer_budget_out);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Select (Eq.4-5): per (layer, KV head, modality) the M largest psi, ties -> lowest index, emitted ascending.
+// One CTA per segment.  MSB-first radix select on the order-preserving uint image of the fp32 score
+// (4 passes x 8 bits, shared-memory histogram with warp-aggregated atomics via match.any), then one ordered
+// sweep: rank = #greater before t + min(#equal before t, need), from warp ballots + a scan of warp totals.
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t order_key(float x) {
+  uint32_t u = __float_as_uint(x);
+  if (u == 0x80000000u) u = 0u;  // -0 == +0
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+constexpr int kSelThreads = 1024;
+
+template <bool kSmem>
+__global__ void __launch_bounds__(kSelThreads) select_kernel(StepParams p, const float* __restrict__ psi_v,
+                                                             const float* __restrict__ psi_a,
+                                                             const int32_t* __restrict__ M_v,
+                                                             const int32_t* __restrict__ M_a, int32_t* __restrict__ idx_v,
+                                                             int32_t* __restrict__ idx_a) {
+  extern __shared__ uint32_t skeys[];
+  __shared__ uint32_t hist[256];
+  __shared__ uint32_t warp_tot[32];
+  __shared__ uint32_t warp_off[32];
+  __shared__ uint32_t sh_digit, sh_need, sh_chunk_tot;
+  const int seg = blockIdx.x;
+  const int m = seg & 1, h = (seg >> 1) % p.Hkv, l = (seg >> 1) / p.Hkv;
+  const int K = seg_len(p, p.n_v[l], p.n[l], m);
+  const int M = m == 0 ? M_v[l] : M_a[l];
+  const long long lh = (long long)l * p.Hkv + h;
+  const float* psi = m == 0 ? psi_v + lh * p.seg_cap_v : psi_a + lh * p.seg_cap_a;
+  int32_t* out = (m == 0 ? idx_v : idx_a) + lh * p.cache_cap;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (M <= 0) return;
+  if (M >= K) {  // nothing to evict in this segment: identity
+    for (int t = tid; t < K; t += kSelThreads) out[t] = t;
+    return;
+  }
+  if (kSmem) {
+    for (int t = tid; t < K; t += kSelThreads) skeys[t] = order_key(psi[t]);
+    __syncthreads();
+  }
+  auto key = [&](int t) -> uint32_t { return kSmem ? skeys[t] : order_key(__ldg(psi + t)); };
+  const int Kpad = (K + kSelThreads - 1) / kSelThreads * kSelThreads;
+  uint32_t prefix = 0u, mask = 0u, need = (uint32_t)M;
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = 24 - 8 * pass;
+    if (tid < 256) hist[tid] = 0u;
+    __syncthreads();
+    for (int t = tid; t < Kpad; t += kSelThreads) {
+      uint32_t d = 256u;  // sentinel: not a candidate
+      if (t < K) {
+        const uint32_t u = key(t);
+        if ((u & mask) == prefix) d = (u >> shift) & 255u;
+      }
+      const uint32_t peers = __match_any_sync(0xffffffffu, d);
+      if (d < 256u && lane == (__ffs(peers) - 1)) atomicAdd(&hist[d], (uint32_t)__popc(peers));
+    }
+    __syncthreads();
+    if (warp == 0) {  // lane i owns bins 255-8i .. 248-8i (descending); find the bin holding the need-th largest
+      uint32_t c = 0u;
+#pragma unroll
+      for (int b = 0; b < 8; ++b) c += hist[255 - 8 * lane - b];
+      uint32_t incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      const uint32_t excl = incl - c;
+      if (excl < need && need <= incl) {
+        uint32_t run = excl;
+        for (int b = 0; b < 8; ++b) {
+          const int bin = 255 - 8 * lane - b;
+          const uint32_t cnt = hist[bin];
+          if (run + cnt >= need) { sh_digit = (uint32_t)bin; sh_need = need - run; break; }
+          run += cnt;
+        }
+      }
+    }
+    __syncthreads();
+    prefix |= sh_digit << shift;
+    mask |= 255u << shift;
+    need = sh_need;
+  }
+  const uint32_t tau = prefix;  // key of the M-th largest score; `need` equal keys are kept, lowest index first (R23)
+  uint32_t gt_before = 0u, eq_before = 0u;
+  for (int base = 0; base < Kpad; base += kSelThreads) {
+    const int t = base + tid;
+    const uint32_t u = t < K ? key(t) : 0u;
+    const bool gt = t < K && u > tau, eq = t < K && u == tau;
+    const uint32_t bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
+    if (lane == 0) warp_tot[warp] = (uint32_t)__popc(bg) | ((uint32_t)__popc(be) << 16);
+    __syncthreads();
+    if (warp == 0) {
+      const uint32_t c = warp_tot[lane];
+      uint32_t incl = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      warp_off[lane] = incl - c;
+      if (lane == 31) sh_chunk_tot = incl;
+    }
+    __syncthreads();
+    const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t off = warp_off[warp];
+    const uint32_t g0 = gt_before + (off & 0xffffu) + (uint32_t)__popc(bg & lt);
+    const uint32_t e0 = eq_before + (off >> 16) + (uint32_t)__popc(be & lt);
+    if (gt) out[g0 + min(e0, need)] = t;
+    else if (eq && e0 < need) out[g0 + e0] = t;
+    const uint32_t tot = sh_chunk_tot;
+    gt_before += tot & 0xffffu;
+    eq_before += tot >> 16;
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_select(const omnimem_ctx* ctx, const StepParams& p, const float* psi_v, const float* psi_a,
+                          const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a, cudaStream_t st,
+                          int* launches) {
+  const int segs = p.L * p.Hkv * 2;
+  const size_t smem = (size_t)(p.seg_cap_v > p.seg_cap_a ? p.seg_cap_v : p.seg_cap_a) * sizeof(uint32_t);
+  ++*launches;
+  if (smem <= 200 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(select_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    select_kernel<true><<<segs, kSelThreads, smem, st>>>(p, psi_v, psi_a, M_v, M_a, idx_v, idx_a);
+  } else {
+    select_kernel<false><<<segs, kSelThreads, 0, st>>>(p, psi_v, psi_a, M_v, M_a, idx_v, idx_a);
+  }
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Compaction (P:66 prune): dst[l,h,j] = src row of the j-th kept index, K and V, 128-bit copies,
+// kTPR threads per row, kR rows in flight per thread.  Also publishes the new row counts.
+// ------------------------------------------------------------------------------------------------------------
+template <int kTPR, int kR>
+__global__ void __launch_bounds__(256) compact_kernel(StepParams p, const uint4* __restrict__ srcK,
+                                                      const uint4* __restrict__ srcV, const uint4* __restrict__ chunkK,
+                                                      const uint4* __restrict__ chunkV, const int32_t* __restrict__ idx_v,
+                                                      const int32_t* __restrict__ idx_a, const int32_t* __restrict__ M_v,
+                                                      const int32_t* __restrict__ M_a, uint4* __restrict__ dstK,
+                                                      uint4* __restrict__ dstV, int32_t* __restrict__ dst_n_v,
+                                                      int32_t* __restrict__ dst_n) {
+  constexpr int kRowsPerPass = 256 / kTPR;
+  const int l = blockIdx.z, h = blockIdx.y;
+  const int Mv = M_v[l], Ma = M_a[l], total = Mv + Ma;
+  if (blockIdx.x == 0 && h == 0 && threadIdx.x == 0) { dst_n_v[l] = Mv; dst_n[l] = total; }
+  const int j0 = blockIdx.x * (kRowsPerPass * kR) + threadIdx.x / kTPR;
+  if (j0 - (int)(threadIdx.x / kTPR) >= total) return;
+  const int sub = threadIdx.x % kTPR;
+  const int n_v = p.n_v[l], n = p.n[l];
+  const long long lh = (long long)l * p.Hkv + h;
+  uint4 vk[kR], vv[kR];
+#pragma unroll
+  for (int r = 0; r < kR; ++r) {
+    const int j = j0 + r * kRowsPerPass;
+    if (j < total) {
+      const int m = j < Mv ? 0 : 1;
+      const int t = m == 0 ? idx_v[lh * p.cache_cap + j] : idx_a[lh * p.cache_cap + (j - Mv)];
+      bool in_chunk;
+      const int row = seg_row(p, n_v, n, m, t, in_chunk);
+      const long long off = in_chunk ? (lh * p.Nn + row) * kTPR + sub : (lh * p.cache_cap + row) * kTPR + sub;
+      vk[r] = __ldg((in_chunk ? chunkK : srcK) + off);
+      vv[r] = __ldg((in_chunk ? chunkV : srcV) + off);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < kR; ++r) {
+    const int j = j0 + r * kRowsPerPass;
+    if (j < total) {
+      const long long off = (lh * p.cache_cap + j) * kTPR + sub;
+      dstK[off] = vk[r];
+      dstV[off] = vv[r];
+    }
+  }
+}
+
+cudaError_t launch_compact(const omnimem_ctx* ctx, const StepParams& p, const void* srcK, const void* srcV,
+                           const void* chunkK, const void* chunkV, const int32_t* idx_v, const int32_t* idx_a,
+                           const int32_t* M_v, const int32_t* M_a, void* dstK, void* dstV, int32_t* dst_n_v,
+                           int32_t* dst_n, cudaStream_t st, int* launches) {
+  const int row_bytes = p.D * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2);
+  const int tpr = row_bytes / 16;
+  constexpr int kR = 4;
+  const int rows_per_block = 256 / tpr * kR;
+  dim3 grid((p.cache_cap + rows_per_block - 1) / rows_per_block, p.Hkv, p.L);
+  ++*launches;
+#define OMNIMEM_CP(TPR)                                                                                              \
+  compact_kernel<TPR, kR><<<grid, 256, 0, st>>>(p, (const uint4*)srcK, (const uint4*)srcV, (const uint4*)chunkK,    \
+                                                (const uint4*)chunkV, idx_v, idx_a, M_v, M_a, (uint4*)dstK,        \
+                                                (uint4*)dstV, dst_n_v, dst_n)
+  if (tpr == 8) OMNIMEM_CP(8); else if (tpr == 16) OMNIMEM_CP(16); else OMNIMEM_CP(32);
+#undef OMNIMEM_CP
+  return cudaGetLastError();
+}
+
+}  // namespace omnimem

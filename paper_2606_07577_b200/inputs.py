@@ -98,6 +98,8 @@ def _randn(g, *shape):
 
 def _ar1_frames(g, Hkv: int, n_frames: int, frame: int, D: int, rho: float) -> torch.Tensor:
     """x[f] = rho x[f-1] + sqrt(1-rho^2) eps, x[0] = eps, per token slot; returns [Hkv, n_frames*frame, D]."""
+    if n_frames == 0:
+        return torch.zeros(Hkv, 0, D)
     eps = _randn(g, n_frames, Hkv, frame, D)
     out = torch.empty_like(eps)
     out[0] = eps[0]

@@ -1,0 +1,301 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+north_star matching rules: (a) scores, entropies, budgets within 2e-3 relative (1e-5 for fp32 inputs);
+(b) selection and compaction bit-exact when fed the oracle's score array; (c) end-to-end kept-index sets
+identical except where adjacent scores differ by less than that tolerance.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ref
+from paper_2606_07577_b200 import inputs as I
+from tests.util import TOL, compare_scores, kept_sets_rule_c, ref_params, scores_to_numpy, seg_lens, to_device
+
+pytestmark = pytest.mark.gpu
+
+
+def engine_for(wl, **kw):
+    from paper_2606_07577_b200.omnimem import OmniMem
+    return OmniMem.for_workload(wl, **kw)
+
+
+def dev_objs(x, wl):
+    from paper_2606_07577_b200.omnimem import Cache, Chunk
+    d = to_device(x)
+    return Cache(d["cacheK"], d["cacheV"], d["n_v"], d["n"]), Chunk(d["chunkK"], d["chunkV"], d["Q"], wl.Nn_v, wl.Nn_a)
+
+
+def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=True, stats_tol=None):
+    """All of rules (a), (b), (c) for one step of workload `wl` (L = number of layers in x)."""
+    eng_kw, ref_kw = dict(eng_kw or {}), dict(ref_kw or {})
+    x = x if x is not None else I.full_inputs(wl)
+    L = x["Q"].shape[0]
+    wl = wl.replace(L=L)
+    tol = TOL[wl.dtype]
+    p = ref_params(wl, L, **ref_kw)
+    B = np.full((L,), wl.budget, np.int32)
+    orc = ref.compress_chunk(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"], B,
+                             sim_source=sim_source, want_rowH=check_rowH)
+    eng = engine_for(wl, sim_source=sim_source, **eng_kw)
+    src, chunk = dev_objs(x, wl)
+    n_v, n = x["n_v"].numpy(), x["n"].numpy()
+    Kv, Ka = seg_lens(wl, n_v, n)
+
+    # ---- rule (a): scoring stages
+    sc = eng.score(src, chunk, want_lse=True, want_row_entropy=check_rowH)
+    torch.cuda.synchronize()
+    g = scores_to_numpy(sc)
+    compare_scores(wl, n_v, n, g, orc, tol, stats_tol)
+    if check_rowH and wl.Nn:
+        np.testing.assert_allclose(g["rowH"], orc["rowH"], rtol=0, atol=max(50 * tol, 1e-3))  # diagnostic only (R16)
+    # softmax rows sum to one => sum_k a[l,h,k] = G * Nq
+    tot = np.array([[g["a_v"][l, h, :Kv[l]].astype(np.float64).sum() + g["a_a"][l, h, :Ka[l]].astype(np.float64).sum()
+                     for h in range(wl.Hkv)] for l in range(L)])
+    np.testing.assert_allclose(tot, wl.G * wl.Nn, rtol=10 * tol, atol=1e-12)
+
+    # ---- budgets from the ORACLE's statistics: exact
+    dev = eng.device
+    Bt = torch.from_numpy(B).to(dev)
+    M_v, M_a, _ = eng.allocate(torch.from_numpy(orc["stats"]).to(dev), src.n_v, src.n, wl.Nn_v, wl.Nn_a, Bt)
+    assert np.array_equal(M_v.cpu().numpy(), orc["M_v"]) and np.array_equal(M_a.cpu().numpy(), orc["M_a"])
+
+    # ---- rule (b): selection + compaction fed the oracle's score array and budgets: bit-exact
+    idx_v, idx_a = eng.select(torch.from_numpy(orc["psi_v"]).to(dev), torch.from_numpy(orc["psi_a"]).to(dev), src.n_v,
+                              src.n, wl.Nn_v, wl.Nn_a, M_v, M_a)
+    iv, ia = idx_v.cpu().numpy(), idx_a.cpu().numpy()
+    for l in range(L):
+        assert np.array_equal(iv[l, :, :orc["M_v"][l]], orc["idx_v"][l, :, :orc["M_v"][l]]), f"idx_v layer {l}"
+        assert np.array_equal(ia[l, :, :orc["M_a"][l]], orc["idx_a"][l, :, :orc["M_a"][l]]), f"idx_a layer {l}"
+    dst = eng.new_cache()
+    eng.compact(src, chunk, idx_v, idx_a, M_v, M_a, dst)
+    torch.cuda.synchronize()
+    dK, dV = dst.k.cpu().view(torch.uint8).numpy(), dst.v.cpu().view(torch.uint8).numpy()
+    for l in range(L):
+        nl = int(orc["n_out"][l])
+        assert np.array_equal(dK[l, :, :nl], orc["dstK"][l, :, :nl]) and np.array_equal(dV[l, :, :nl], orc["dstV"][l, :, :nl])
+    assert np.array_equal(dst.n_v.cpu().numpy(), orc["n_v_out"]) and np.array_equal(dst.n.cpu().numpy(), orc["n_out"])
+
+    # ---- rule (c): the fused step end to end
+    dst2 = eng.new_cache()
+    idx_v2, idx_a2 = eng.new_indices()
+    M_v2 = torch.zeros(L, dtype=torch.int32, device=dev)
+    M_a2 = torch.zeros_like(M_v2)
+    eng.compress_chunk(src, chunk, Bt, dst2, idx_v=idx_v2, idx_a=idx_a2, M_v=M_v2, M_a=M_a2)
+    torch.cuda.synchronize()
+    mv, ma = M_v2.cpu().numpy(), M_a2.cpu().numpy()
+    iv, ia = idx_v2.cpu().numpy(), idx_a2.cpu().numpy()
+    n_diff = 0
+    for l in range(L):
+        assert mv[l] + ma[l] == min(wl.budget, Kv[l] + Ka[l])
+        if mv[l] != orc["M_v"][l]:   # allowed only when w_v B sits within tol B of a half-integer
+            st = orc["stats"][l]
+            wv = 5.0 * st[4] / (5.0 * st[4] + st[5])
+            assert abs(mv[l] - orc["M_v"][l]) <= max(1, int(tol * wl.budget)) and \
+                abs((wv * wl.budget) % 1.0 - 0.5) < tol * wl.budget, f"M_v[{l}] {mv[l]} vs {orc['M_v'][l]}"
+            continue
+        for h in range(wl.Hkv):
+            n_diff += kept_sets_rule_c(f"v[{l},{h}]", iv[l, h], orc["idx_v"][l, h], int(mv[l]), orc["psi_v"][l, h, :Kv[l]], tol)
+            n_diff += kept_sets_rule_c(f"a[{l},{h}]", ia[l, h], orc["idx_a"][l, h], int(ma[l]), orc["psi_a"][l, h, :Ka[l]], tol)
+    # whatever was kept, dst rows are byte-exact copies of the rows the GPU's indices name
+    dK2 = dst2.k.cpu().view(torch.uint8).numpy()
+    rawc, rawk = x["cacheK"].view(torch.uint8).numpy(), x["chunkK"].view(torch.uint8).numpy()
+    for l in range(L):
+        for h in range(wl.Hkv):
+            vis = np.concatenate([rawc[l, h, :n_v[l]], rawk[l, h, :wl.Nn_v]])
+            aud = np.concatenate([rawc[l, h, n_v[l]:n[l]], rawk[l, h, wl.Nn_v:]])
+            assert np.array_equal(dK2[l, h, :mv[l]], vis[iv[l, h, :mv[l]]])
+            assert np.array_equal(dK2[l, h, mv[l]:mv[l] + ma[l]], aud[ia[l, h, :ma[l]]])
+    eng.close()
+    return n_diff
+
+
+# ---------------------------------------------------------------------------------------------- CFG1 (fp32, SIMT)
+def test_cfg1_full():
+    assert check_step(I.CFG1) == 0                 # fp32: the kept sets must be identical
+
+
+def test_cfg1_paper_literal_stride_and_key_similarity():
+    wl = I.CFG1.replace(sim_stride_v=1)
+    check_step(wl)
+    check_step(wl, sim_source=1)
+
+
+# ---------------------------------------------------------------------------------------------- bf16, tcgen05 path
+SMALL2 = I.CFG2.replace(L=2, Hq=4, Hkv=2, n_v=700, n_a=150, Nn_v=400, Nn_a=123, budget=850, cache_cap=850)
+SMALL3 = I.CFG3.replace(L=2, Hq=4, Hkv=2, n_v=1024, n_a=200, Nn_v=512, Nn_a=100, budget=1224, cache_cap=1300)
+SMALL4 = I.CFG4.replace(L=2, Hq=4, Hkv=1, n_v=333, n_a=67, Nn_v=512, Nn_a=70, budget=400, cache_cap=400)
+
+
+@pytest.mark.parametrize("wl", [SMALL2, SMALL3, SMALL4], ids=lambda w: w.name)
+def test_bf16_tcgen05_small(wl):
+    check_step(wl)
+
+
+@pytest.mark.parametrize("wl", [SMALL2, SMALL4], ids=lambda w: w.name)
+def test_bf16_simt_path_small(wl):
+    check_step(wl, eng_kw=dict(score_path=1))
+
+
+def test_bf16_head_dim_64_simt():
+    check_step(SMALL2.replace(D=64))
+
+
+def test_noncausal_and_lambda_zero():
+    check_step(SMALL2, eng_kw=dict(causal=0), ref_kw=dict(causal=0))
+    check_step(SMALL3, eng_kw=dict(lam=0.0), ref_kw=dict(lam=0.0))      # cosine-only ablation
+    check_step(I.CFG1, eng_kw=dict(causal=0, lam=1.0, ratio_r=2.0), ref_kw=dict(causal=0, lam=1.0, ratio_r=2.0))
+
+
+def test_edge_shapes():
+    check_step(SMALL2.replace(n_a=0, Nn_a=0))                     # single modality ("no split")
+    check_step(SMALL2.replace(n_v=0, n_a=0))                      # empty cache (first chunk of a stream)
+    check_step(SMALL2.replace(budget=2000, cache_cap=2000))       # nothing to evict: keep all, identity indices
+    check_step(SMALL2.replace(Nn_v=1, Nn_a=0))                    # one-token chunk
+    check_step(SMALL2.replace(n_v=128, n_a=128, Nn_v=128, Nn_a=128, budget=256, cache_cap=256))   # tile-aligned
+    check_step(I.CFG1.replace(n_v=0, n_a=64, Nn_v=0, cache_cap=200, budget=40))                  # audio only
+
+
+def test_empty_chunk_keeps_everything():
+    wl = SMALL2.replace(Nn_v=0, Nn_a=0, budget=850)
+    x = I.full_inputs(SMALL2)
+    x["chunkK"], x["chunkV"], x["Q"] = x["chunkK"][:, :, :0], x["chunkV"][:, :, :0], x["Q"][:, :, :0]
+    check_step(wl, x=x, check_rowH=False)
+
+
+def test_supplied_lse_skips_pass1():
+    """chunk.lse given (the model's attention forward already has it): pass 2 alone must reproduce a."""
+    from paper_2606_07577_b200.omnimem import Chunk
+    for wl, kw in ((SMALL3, {}), (I.CFG1, {})):
+        x = I.full_inputs(wl)
+        L = x["Q"].shape[0]
+        p = ref_params(wl, L)
+        orc = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+        eng = engine_for(wl.replace(L=L), **kw)
+        src, chunk = dev_objs(x, wl)
+        chunk = Chunk(chunk.k, chunk.v, chunk.q, wl.Nn_v, wl.Nn_a, lse=torch.from_numpy(orc["lse"]).float().cuda())
+        eng.set_profiling(True)
+        sc = eng.score(src, chunk)
+        torch.cuda.synchronize()
+        ms, _ = eng.stage_ms()
+        assert ms["lse"] == 0.0 and ms["colsum"] > 0.0
+        compare_scores(wl, x["n_v"].numpy(), x["n"].numpy(), scores_to_numpy(sc), orc, TOL[wl.dtype])
+        eng.close()
+
+
+# ---------------------------------------------------------------------------------------------- rule (b) at scale
+def test_select_compact_bit_exact_with_ties_large():
+    """Random fp32 scores with many ties and negative zeros, ragged per-layer budgets: select + compact are bit-exact."""
+    from paper_2606_07577_b200.omnimem import Cache, Chunk
+    wl = I.CFG2.replace(L=3, Hq=2, Hkv=2, n_v=20000, n_a=3000, Nn_v=4096, Nn_a=1500, cache_cap=23000, budget=16384)
+    L = wl.L
+    eng = engine_for(wl)
+    p = ref_params(wl, L)
+    g = np.random.default_rng(5)
+    n_v = np.array([20000, 17000, 1], np.int32)
+    n = np.array([23000, 18001, 3], np.int32)
+    psi_v = np.round(g.random((L, wl.Hkv, p.seg_cap_v)), 3).astype(np.float32)       # ~1000 distinct values: heavy ties
+    psi_a = (g.random((L, wl.Hkv, p.seg_cap_a)).astype(np.float32)) ** 8
+    psi_a[0, 0, :50] = -0.0
+    psi_a[0, 0, 50:100] = 0.0
+    psi_v[1, 1] = 0.25                                                               # all equal
+    Kv, Ka = seg_lens(wl, n_v, n)
+    M_v = np.array([13000, 9999, 0], np.int32)
+    M_a = np.array([3384, 2000, 700], np.int32)
+    M_v[2] = Kv[2]                                                                   # keep every visual row
+    iv_ref, ia_ref = ref.select(p, psi_v, psi_a, n_v, n, M_v, M_a)
+    t = lambda a: torch.from_numpy(a).cuda()
+    iv, ia = eng.select(t(psi_v), t(psi_a), t(n_v), t(n), wl.Nn_v, wl.Nn_a, t(M_v), t(M_a))
+    iv, ia = iv.cpu().numpy(), ia.cpu().numpy()
+    for l in range(L):
+        assert np.array_equal(iv[l, :, :M_v[l]], iv_ref[l, :, :M_v[l]]) and np.array_equal(ia[l, :, :M_a[l]], ia_ref[l, :, :M_a[l]])
+    gK = torch.Generator().manual_seed(1)
+    cacheK = torch.randn(L, wl.Hkv, wl.cache_cap, wl.D, generator=gK).to(torch.bfloat16)
+    cacheV = torch.randn(L, wl.Hkv, wl.cache_cap, wl.D, generator=gK).to(torch.bfloat16)
+    chunkK = torch.randn(L, wl.Hkv, wl.Nn, wl.D, generator=gK).to(torch.bfloat16)
+    chunkV = torch.randn(L, wl.Hkv, wl.Nn, wl.D, generator=gK).to(torch.bfloat16)
+    dK_ref, nv2, n2 = ref.compact(p, cacheK, chunkK, n_v, n, iv_ref, ia_ref, M_v, M_a)
+    dV_ref, _, _ = ref.compact(p, cacheV, chunkV, n_v, n, iv_ref, ia_ref, M_v, M_a)
+    src = Cache(cacheK.cuda(), cacheV.cuda(), t(n_v), t(n))
+    chunk = Chunk(chunkK.cuda(), chunkV.cuda(), chunkK.cuda(), wl.Nn_v, wl.Nn_a)
+    dst = eng.new_cache()
+    eng.compact(src, chunk, t(iv_ref), t(ia_ref), t(M_v), t(M_a), dst)
+    torch.cuda.synchronize()
+    dK, dV = dst.k.cpu().view(torch.uint8).numpy(), dst.v.cpu().view(torch.uint8).numpy()
+    for l in range(L):
+        assert np.array_equal(dK[l, :, :n2[l]], dK_ref[l, :, :n2[l]]) and np.array_equal(dV[l, :, :n2[l]], dV_ref[l, :, :n2[l]])
+    assert np.array_equal(dst.n.cpu().numpy(), n2) and np.array_equal(dst.n_v.cpu().numpy(), nv2)
+    eng.close()
+
+
+def test_layer_budgets_eq14_on_device():
+    """Eq.13-14 in omnimem_allocate (layer_budget == NULL) against the oracle (itself pinned only by invariants, R20)."""
+    wl = I.CFG1.replace(L=9)
+    L = wl.L
+    st = np.zeros((L, 8))
+    g = np.random.default_rng(2)
+    st[:, 6], st[:, 7] = g.uniform(0.5, 0.95, L), g.uniform(0.0, 0.5, L)
+    st[:, 4], st[:, 5] = g.uniform(0.1, 0.9, L), g.uniform(0.1, 0.9, L)
+    n_v, n = np.full(L, 512, np.int32), np.full(L, 576, np.int32)
+    for bmin, bmax in ((0, 0), (200, 320)):
+        eng = engine_for(wl, budget_min=bmin, budget_max=bmax)
+        p = ref_params(wl, L, budget_min=bmin, budget_max=bmax)
+        B_ref = ref.layer_budgets(p, st, 256 * L)
+        M_v_ref, M_a_ref = ref.allocate(p, st, n_v, n, B_ref)
+        t = lambda a: torch.from_numpy(a).cuda()
+        M_v, M_a, B = eng.allocate(t(st), t(n_v), t(n), wl.Nn_v, wl.Nn_a, None, 256 * L)
+        assert np.array_equal(B.cpu().numpy(), B_ref) and B_ref.sum() == 256 * L
+        assert np.array_equal(M_v.cpu().numpy(), M_v_ref) and np.array_equal(M_a.cpu().numpy(), M_a_ref)
+        eng.close()
+
+
+# ---------------------------------------------------------------------------------------------- streaming (cfg5 shape logic at cfg1 size)
+def test_streaming_free_running_small():
+    """Twelve consecutive chunks from an empty cache (append-only steps, first eviction, steady state), both sides
+    free-running on their own state; fp32 so the kept sets must stay identical at every step."""
+    from paper_2606_07577_b200.omnimem import Chunk
+    wl = I.CFG1.replace(n_v=0, n_a=0, budget=300, cache_cap=300, steps=12, recipe="ar1")
+    L = wl.L
+    eng = engine_for(wl)
+    p = ref_params(wl, L)
+    B = np.full((L,), wl.budget, np.int32)
+    Bt = torch.from_numpy(B).cuda()
+    src, dst = eng.new_cache(), eng.new_cache()
+    rK = np.zeros((L, wl.Hkv, wl.cache_cap, wl.D), np.float32)
+    rV = np.zeros_like(rK)
+    r_nv, r_n = np.zeros(L, np.int32), np.zeros(L, np.int32)
+    for step in range(wl.steps):
+        x = I.full_inputs(wl, step=step, with_cache=False)
+        orc = ref.compress_chunk(p, rK, rV, r_nv, r_n, x["chunkK"], x["chunkV"], x["Q"], B)
+        rK = orc["dstK"].view(np.float32).reshape(rK.shape)
+        rV = orc["dstV"].view(np.float32).reshape(rV.shape)
+        r_nv, r_n = orc["n_v_out"], orc["n_out"]
+        chunk = Chunk(x["chunkK"].cuda(), x["chunkV"].cuda(), x["Q"].cuda(), wl.Nn_v, wl.Nn_a)
+        eng.compress_chunk(src, chunk, Bt, dst)
+        src, dst = dst, src
+        torch.cuda.synchronize()
+        assert np.array_equal(src.n.cpu().numpy(), r_n) and np.array_equal(src.n_v.cpu().numpy(), r_nv), f"step {step}"
+        for l in range(L):
+            assert np.array_equal(src.k[l, :, :r_n[l]].cpu().numpy(), rK[l, :, :r_n[l]]), f"step {step} layer {l}"
+            assert np.array_equal(src.v[l, :, :r_n[l]].cpu().numpy(), rV[l, :, :r_n[l]])
+    assert r_n.max() == wl.budget
+    eng.close()
+
+
+def test_error_codes():
+    from paper_2606_07577_b200.omnimem import OmniMem, OmniMemError, Chunk
+    with pytest.raises(OmniMemError):
+        OmniMem(L=1, Hq=3, Hkv=2, D=64, dtype="fp32", cache_cap=8, max_chunk_v=4, max_chunk_a=4)     # Hq % Hkv
+    with pytest.raises(OmniMemError):
+        OmniMem(L=1, Hq=2, Hkv=2, D=96, dtype="fp32", cache_cap=8, max_chunk_v=4, max_chunk_a=4)     # head_dim
+    wl = I.CFG1
+    eng = engine_for(wl)
+    x = I.full_inputs(wl)
+    src, chunk = dev_objs(x, wl)
+    big = Chunk(chunk.k, chunk.v, chunk.q, wl.Nn_v + 1, wl.Nn_a)
+    with pytest.raises(OmniMemError, match="capacities"):
+        eng.score(src, big)
+    Bt = torch.full((wl.L,), wl.budget, dtype=torch.int32, device="cuda")
+    with pytest.raises(OmniMemError, match="invalid"):
+        eng.compress_chunk(src, chunk, Bt, src)                                                   # dst aliases src
+    eng.close()

@@ -345,6 +345,15 @@ def test_layer_budgets_invariants():
     b = ref.layer_budgets(p, st, 7 * 8192)
     assert b.sum() == 7 * 8192 and b.min() >= 4096 and b.max() <= 12288
     assert b[0] == 4096 and b[-1] == 12288
+    # two-sided clamp where both bounds bite: the total must survive (one side is fixed per round)
+    g = np.random.default_rng(2)
+    st9 = np.zeros((9, 8))
+    st9[:, 6], st9[:, 7] = g.uniform(0.5, 0.95, 9), g.uniform(0.0, 0.5, 9)
+    p9 = ref.RefParams(L=9, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=0.2, budget_min=200, budget_max=320)
+    b = ref.layer_budgets(p9, st9, 256 * 9)
+    assert b.sum() == 256 * 9 and b.min() >= 200 and b.max() <= 320
+    C9 = st9[:, 6] * (1 - st9[:, 7])
+    assert np.all(np.diff(b[np.argsort(C9)]) >= 0)            # monotone in compressibility
 
 
 # ------------------------------------------------------------------------------------------ O7 (Eq.4-5)
