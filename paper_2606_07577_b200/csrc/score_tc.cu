@@ -7,8 +7,10 @@
 //                        queries is thread-local: a_k = sum_{g,i} 2^(c2 s - lse2_i).  No atomics, no shuffles.
 // One CTA holds two stationary 128-row sub-tiles (A operand, 64 KB) and streams 128-row tiles of the other
 // operand (B, 32 KB stages) by TMA; one thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile) into a
-// double-buffered 128-column TMEM accumulator per sub-tile; two 4-warp softmax groups drain them with
-// tcgen05.ld 32x32b.  Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-7 / 8-11 = epilogue.
+// double-buffered 128-column TMEM accumulator per sub-tile; four 4-warp epilogue groups (sub-tile x column half)
+// drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns, frees the TMEM buffer
+// as soon as its registers hold the data, and merges with its partner thread once, at the end.
+// Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-19 = epilogue.
 #include <cuda.h>
 #include <math.h>
 
@@ -22,9 +24,15 @@ constexpr int kKBlock = 64;        // bf16 elements per 128-byte swizzle atom ro
 constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16 KB K-blocks
 constexpr int kKBlockBytes = kTile * kKBlock * 2; // 16 KB
 constexpr int kStages = 4;
-constexpr int kThreads = 384;
+constexpr int kThreads = 640;       // 4 control warps + 16 epilogue warps (4 groups: sub-tile x column half)
 constexpr int kTmemCols = 512;
-constexpr size_t kSmemBytes = 1024 /*align slack*/ + 2 * kTileBytes + kStages * kTileBytes + 256 /*barriers*/;
+constexpr int kLseSlots = 16;       // pass 2: ring of 128-float lse2 tiles (512 B each); see the reuse argument at the producer
+constexpr int kHalf = kTile / 2;    // columns of a tile owned by one epilogue thread
+constexpr int kOffB = 2 * kTileBytes;
+constexpr int kOffLse = kOffB + kStages * kTileBytes;
+constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 rows] float4
+constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
+constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
 // ---- PTX wrappers -------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -50,6 +58,18 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
           "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -185,17 +205,21 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const uint32_t sA = smem_u32(smem);                    // [2 sub][2 kb][16 KB]
-  const uint32_t sB = sA + 2 * kTileBytes;               // [kStages][2 kb][16 KB]
-  const uint32_t bars = sB + kStages * kTileBytes;
+  const uint32_t sB = sA + kOffB;                        // [kStages][2 kb][16 KB]
+  const uint32_t sLse = sA + kOffLse;                    // [kLseSlots][128] float (pass 2)
+  float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 sub][128]
+  const uint32_t bars = sA + kOffBars;
   const uint32_t bar_full = bars, bar_empty = bars + 8 * kStages, bar_a = bars + 16 * kStages;
   const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 32;  // [sub*2+buf]
-  uint32_t* tmem_slot = (uint32_t*)(smem + 2 * kTileBytes + kStages * kTileBytes + 16 * kStages + 8 + 64);
+  const uint32_t bar_lse = bar_sempty + 32;                           // [kLseSlots]
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 64 + 8 * kLseSlots);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
     mbar_init(bar_a, 1);
-    for (int i = 0; i < 4; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 4); }
+    for (int i = 0; i < 4; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
+    for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
@@ -231,6 +255,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           mB = &mapQ;
           row0 = (w.it0[0] + j % w.tiles_per_g) * kTile;
           lh = w.hq0 + j / w.tiles_per_g;
+          // lse2 of these 128 queries: its own ring + barrier; slot j % 16 was last read for tile j - 16; every
+          // epilogue thread finished computing that tile before the MMA of tile j - 4 completed (TMEM buffers are 2 deep,
+          // a sub-tile skips at most every other tile), and this load is issued after that MMA freed the B stage.
+          const int slot = j % kLseSlots;
+          mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
+          bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
         }
         for (int kb = 0; kb < 2; ++kb)
           tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
@@ -266,12 +296,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
-    const int s = (warp - 4) >> 2;       // sub-tile
-    const int q4 = warp & 3;             // TMEM lane quarter owned by this warp
+    const int grp = (warp - 4) >> 2;     // 0..3
+    const int s = grp >> 1;              // sub-tile
+    const int half = grp & 1;            // which 64 of the tile's 128 columns
+    const int q4 = warp & 3;             // TMEM lane quarter this warp may touch
     const int r = q4 * 32 + lane;        // row of the sub-tile == TMEM lane
+    const int col0 = half * kHalf;
     const float c2 = p.scale_log2e;
     if (w.sub_valid[s]) {
-      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16) + (uint32_t)col0;
       int js = 0;
       if (kPass == 1) {
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
@@ -279,7 +312,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         float m_run = -1e30f, Z = 0.f, W = 0.f;
         for (int j = 0; j < w.ntiles_sub[s]; ++j, ++js) {
           const int buf = js & 1;
-          // number of visible key columns of this tile for this row
+          // number of visible key columns of this tile for this row, relative to this thread's first column
           int limit;
           if (j < w.n_cache_tiles) limit = n - j * kTile;
           else {
@@ -287,51 +320,62 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             limit = p.Nn - t0;
             if (p.causal) limit = min(limit, i - t0 + 1);
           }
+          limit -= col0;
           mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
           tc_fence_after();
           const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
-#pragma unroll 1
-          for (int c = 0; c < 4; ++c) {
-            uint32_t v[32];
-            tc_ld32(t_addr + c * 32, v);
-            tc_wait_ld();
-            float x[32];
-            const int lim_c = limit - c * 32;
-            if (lim_c >= 32) {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) x[e] = __uint_as_float(v[e]);
-            } else {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) x[e] = e < lim_c ? __uint_as_float(v[e]) : -INFINITY;
-            }
-            float mx[4] = {x[0], x[1], x[2], x[3]};
-#pragma unroll
-            for (int e = 4; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], x[e]);
-            const float cmax = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
-            const float m_new = fmaxf(m_run, cmax * c2);
-            const float rs = ex2(m_run - m_new);
-            m_run = m_new;
-            float z[4] = {0.f, 0.f, 0.f, 0.f}, wz[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int e = 0; e < 32; ++e) {
-              const float pe = ex2(fmaf(x[e], c2, -m_new));
-              z[e & 3] += pe;
-              if (kEntropy) wz[e & 3] = fmaf(pe, lim_c > e ? x[e] * c2 : 0.f, wz[e & 3]);
-            }
-            Z = fmaf(Z, rs, (z[0] + z[1]) + (z[2] + z[3]));
-            if (kEntropy) W = fmaf(W, rs, (wz[0] + wz[1]) + (wz[2] + wz[3]));
-          }
+          uint32_t v0[32], v1[32];
+          tc_ld32(t_addr, v0);
+          tc_ld32(t_addr + 32, v1);
+          tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));
+          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));  // registers hold the tile: free the TMEM buffer
+          float x[kHalf];
+          if (limit >= kHalf) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) { x[e] = __uint_as_float(v0[e]); x[32 + e] = __uint_as_float(v1[e]); }
+          } else {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+              x[e] = e < limit ? __uint_as_float(v0[e]) : -INFINITY;
+              x[32 + e] = 32 + e < limit ? __uint_as_float(v1[e]) : -INFINITY;
+            }
+          }
+          float mx[4] = {x[0], x[1], x[2], x[3]};
+#pragma unroll
+          for (int e = 4; e < kHalf; ++e) mx[e & 3] = fmaxf(mx[e & 3], x[e]);
+          const float cmax = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+          const float m_new = fmaxf(m_run, cmax * c2);
+          const float rs = ex2(m_run - m_new);
+          m_run = m_new;
+          float z[4] = {0.f, 0.f, 0.f, 0.f}, wz[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int e = 0; e < kHalf; ++e) {
+            const float pe = ex2(fmaf(x[e], c2, -m_new));
+            z[e & 3] += pe;
+            if (kEntropy) wz[e & 3] = fmaf(pe, limit > e ? x[e] * c2 : 0.f, wz[e & 3]);
+          }
+          Z = fmaf(Z, rs, (z[0] + z[1]) + (z[2] + z[3]));
+          if (kEntropy) W = fmaf(W, rs, (wz[0] + wz[1]) + (wz[2] + wz[3]));
         }
-        // lse2 = log2 sum_k 2^(c2 s_k); padded rows (i >= Nn) publish +inf so that pass 2 adds nothing for them
-        const long long hq = (long long)w.lhA;
-        const float l2 = m_run + log2f(Z);
-        a.lse2[hq * a.lse_stride + i] = i < p.Nn ? l2 : INFINITY;
-        if (i < p.Nn) {
-          if (a.lse_nat) a.lse_nat[hq * p.Nn + i] = l2 * 0.6931471805599453f;
-          if (kEntropy && a.row_entropy) a.row_entropy[hq * p.Nn + i] = (l2 - W / Z) * 0.6931471805599453f;
+        // merge the two column halves of each row (online-softmax partials), then publish
+        if (half == 1) sMerge[s * kTile + r] = make_float4(m_run, Z, W, 0.f);
+        named_bar_sync(1 + s, 256);
+        if (half == 0) {
+          const float4 o = sMerge[s * kTile + r];
+          const float m = fmaxf(m_run, o.x);
+          const float r0 = ex2(m_run - m), r1 = ex2(o.x - m);
+          Z = Z * r0 + o.y * r1;
+          W = W * r0 + o.z * r1;
+          // lse2 = log2 sum_k 2^(c2 s_k); padded rows (i >= Nn) publish +inf so that pass 2 adds nothing for them
+          const long long hq = (long long)w.lhA;
+          const float l2 = m + log2f(Z);
+          a.lse2[hq * a.lse_stride + i] = i < p.Nn ? l2 : INFINITY;
+          if (i < p.Nn) {
+            if (a.lse_nat) a.lse_nat[hq * p.Nn + i] = l2 * 0.6931471805599453f;
+            if (kEntropy && a.row_entropy) a.row_entropy[hq * p.Nn + i] = (l2 - W / Z) * 0.6931471805599453f;
+          }
         }
       } else {
         const int krow = w.rowA0 + s * kTile + r;  // key row in cache or chunk
@@ -339,49 +383,60 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         for (int j = 0; j < w.ntiles; ++j) {
           const int it = w.it0[0] + j % w.tiles_per_g;
           if (it < w.it0[s]) continue;
-          const int g = j / w.tiles_per_g;
           const int buf = js & 1;
-          // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column of this tile:
-          const int first = (p.causal && w.a_chunk) ? krow - it * kTile : 0;
-          const float4* l4 = reinterpret_cast<const float4*>(a.lse2 + (long long)(w.hq0 + g) * a.lse_stride + it * kTile);
+          // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
+          const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
           mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
           tc_fence_after();
           const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
-#pragma unroll 1
-          for (int c = 0; c < 4; ++c) {
-            uint32_t v[32];
-            tc_ld32(t_addr + c * 32, v);
-            float ls[32];
-#pragma unroll
-            for (int e4 = 0; e4 < 8; ++e4) {
-              const float4 t4 = __ldg(l4 + c * 8 + e4);
-              ls[4 * e4] = t4.x; ls[4 * e4 + 1] = t4.y; ls[4 * e4 + 2] = t4.z; ls[4 * e4 + 3] = t4.w;
-            }
-            tc_wait_ld();
-            const int first_c = first - c * 32;
-            if (first_c <= 0) {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) acc[e & 3] += ex2(fmaf(__uint_as_float(v[e]), c2, -ls[e]));
-            } else {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) {
-                const float pe = ex2(fmaf(__uint_as_float(v[e]), c2, -ls[e]));
-                acc[e & 3] += e >= first_c ? pe : 0.f;
-              }
-            }
-          }
+          uint32_t v0[32], v1[32];
+          tc_ld32(t_addr, v0);
+          tc_ld32(t_addr + 32, v1);
+          tc_wait_ld();
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));
+          const int slot = j % kLseSlots;
+          mbar_wait(bar_lse + 8 * slot, (j / kLseSlots) & 1);
+          const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
+          if (first <= 0) {
+#pragma unroll
+            for (int e4 = 0; e4 < 8; ++e4) {
+              const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
+              acc[0] += ex2(fmaf(__uint_as_float(v0[4 * e4]), c2, -la.x));
+              acc[1] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 1]), c2, -la.y));
+              acc[2] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 2]), c2, -la.z));
+              acc[3] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 3]), c2, -la.w));
+              acc[0] += ex2(fmaf(__uint_as_float(v1[4 * e4]), c2, -lb.x));
+              acc[1] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 1]), c2, -lb.y));
+              acc[2] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 2]), c2, -lb.z));
+              acc[3] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 3]), c2, -lb.w));
+            }
+          } else {
+#pragma unroll
+            for (int e4 = 0; e4 < 8; ++e4) {
+              const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
+              const float le[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const float pa = ex2(fmaf(__uint_as_float(v0[4 * e4 + u]), c2, -le[u]));
+                const float pb = ex2(fmaf(__uint_as_float(v1[4 * e4 + u]), c2, -le[4 + u]));
+                acc[u] += (4 * e4 + u >= first ? pa : 0.f) + (32 + 4 * e4 + u >= first ? pb : 0.f);
+              }
+            }
+          }
           ++js;
         }
+        const float part = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+        if (half == 1) sMerge[s * kTile + r].x = part;
+        named_bar_sync(1 + s, 256);
         const int n_v = p.n_v[w.l], n = p.n[w.l];
         const bool valid = w.a_chunk ? krow < p.Nn : krow < n;
-        if (valid) {
+        if (half == 0 && valid) {
           int m, t;
           if (w.a_chunk) chunk_row_to_seg(p, n_v, n, krow, m, t); else cache_row_to_seg(n_v, krow, m, t);
           float* out = m == 0 ? a.a_v + (long long)w.lhA * p.seg_cap_v : a.a_a + (long long)w.lhA * p.seg_cap_a;
-          out[t] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+          out[t] = part + sMerge[s * kTile + r].x;
         }
       }
     }
