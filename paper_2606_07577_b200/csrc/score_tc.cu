@@ -49,10 +49,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
       "@p bra WAIT_DONE;\n\t"
       "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");  // suspend-time hint: sleep, do not spin
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
   asm volatile(
@@ -84,6 +84,11 @@ __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, ui
       "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+#ifdef OMNIMEM_DBG_NOLD
+#pragma unroll
+  for (int i = 0; i < 32; ++i) r[i] = taddr + i;   // timing experiment only
+  return;
+#endif
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
@@ -94,10 +99,58 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
       : "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// packed fp32x2 arithmetic (sm_100): one issue slot for two lanes' worth of FMA / ADD
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ uint64_t pack2u(uint32_t lo, uint32_t hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
 __device__ __forceinline__ float ex2(float x) {
+#ifdef OMNIMEM_DBG_NOEXP
+  return x;   // timing experiment only: results are wrong
+#endif
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+
+// 2^x on the FMA/ALU pipes for x <= 0 (Cody-Waite split + degree-4 minimax polynomial on [-0.5, 0.5], max relative
+// error 2.7e-6; coefficients fitted for this file).  The MUFU ex2 pipe (16/clk/SM) is the
+// limiter of both scoring passes; with kPolyEvery > 0 every kPolyEvery-th exponential of a row is evaluated here.
+__device__ __forceinline__ float ex2_poly(float x) {
+  x = fmaxf(x, -126.f);            // keeps the biased exponent of q * 2^round(x) >= 0
+  const float t = x + 12582912.f;  // 1.5 * 2^23: the low mantissa bits of t now hold round(x)
+  const float f = x - (t - 12582912.f);
+  float q = fmaf(0.009570066817104816f, f, 0.05591786280274391f);
+  q = fmaf(q, f, 0.2402474582195282f);
+  q = fmaf(q, f, 0.6931217908859253f);
+  q = fmaf(q, f, 0.9999992847442627f);
+  return __int_as_float(__float_as_int(q) + (__float_as_int(t) << 23));  // q * 2^round(x)
+}
+#ifndef OMNIMEM_POLY_EVERY
+#define OMNIMEM_POLY_EVERY 0
+#endif
+constexpr int kPolyEvery = OMNIMEM_POLY_EVERY;
+__device__ __forceinline__ float ex2_sel(float x, int idx) {
+  return (kPolyEvery > 0 && (idx % (kPolyEvery > 0 ? kPolyEvery : 1)) == kPolyEvery - 1) ? ex2_poly(x) : ex2(x);
 }
 
 // UMMA shared-memory descriptor, K-major, 128-byte swizzle: 8-row groups are 1024 B apart (SBO), LBO unused,
@@ -114,7 +167,7 @@ constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTi
 
 struct TcArgs {
   StepParams p;
-  float* lse2;         // [L, Hq, lse_stride] log2-domain LSE (internal, padded rows hold +inf)
+  float* lse2;         // [L, Hq, lse_stride] NEGATED log2-domain LSE (internal; padded rows hold -inf)
   int lse_stride;
   float* lse_nat;      // pass 1: optional natural-log output [L, Hq, Nn]
   float* row_entropy;  // pass 1: optional [L, Hq, Nn]
@@ -285,8 +338,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
             const uint32_t koff = (uint32_t)((kk >> 2) * kKBlockBytes + (kk & 3) * 32);
+#ifndef OMNIMEM_DBG_NOMMA
             tc_mma_bf16(d_tmem, umma_desc_sw128(sA + s * kTileBytes + koff), umma_desc_sw128(sB + stage * kTileBytes + koff),
                         kIdesc, kk > 0 ? 1u : 0u);
+#endif
           }
           tc_commit(bar_sfull + 8 * (s * 2 + buf));
           ++js[s];
@@ -349,14 +404,28 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const float m_new = fmaxf(m_run, cmax * c2);
           const float rs = ex2(m_run - m_new);
           m_run = m_new;
-          float z[4] = {0.f, 0.f, 0.f, 0.f}, wz[4] = {0.f, 0.f, 0.f, 0.f};
+          float wz[4] = {0.f, 0.f, 0.f, 0.f};
+          uint64_t z01 = 0ull, z23 = 0ull;  // packed fp32x2 partial sums
+          const uint64_t c2c2 = pack2(c2, c2), nm = pack2(-m_new, -m_new);
 #pragma unroll
-          for (int e = 0; e < kHalf; ++e) {
-            const float pe = ex2(fmaf(x[e], c2, -m_new));
-            z[e & 3] += pe;
-            if (kEntropy) wz[e & 3] = fmaf(pe, limit > e ? x[e] * c2 : 0.f, wz[e & 3]);
+          for (int e = 0; e < kHalf; e += 4) {
+            float a0, a1, a2, a3;
+            unpack2(fma2(pack2(x[e], x[e + 1]), c2c2, nm), a0, a1);
+            unpack2(fma2(pack2(x[e + 2], x[e + 3]), c2c2, nm), a2, a3);
+            const float p0 = ex2_sel(a0, e), p1 = ex2_sel(a1, e + 1), p2 = ex2_sel(a2, e + 2), p3 = ex2_sel(a3, e + 3);
+            z01 = add2(z01, pack2(p0, p1));
+            z23 = add2(z23, pack2(p2, p3));
+            if (kEntropy) {  // sum p z2 over visible columns (masked ones have p = 0 but z2 = -inf)
+              wz[0] = fmaf(p0, limit > e ? a0 + m_new : 0.f, wz[0]);
+              wz[1] = fmaf(p1, limit > e + 1 ? a1 + m_new : 0.f, wz[1]);
+              wz[2] = fmaf(p2, limit > e + 2 ? a2 + m_new : 0.f, wz[2]);
+              wz[3] = fmaf(p3, limit > e + 3 ? a3 + m_new : 0.f, wz[3]);
+            }
           }
-          Z = fmaf(Z, rs, (z[0] + z[1]) + (z[2] + z[3]));
+          float z0, z1, z2, z3;
+          unpack2(z01, z0, z1);
+          unpack2(z23, z2, z3);
+          Z = fmaf(Z, rs, (z0 + z1) + (z2 + z3));
           if (kEntropy) W = fmaf(W, rs, (wz[0] + wz[1]) + (wz[2] + wz[3]));
         }
         // merge the two column halves of each row (online-softmax partials), then publish
@@ -368,10 +437,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const float r0 = ex2(m_run - m), r1 = ex2(o.x - m);
           Z = Z * r0 + o.y * r1;
           W = W * r0 + o.z * r1;
-          // lse2 = log2 sum_k 2^(c2 s_k); padded rows (i >= Nn) publish +inf so that pass 2 adds nothing for them
+          // lse2 = log2 sum_k 2^(c2 s_k), stored negated; padded rows (i >= Nn) publish -inf so that pass 2 adds 2^-inf = 0
           const long long hq = (long long)w.lhA;
           const float l2 = m + log2f(Z);
-          a.lse2[hq * a.lse_stride + i] = i < p.Nn ? l2 : INFINITY;
+          a.lse2[hq * a.lse_stride + i] = i < p.Nn ? -l2 : -INFINITY;  // stored NEGATED: pass 2 does one FMA
           if (i < p.Nn) {
             if (a.lse_nat) a.lse_nat[hq * p.Nn + i] = l2 * 0.6931471805599453f;
             if (kEntropy && a.row_entropy) a.row_entropy[hq * p.Nn + i] = (l2 - W / Z) * 0.6931471805599453f;
@@ -380,6 +449,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       } else {
         const int krow = w.rowA0 + s * kTile + r;  // key row in cache or chunk
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        uint64_t acc01 = 0ull, acc23 = 0ull;   // packed fp32x2 partial sums of the unmasked tiles
+        const uint64_t c2c2 = pack2(c2, c2);
         for (int j = 0; j < w.ntiles; ++j) {
           const int it = w.it0[0] + j % w.tiles_per_g;
           if (it < w.it0[s]) continue;
@@ -403,14 +474,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 #pragma unroll
             for (int e4 = 0; e4 < 8; ++e4) {
               const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
-              acc[0] += ex2(fmaf(__uint_as_float(v0[4 * e4]), c2, -la.x));
-              acc[1] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 1]), c2, -la.y));
-              acc[2] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 2]), c2, -la.z));
-              acc[3] += ex2(fmaf(__uint_as_float(v0[4 * e4 + 3]), c2, -la.w));
-              acc[0] += ex2(fmaf(__uint_as_float(v1[4 * e4]), c2, -lb.x));
-              acc[1] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 1]), c2, -lb.y));
-              acc[2] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 2]), c2, -lb.z));
-              acc[3] += ex2(fmaf(__uint_as_float(v1[4 * e4 + 3]), c2, -lb.w));
+              float p0, p1, p2, p3, p4, p5, p6, p7;
+              unpack2(fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y)), p0, p1);
+              unpack2(fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w)), p2, p3);
+              unpack2(fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y)), p4, p5);
+              unpack2(fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w)), p6, p7);
+              acc01 = add2(acc01, pack2(ex2_sel(p0, 4 * e4), ex2_sel(p1, 4 * e4 + 1)));
+              acc23 = add2(acc23, pack2(ex2_sel(p2, 4 * e4 + 2), ex2_sel(p3, 4 * e4 + 3)));
+              acc01 = add2(acc01, pack2(ex2_sel(p4, 4 * e4), ex2_sel(p5, 4 * e4 + 1)));
+              acc23 = add2(acc23, pack2(ex2_sel(p6, 4 * e4 + 2), ex2_sel(p7, 4 * e4 + 3)));
             }
           } else {
 #pragma unroll
@@ -419,15 +491,18 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
               const float le[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
 #pragma unroll
               for (int u = 0; u < 4; ++u) {
-                const float pa = ex2(fmaf(__uint_as_float(v0[4 * e4 + u]), c2, -le[u]));
-                const float pb = ex2(fmaf(__uint_as_float(v1[4 * e4 + u]), c2, -le[4 + u]));
+                const float pa = ex2(fmaf(__uint_as_float(v0[4 * e4 + u]), c2, le[u]));
+                const float pb = ex2(fmaf(__uint_as_float(v1[4 * e4 + u]), c2, le[4 + u]));
                 acc[u] += (4 * e4 + u >= first ? pa : 0.f) + (32 + 4 * e4 + u >= first ? pb : 0.f);
               }
             }
           }
           ++js;
         }
-        const float part = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+        float q0, q1, q2, q3;
+        unpack2(acc01, q0, q1);
+        unpack2(acc23, q2, q3);
+        const float part = ((acc[0] + acc[1]) + (acc[2] + acc[3])) + ((q0 + q1) + (q2 + q3));
         if (half == 1) sMerge[s * kTile + r].x = part;
         named_bar_sync(1 + s, 256);
         const int n_v = p.n_v[w.l], n = p.n[w.l];
@@ -455,7 +530,7 @@ __global__ void lse_to_log2_kernel(const float* __restrict__ lse_nat, float* __r
   if (idx >= (long long)rows * stride) return;
   const int i = (int)(idx % stride);
   const long long r = idx / stride;
-  lse2[idx] = i < Nn ? lse_nat[r * Nn + i] * 1.4426950408889634f : INFINITY;
+  lse2[idx] = i < Nn ? -lse_nat[r * Nn + i] * 1.4426950408889634f : -INFINITY;
 }
 
 // ---- host side -------------------------------------------------------------------------------------------------
