@@ -23,13 +23,14 @@ constexpr int kHeadDim = 128;      // D
 constexpr int kKBlock = 64;        // bf16 elements per 128-byte swizzle atom row
 constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16 KB K-blocks
 constexpr int kKBlockBytes = kTile * kKBlock * 2; // 16 KB
-constexpr int kStages = 4;
+constexpr int kStages = 6;          // B ring (32 KB stages)
 constexpr int kThreads = 640;       // 4 control warps + 16 epilogue warps (4 groups: sub-tile x column half)
 constexpr int kTmemCols = 512;
+constexpr int kAccBufs = 3;         // TMEM accumulator ring shared by both sub-tiles: columns [0, 384)
+constexpr int kTmemA = kAccBufs * kTile;  // stationary operand: 64 columns per sub-tile at [384, 512)
 constexpr int kLseSlots = 16;       // pass 2: ring of 128-float lse2 tiles (512 B each); see the reuse argument at the producer
 constexpr int kHalf = kTile / 2;    // columns of a tile owned by one epilogue thread
-constexpr int kOffB = 2 * kTileBytes;
-constexpr int kOffLse = kOffB + kStages * kTileBytes;
+constexpr int kOffLse = kStages * kTileBytes;
 constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 rows] float4
 constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
@@ -71,6 +72,13 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
+// one lane of a fully converged warp (the rest of the warp keeps executing the same uniform control flow)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ int uniform(int x) { return __shfl_sync(0xffffffffu, x, 0); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
@@ -97,6 +105,19 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tc_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+               :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+}
+__device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// D[tmem] (+)= A[tmem] * B[smem]^T : the stationary operand is read from tensor memory, only B from shared memory
+__device__ __forceinline__ void tc_mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
+      "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // packed fp32x2 arithmetic (sm_100): one issue slot for two lanes' worth of FMA / ADD
@@ -149,6 +170,11 @@ __device__ __forceinline__ float ex2_poly(float x) {
 #define OMNIMEM_POLY_EVERY 0
 #endif
 constexpr int kPolyEvery = OMNIMEM_POLY_EVERY;
+#ifdef OMNIMEM_DBG_NOACC
+#define OMNIMEM_DBG_ACC(kk) 0u
+#else
+#define OMNIMEM_DBG_ACC(kk) ((kk) > 0 ? 1u : 0u)
+#endif
 __device__ __forceinline__ float ex2_sel(float x, int idx) {
   return (kPolyEvery > 0 && (idx % (kPolyEvery > 0 ? kPolyEvery : 1)) == kPolyEvery - 1) ? ex2_poly(x) : ex2(x);
 }
@@ -174,6 +200,7 @@ struct TcArgs {
   float* a_v;          // pass 2 outputs
   float* a_a;
   int n_cache_pairs;   // pass 2: ceil(cache_cap / 256)
+  const __nv_bfloat16 *q, *kc, *kn;  // raw operands (stationary rows are staged into TMEM by the epilogue threads)
 };
 
 // What one CTA works on, computed identically by every role.
@@ -193,8 +220,9 @@ template <int kPass>
 __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
   const StepParams& p = a.p;
   w.l = blockIdx.z;
-  if (layer_skips_scoring(p, w.l)) return false;
-  const int n = p.n[w.l];
+  // values loaded from memory are made provably warp-uniform (shfl) so that the control warps stay on the uniform datapath
+  const int n = uniform(p.n[w.l]);
+  if (p.skip_budget != nullptr && n + p.Nn <= uniform(p.skip_budget[w.l])) return false;
   if (kPass == 1) {
     const int j = blockIdx.y;  // query head
     w.h = j / p.G;
@@ -257,21 +285,20 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   if (!make_work<kPass>(a, w)) return;  // uniform across the CTA
 
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  const uint32_t sA = smem_u32(smem);                    // [2 sub][2 kb][16 KB]
-  const uint32_t sB = sA + kOffB;                        // [kStages][2 kb][16 KB]
-  const uint32_t sLse = sA + kOffLse;                    // [kLseSlots][128] float (pass 2)
+  const uint32_t sB = smem_u32(smem);                    // [kStages][2 kb][16 KB]
+  const uint32_t sLse = sB + kOffLse;                    // [kLseSlots][128] float (pass 2)
   float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 sub][128]
-  const uint32_t bars = sA + kOffBars;
-  const uint32_t bar_full = bars, bar_empty = bars + 8 * kStages, bar_a = bars + 16 * kStages;
-  const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 32;  // [sub*2+buf]
-  const uint32_t bar_lse = bar_sempty + 32;                           // [kLseSlots]
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 64 + 8 * kLseSlots);
+  const uint32_t bars = sB + kOffBars;
+  const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages, bar_a = bar_empty + 8 * kStages;
+  const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
+  const uint32_t bar_lse = bar_sempty + 8 * kAccBufs;                           // [kLseSlots]
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
-    mbar_init(bar_a, 1);
-    for (int i = 0; i < 4; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
+    mbar_init(bar_a, w.sub_valid[1] ? 16 : 8);  // one arrival per epilogue warp that stages stationary rows
+    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -282,35 +309,37 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
   if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (lane == 0) {
-      const CUtensorMap* mA = kPass == 1 ? &mapQ : (w.a_chunk ? &mapKn : &mapKc);
-      const int nsub = w.sub_valid[1] ? 2 : 1;
-      mbar_expect_tx(bar_a, nsub * kTileBytes);
-      for (int s = 0; s < nsub; ++s)
-        for (int kb = 0; kb < 2; ++kb)
-          tma_load_3d(sA + s * kTileBytes + kb * kKBlockBytes, mA, kb * kKBlock, w.rowA0 + s * kTile, w.lhA, bar_a);
-      for (int j = 0; j < w.ntiles; ++j) {
-        const int stage = j % kStages;
-        mbar_wait(bar_empty + 8 * stage, ((j / kStages) & 1) ^ 1);
+    // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
+    for (int j = 0; j < w.ntiles; ++j) {
+      const int stage = j % kStages;
+      mbar_wait(bar_empty + 8 * stage, ((j / kStages) & 1) ^ 1);
+      const CUtensorMap* mB;
+      int row0, lh;
+      if (kPass == 1) {
+        const bool cache = j < w.n_cache_tiles;
+        mB = cache ? &mapKc : &mapKn;
+        row0 = (cache ? j : j - w.n_cache_tiles) * kTile;
+        lh = w.l * p.Hkv + w.h;
+      } else {
+        mB = &mapQ;
+        row0 = (w.it0[0] + j % w.tiles_per_g) * kTile;
+        lh = w.hq0 + j / w.tiles_per_g;
+      }
+#ifdef OMNIMEM_DBG_NOTMA
+      if (elect_one()) { mbar_arrive(bar_full + 8 * stage); if (kPass == 2) mbar_arrive(bar_lse + 8 * (j % kLseSlots)); }
+      __syncwarp();
+      continue;
+#endif
+      if (elect_one()) {
         mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
-        const CUtensorMap* mB;
-        int row0, lh;
-        if (kPass == 1) {
-          const bool cache = j < w.n_cache_tiles;
-          mB = cache ? &mapKc : &mapKn;
-          row0 = (cache ? j : j - w.n_cache_tiles) * kTile;
-          lh = w.l * p.Hkv + w.h;
-        } else {
-          mB = &mapQ;
-          row0 = (w.it0[0] + j % w.tiles_per_g) * kTile;
-          lh = w.hq0 + j / w.tiles_per_g;
-          // lse2 of these 128 queries: its own ring + barrier; slot j % 16 was last read for tile j - 16; every
-          // epilogue thread finished computing that tile before the MMA of tile j - 4 completed (TMEM buffers are 2 deep,
-          // a sub-tile skips at most every other tile), and this load is issued after that MMA freed the B stage.
+        if (kPass == 2) {
+          // lse2 of these 128 queries: its own ring + barrier.  Slot j % 16 was last read for tile j - 16; this load is
+          // issued only after the MMAs of tile j - kStages completed, which needed the accumulator of a batch at most 3
+          // batches (<= 3 tiles) older to be released, and an epilogue thread releases a batch only after it finished
+          // computing all earlier ones: tile j - 16 is long done.
           const int slot = j % kLseSlots;
           mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
           bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
@@ -318,36 +347,40 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         for (int kb = 0; kb < 2; ++kb)
           tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
       }
+      __syncwarp();
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      mbar_wait(bar_a, 0);
+    mbar_wait(bar_a, 0);  // stationary rows are in TMEM
+    tc_fence_after();
+    int buf = 0, ph = 0;  // accumulator ring position of the next batch
+    for (int j = 0; j < w.ntiles; ++j) {
+      const int stage = j % kStages;
+      mbar_wait(bar_full + 8 * stage, (j / kStages) & 1);
       tc_fence_after();
-      int js[2] = {0, 0};
-      for (int j = 0; j < w.ntiles; ++j) {
-        const int stage = j % kStages;
-        mbar_wait(bar_full + 8 * stage, (j / kStages) & 1);
+      for (int s = 0; s < 2; ++s) {
+        if (!sub_takes_tile<kPass>(w, s, j)) continue;
+        mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
         tc_fence_after();
-        for (int s = 0; s < 2; ++s) {
-          if (!sub_takes_tile<kPass>(w, s, j)) continue;
-          const int buf = js[s] & 1;
-          mbar_wait(bar_sempty + 8 * (s * 2 + buf), ((js[s] >> 1) & 1) ^ 1);
-          tc_fence_after();
-          const uint32_t d_tmem = tmem_base + (uint32_t)((s * 2 + buf) * kTile);
+        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
+        const uint32_t a_tmem = tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2));
+        const uint64_t b_desc = umma_desc_sw128(sB + stage * kTileBytes);
+        if (elect_one()) {
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-            const uint32_t koff = (uint32_t)((kk >> 2) * kKBlockBytes + (kk & 3) * 32);
+            // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
+            const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
 #ifndef OMNIMEM_DBG_NOMMA
-            tc_mma_bf16(d_tmem, umma_desc_sw128(sA + s * kTileBytes + koff), umma_desc_sw128(sB + stage * kTileBytes + koff),
-                        kIdesc, kk > 0 ? 1u : 0u);
+            tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, OMNIMEM_DBG_ACC(kk));
 #endif
           }
-          tc_commit(bar_sfull + 8 * (s * 2 + buf));
-          ++js[s];
+          tc_commit(bar_sfull + 8 * buf);
         }
-        tc_commit(bar_empty + 8 * stage);
+        __syncwarp();
+        if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
       }
+      if (elect_one()) tc_commit(bar_empty + 8 * stage);
+      __syncwarp();
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
@@ -359,14 +392,42 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     const int col0 = half * kHalf;
     const float c2 = p.scale_log2e;
     if (w.sub_valid[s]) {
-      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16) + (uint32_t)col0;
-      int js = 0;
+      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+      {
+        // Stage this thread's share of the stationary operand: row r of the sub-tile, bf16 elements [64 half, 64 half + 64)
+        // = 32 words, straight from global memory into TMEM columns kTmemA + 64 s + 32 half (lane = row, word c = elements
+        // 2c, 2c+1: the A-operand layout of tcgen05.mma).  Rows past the end are zero.
+        const int row = w.rowA0 + s * kTile + r;
+        const __nv_bfloat16* base = kPass == 1 ? a.q : (w.a_chunk ? a.kn : a.kc);
+        const int rows_total = (kPass == 1 || w.a_chunk) ? p.Nn : p.cache_cap;
+        const int rows_valid = (kPass == 1 || w.a_chunk) ? p.Nn : p.n[w.l];
+        uint32_t av[32];
+        if (row < rows_valid) {
+          const uint4* src = reinterpret_cast<const uint4*>(base + ((long long)w.lhA * rows_total + row) * kHeadDim) + half * 8;
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const uint4 t4 = __ldg(src + u);
+            av[4 * u] = t4.x; av[4 * u + 1] = t4.y; av[4 * u + 2] = t4.z; av[4 * u + 3] = t4.w;
+          }
+        } else {
+#pragma unroll
+          for (int u = 0; u < 32; ++u) av[u] = 0u;
+        }
+        tc_st32(t_lane + (uint32_t)(kTmemA + s * (kHeadDim / 2) + half * 32), av);
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_a);
+      }
+      const uint32_t t_col = t_lane + (uint32_t)col0;
+      int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile
       if (kPass == 1) {
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
         const int n = p.n[w.l];
         float m_run = -1e30f, Z = 0.f, W = 0.f;
-        for (int j = 0; j < w.ntiles_sub[s]; ++j, ++js) {
-          const int buf = js & 1;
+        for (int j = 0; j < w.ntiles; ++j) {
+          if (s == 1 && j < w.ntiles_sub[0]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
+          if (j >= w.ntiles_sub[s]) { if (s == 0 && j < w.ntiles_sub[1]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // number of visible key columns of this tile for this row, relative to this thread's first column
           int limit;
           if (j < w.n_cache_tiles) limit = n - j * kTile;
@@ -376,16 +437,18 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             if (p.causal) limit = min(limit, i - t0 + 1);
           }
           limit -= col0;
-          mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
+          mbar_wait(bar_sfull + 8 * buf, ph);
           tc_fence_after();
-          const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
+          const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
           uint32_t v0[32], v1[32];
           tc_ld32(t_addr, v0);
           tc_ld32(t_addr + 32, v1);
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));  // registers hold the tile: free the TMEM buffer
+          if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);  // registers hold the tile: free the TMEM buffer
+          if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+          if (s == 0 && j < w.ntiles_sub[1]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
           float x[kHalf];
           if (limit >= kHalf) {
 #pragma unroll
@@ -453,20 +516,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const uint64_t c2c2 = pack2(c2, c2);
         for (int j = 0; j < w.ntiles; ++j) {
           const int it = w.it0[0] + j % w.tiles_per_g;
-          if (it < w.it0[s]) continue;
-          const int buf = js & 1;
+          const bool other = sub_takes_tile<kPass>(w, s ^ 1, j);
+          if (s == 1 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j comes first
+          if (it < w.it0[s]) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
-          mbar_wait(bar_sfull + 8 * (s * 2 + buf), (js >> 1) & 1);
+          mbar_wait(bar_sfull + 8 * buf, ph);
           tc_fence_after();
-          const uint32_t t_addr = t_lane + (uint32_t)((s * 2 + buf) * kTile);
+          const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
           uint32_t v0[32], v1[32];
           tc_ld32(t_addr, v0);
           tc_ld32(t_addr + 32, v1);
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_sempty + 8 * (s * 2 + buf));
+          if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);
+          if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+          if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
           const int slot = j % kLseSlots;
           mbar_wait(bar_lse + 8 * slot, (j / kLseSlots) & 1);
           const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
@@ -497,7 +563,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
               }
             }
           }
-          ++js;
         }
         float q0, q1, q2, q3;
         unpack2(acc01, q0, q1);
@@ -585,6 +650,9 @@ static TcArgs make_args(const StepParams& p, const StepBuffers& b) {
   a.a_v = b.a_v;
   a.a_a = b.a_a;
   a.n_cache_pairs = (p.cache_cap + 2 * kTile - 1) / (2 * kTile);
+  a.q = (const __nv_bfloat16*)b.Q;
+  a.kc = (const __nv_bfloat16*)b.cacheK;
+  a.kn = (const __nv_bfloat16*)b.chunkK;
   return a;
 }
 
