@@ -32,7 +32,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         s, o = os.path.join(CSRC, src), os.path.join(objdir, src.replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + headers):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
+            extra = os.environ.get("OMNIMEM_NVCC_EXTRA", "").split()      # e.g. -DOMNIMEM_POLY_NUM=4 (kernel tuning sweeps)
+            cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             jobs.append(cmd)
     with ThreadPoolExecutor(max_workers=4) as ex:
         for r in ex.map(lambda c: subprocess.run(c, capture_output=True, text=True), jobs):

@@ -153,30 +153,54 @@ __device__ __forceinline__ float ex2(float x) {
   return y;
 }
 
-// 2^x on the FMA/ALU pipes for x <= 0 (Cody-Waite split + degree-4 minimax polynomial on [-0.5, 0.5], max relative
-// error 2.7e-6; coefficients fitted for this file).  The MUFU ex2 pipe (16/clk/SM) is the
-// limiter of both scoring passes; with kPolyEvery > 0 every kPolyEvery-th exponential of a row is evaluated here.
-__device__ __forceinline__ float ex2_poly(float x) {
-  x = fmaxf(x, -126.f);            // keeps the biased exponent of q * 2^round(x) >= 0
-  const float t = x + 12582912.f;  // 1.5 * 2^23: the low mantissa bits of t now hold round(x)
-  const float f = x - (t - 12582912.f);
-  float q = fmaf(0.009570066817104816f, f, 0.05591786280274391f);
-  q = fmaf(q, f, 0.2402474582195282f);
-  q = fmaf(q, f, 0.6931217908859253f);
-  q = fmaf(q, f, 0.9999992847442627f);
-  return __int_as_float(__float_as_int(q) + (__float_as_int(t) << 23));  // q * 2^round(x)
+// 2^x on the FMA/ALU pipes (Cody-Waite split + degree-4 minimax polynomial on [-0.5, 0.5], max relative error
+// 2.7e-6, mean error 4e-8; coefficients fitted for this file), two lanes per instruction
+// (fp32x2).  The MUFU ex2 pipe (16/clk/SM) is the limiter of both scoring passes (ncu: xu pipe 89 %), so
+// kPolyNum of every kPolyDen exponential PAIRS of a row are evaluated here instead of on the MUFU.
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
 }
-#ifndef OMNIMEM_POLY_EVERY
-#define OMNIMEM_POLY_EVERY 0
+__device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
+  float x0, x1;
+  unpack2(X, x0, x1);
+  X = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));   // keeps the biased exponent of q * 2^round(x) >= 0
+  const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
+  const uint64_t T = add2(X, MG);
+  const uint64_t F = sub2(X, sub2(T, MG));
+  uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
+  Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
+  Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
+  Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
+  float q0, q1, t0, t1;
+  unpack2(Q, q0, q1);
+  unpack2(T, t0, t1);
+  return pack2(__int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23)),   // q * 2^round(x)
+               __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23)));
+}
+#ifndef OMNIMEM_POLY_NUM
+#define OMNIMEM_POLY_NUM 2
 #endif
-constexpr int kPolyEvery = OMNIMEM_POLY_EVERY;
+#ifndef OMNIMEM_POLY_DEN
+#define OMNIMEM_POLY_DEN 8
+#endif
+constexpr int kPolyNum = OMNIMEM_POLY_NUM, kPolyDen = OMNIMEM_POLY_DEN;
 #ifdef OMNIMEM_DBG_NOACC
 #define OMNIMEM_DBG_ACC(kk) 0u
 #else
 #define OMNIMEM_DBG_ACC(kk) ((kk) > 0 ? 1u : 0u)
 #endif
-__device__ __forceinline__ float ex2_sel(float x, int idx) {
-  return (kPolyEvery > 0 && (idx % (kPolyEvery > 0 ? kPolyEvery : 1)) == kPolyEvery - 1) ? ex2_poly(x) : ex2(x);
+// pair `pi` of a row goes to the polynomial iff the Bresenham line of slope kPolyNum / kPolyDen steps there
+__device__ __forceinline__ constexpr bool pair_is_poly(int pi) {
+  return ((pi + 1) * kPolyNum) / kPolyDen > (pi * kPolyNum) / kPolyDen;
+}
+// 2^x of a packed pair: MUFU for both lanes, or the FMA-pipe polynomial
+__device__ __forceinline__ uint64_t ex2_pair(uint64_t X, int pi) {
+  if (pair_is_poly(pi)) return ex2_poly2(X);
+  float x0, x1;
+  unpack2(X, x0, x1);
+  return pack2(ex2(x0), ex2(x1));
 }
 
 // UMMA shared-memory descriptor, K-major, 128-byte swizzle: 8-row groups are 1024 B apart (SBO), LBO unused,
@@ -472,12 +496,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const uint64_t c2c2 = pack2(c2, c2), nm = pack2(-m_new, -m_new);
 #pragma unroll
           for (int e = 0; e < kHalf; e += 4) {
-            float a0, a1, a2, a3;
-            unpack2(fma2(pack2(x[e], x[e + 1]), c2c2, nm), a0, a1);
-            unpack2(fma2(pack2(x[e + 2], x[e + 3]), c2c2, nm), a2, a3);
-            const float p0 = ex2_sel(a0, e), p1 = ex2_sel(a1, e + 1), p2 = ex2_sel(a2, e + 2), p3 = ex2_sel(a3, e + 3);
-            z01 = add2(z01, pack2(p0, p1));
-            z23 = add2(z23, pack2(p2, p3));
+            const uint64_t A01 = fma2(pack2(x[e], x[e + 1]), c2c2, nm), A23 = fma2(pack2(x[e + 2], x[e + 3]), c2c2, nm);
+            const uint64_t P01 = ex2_pair(A01, e / 2), P23 = ex2_pair(A23, e / 2 + 1);
+            z01 = add2(z01, P01);
+            z23 = add2(z23, P23);
+            float a0, a1, a2, a3, p0, p1, p2, p3;
+            unpack2(A01, a0, a1);
+            unpack2(A23, a2, a3);
+            unpack2(P01, p0, p1);
+            unpack2(P23, p2, p3);
             if (kEntropy) {  // sum p z2 over visible columns (masked ones have p = 0 but z2 = -inf)
               wz[0] = fmaf(p0, limit > e ? a0 + m_new : 0.f, wz[0]);
               wz[1] = fmaf(p1, limit > e + 1 ? a1 + m_new : 0.f, wz[1]);
@@ -540,15 +567,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 #pragma unroll
             for (int e4 = 0; e4 < 8; ++e4) {
               const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
-              float p0, p1, p2, p3, p4, p5, p6, p7;
-              unpack2(fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y)), p0, p1);
-              unpack2(fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w)), p2, p3);
-              unpack2(fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y)), p4, p5);
-              unpack2(fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w)), p6, p7);
-              acc01 = add2(acc01, pack2(ex2_sel(p0, 4 * e4), ex2_sel(p1, 4 * e4 + 1)));
-              acc23 = add2(acc23, pack2(ex2_sel(p2, 4 * e4 + 2), ex2_sel(p3, 4 * e4 + 3)));
-              acc01 = add2(acc01, pack2(ex2_sel(p4, 4 * e4), ex2_sel(p5, 4 * e4 + 1)));
-              acc23 = add2(acc23, pack2(ex2_sel(p6, 4 * e4 + 2), ex2_sel(p7, 4 * e4 + 3)));
+              const uint64_t x0 = fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y));
+              const uint64_t x1 = fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w));
+              const uint64_t x2 = fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y));
+              const uint64_t x3 = fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w));
+              acc01 = add2(acc01, ex2_pair(x0, 4 * e4));
+              acc23 = add2(acc23, ex2_pair(x1, 4 * e4 + 1));
+              acc01 = add2(acc01, ex2_pair(x2, 4 * e4 + 2));
+              acc23 = add2(acc23, ex2_pair(x3, 4 * e4 + 3));
             }
           } else {
 #pragma unroll

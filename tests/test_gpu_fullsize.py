@@ -1,0 +1,182 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one fused
+`omnimem_compress_chunk` over all layers).
+
+The oracle cannot redo a whole step (CFG2: 21.5 fp64 TFLOP), so each test checks
+  * properties that hold at any size, on EVERY layer: softmax rows sum to one (sum_k a = G Nq per KV head, Eq.6),
+    budgets sum to B, indices ascending / in range / M of them, dst rows byte-identical to the rows the kept
+    indices name, counts published; and
+  * SAMPLED layers in full against the oracle (one layer is an independent unit: all heads are needed by the AVBA
+    statistics of Eq.9-10): rule (a) on a, s, psi, lse, statistics; budgets equal; rule (b) select + compact bit-exact
+    when fed the oracle's psi; rule (c) on the fused step's kept sets.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ref
+from paper_2606_07577_b200 import inputs as I
+from tests.util import TOL, compare_scores, kept_sets_rule_c, ref_params, seg_lens
+
+pytestmark = pytest.mark.gpu
+
+
+def oracle_layer(wl, x, i, n_v, n, cacheK=None, cacheV=None):
+    """The oracle on layer slot `i` of the stacked inputs (L = 1).  cacheK / cacheV override x's cache (teacher forcing)."""
+    p = ref_params(wl, 1)
+    cK = x["cacheK"][i:i + 1] if cacheK is None else cacheK
+    cV = x["cacheV"][i:i + 1] if cacheV is None else cacheV
+    return ref.compress_chunk(p, cK, cV, np.array([n_v], np.int32), np.array([n], np.int32), x["chunkK"][i:i + 1],
+                              x["chunkV"][i:i + 1], x["Q"][i:i + 1], np.array([wl.budget], np.int32))
+
+
+def gpu_layer_scores(sc, l):
+    f = lambda t: t[l:l + 1].detach().cpu().numpy()
+    return dict(a_v=f(sc.a_v), a_a=f(sc.a_a), s_v=f(sc.s_v), s_a=f(sc.s_a), psi_v=f(sc.psi_v), psi_a=f(sc.psi_a),
+                stats=f(sc.stats), lse=f(sc.lse))
+
+
+def check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n):
+    """Properties of the fused step's outputs that need no oracle; every layer, every head; computed with torch ops on
+    the device (an independent gather, not the library's)."""
+    L, tol = wl.L, TOL[wl.dtype]
+    Kv, Ka = seg_lens(wl, n_v, n)
+    mv, ma = M_v.cpu().numpy(), M_a.cpu().numpy()
+    assert np.array_equal(mv + ma, np.minimum(wl.budget, Kv + Ka)), "budgets do not sum to B"
+    assert np.all(mv <= Kv) and np.all(ma <= Ka) and np.all(mv >= 0) and np.all(ma >= 0)
+    assert np.array_equal(dst.n_v.cpu().numpy(), mv) and np.array_equal(dst.n.cpu().numpy(), mv + ma)
+    for l in range(L):
+        tot = sc.a_v[l, :, :Kv[l]].double().sum(-1) + sc.a_a[l, :, :Ka[l]].double().sum(-1)
+        np.testing.assert_allclose(tot.cpu().numpy(), wl.G * wl.Nn, rtol=10 * tol)
+        assert bool((sc.a_v[l, :, :Kv[l]] >= 0).all()) and bool((sc.psi_v[l, :, :Kv[l]] >= 0).all())
+        for idx, M, K, off_c, cnt_c, off_n in ((idx_v, mv[l], Kv[l], 0, n_v[l], 0),
+                                               (idx_a, ma[l], Ka[l], n_v[l], n[l] - n_v[l], wl.Nn_v)):
+            if M == 0:
+                continue
+            ii = idx[l, :, :M].long()
+            assert int(ii.min()) >= 0 and int(ii.max()) < K
+            assert bool((ii[:, 1:] > ii[:, :-1]).all()), f"layer {l}: indices not strictly ascending"
+            base = 0 if idx is idx_v else mv[l]
+            for name, c_src, c_new, c_dst in (("K", src.k, chunk.k, dst.k), ("V", src.v, chunk.v, dst.v)):
+                seg = torch.cat([c_src[l, :, off_c:off_c + cnt_c], c_new[l, :, off_n:off_n + (K - cnt_c)]], 1)
+                want = torch.gather(seg, 1, ii.unsqueeze(-1).expand(-1, -1, wl.D))
+                assert torch.equal(c_dst[l, :, base:base + M].view(torch.int16), want.view(torch.int16)), \
+                    f"layer {l} {name}: compacted rows differ from the gathered rows"
+
+
+def check_sampled_layer(wl, eng, x, i, l, src, chunk, sc, idx_v, idx_a, M_v, M_a, n_v_l, n_l, orc=None):
+    """Layer `l` of the device state (slot `i` of the host inputs x) in full against the oracle."""
+    tol = TOL[wl.dtype]
+    orc = orc if orc is not None else oracle_layer(wl, x, i, n_v_l, n_l)
+    nv1, n1 = np.array([n_v_l], np.int32), np.array([n_l], np.int32)
+    compare_scores(wl, nv1, n1, gpu_layer_scores(sc, l), orc, tol)                       # rule (a)
+    Kv, Ka = n_v_l + wl.Nn_v, (n_l - n_v_l) + wl.Nn_a
+    mv, ma = int(M_v[l]), int(M_a[l])
+    assert mv == orc["M_v"][0] and ma == orc["M_a"][0], f"layer {l}: budgets {mv},{ma} vs {orc['M_v'][0]},{orc['M_a'][0]}"
+    n_diff = 0
+    iv, ia = idx_v[l].cpu().numpy(), idx_a[l].cpu().numpy()
+    for h in range(wl.Hkv):                                                               # rule (c)
+        n_diff += kept_sets_rule_c(f"v[{l},{h}]", iv[h], orc["idx_v"][0, h], mv, orc["psi_v"][0, h, :Kv], tol)
+        n_diff += kept_sets_rule_c(f"a[{l},{h}]", ia[h], orc["idx_a"][0, h], ma, orc["psi_a"][0, h, :Ka], tol)
+    # rule (b): the library's select + compact over ALL layers, this layer fed the oracle's psi: bit-exact there
+    psi_v, psi_a = sc.psi_v.clone(), sc.psi_a.clone()
+    psi_v[l] = torch.from_numpy(orc["psi_v"][0]).to(psi_v.device)
+    psi_a[l] = torch.from_numpy(orc["psi_a"][0]).to(psi_a.device)
+    jv, ja = eng.select(psi_v, psi_a, src.n_v, src.n, wl.Nn_v, wl.Nn_a, M_v, M_a)
+    assert np.array_equal(jv[l, :, :mv].cpu().numpy(), orc["idx_v"][0, :, :mv]), f"layer {l}: select(oracle psi) differs"
+    assert np.array_equal(ja[l, :, :ma].cpu().numpy(), orc["idx_a"][0, :, :ma])
+    dst = eng.new_cache()
+    eng.compact(src, chunk, jv, ja, M_v, M_a, dst)
+    torch.cuda.synchronize()
+    nl = mv + ma
+    assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][0, :, :nl])
+    assert np.array_equal(dst.v[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstV"][0, :, :nl])
+    del dst, psi_v, psi_a
+    return n_diff
+
+
+def run_full_step(wl, sample_layers):
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
+    x = I.full_inputs(wl)
+    eng = OmniMem.for_workload(wl)
+    dev = eng.device
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+    dst = eng.new_cache()
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
+    sc = eng.new_scores(wl.Nn, want_lse=True)
+    M_v = torch.zeros(wl.L, dtype=torch.int32, device=dev)
+    M_a = torch.zeros_like(M_v)
+    idx_v, idx_a = eng.new_indices()
+    eng.compress_chunk(src, chunk, B, dst, out=sc, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)   # what bench.py times
+    torch.cuda.synchronize()
+    n_v, n = x["n_v"].numpy(), x["n"].numpy()
+    check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n)
+    n_diff = 0
+    for l in sample_layers:
+        n_diff += check_sampled_layer(wl, eng, x, l, l, src, chunk, sc, idx_v, idx_a, M_v, M_a, int(n_v[l]), int(n[l]))
+    eng.close()
+    return n_diff
+
+
+def test_cfg2_full_size():
+    n_diff = run_full_step(I.CFG2, sample_layers=(0, 27))
+    assert n_diff <= 8, f"{n_diff} kept indices differ (all inside rule (c)'s tolerance band, but fp32-level agreement is the target)"
+
+
+def test_cfg4_full_size():
+    n_diff = run_full_step(I.CFG4, sample_layers=(0, 18, 35))
+    assert n_diff <= 8
+
+
+def test_cfg3_full_size():
+    n_diff = run_full_step(I.CFG3, sample_layers=(35,))
+    assert n_diff <= 8
+
+
+def test_cfg5_streaming_teacher_forced():
+    """CFG5 (hour-long stream, Qwen2.5-Omni-7B shape, B = 32768): the GPU runs free from an empty cache through the
+    append-only steps, the first eviction (step index 5) and into the steady state; at sampled (step, layer) pairs the
+    oracle starts from the GPU's own pre-step cache state of that layer, so each sampled step is checked on its own."""
+    from paper_2606_07577_b200.omnimem import Chunk, OmniMem
+    wl = I.CFG5
+    n_steps, samples = 8, {4: 9, 5: 3, 7: 20}                # step index -> layer checked in full
+    eng = OmniMem.for_workload(wl)
+    dev = eng.device
+    src, dst = eng.new_cache(), eng.new_cache()
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
+    sc = eng.new_scores(wl.Nn, want_lse=True)
+    M_v = torch.zeros(wl.L, dtype=torch.int32, device=dev)
+    M_a = torch.zeros_like(M_v)
+    idx_v, idx_a = eng.new_indices()
+    n_diff = 0
+    for step in range(n_steps):
+        x = I.full_inputs(wl, step=step, with_cache=False)
+        chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+        n_v, n = src.n_v.cpu().numpy(), src.n.cpu().numpy()
+        assert np.all(n == min(step * wl.Nn, wl.budget)), f"step {step}: cache rows {n}"
+        eng.compress_chunk(src, chunk, B, dst, out=sc, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+        torch.cuda.synchronize()
+        check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n)
+        if n[0] + wl.Nn <= wl.budget:                        # append-only: everything kept, in order
+            assert np.array_equal(dst.n.cpu().numpy(), n + wl.Nn) and np.array_equal(dst.n_v.cpu().numpy(), n_v + wl.Nn_v)
+            for l in (0, wl.L - 1):
+                assert torch.equal(dst.k[l, :, :n_v[l]], src.k[l, :, :n_v[l]])
+                assert torch.equal(dst.k[l, :, n_v[l]:n_v[l] + wl.Nn_v], chunk.k[l, :, :wl.Nn_v])
+                assert torch.equal(dst.v[l, :, n_v[l] + wl.Nn_v:n[l] + wl.Nn_v], src.v[l, :, n_v[l]:n[l]])
+                assert torch.equal(dst.v[l, :, n[l] + wl.Nn_v:n[l] + wl.Nn], chunk.v[l, :, wl.Nn_v:])
+        if step in samples:
+            l = samples[step]
+            cK, cV = src.k[l:l + 1].cpu(), src.v[l:l + 1].cpu()
+            orc = oracle_layer(wl, x, l, int(n_v[l]), int(n[l]), cacheK=cK, cacheV=cV)
+            nl = int(orc["n_out"][0])
+            if n[l] + wl.Nn > wl.budget:
+                n_diff += check_sampled_layer(wl, eng, x, l, l, src, chunk, sc, idx_v, idx_a, M_v, M_a, int(n_v[l]), int(n[l]),
+                                              orc=orc)
+            else:
+                assert nl == n[l] + wl.Nn
+                assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][0, :, :nl])
+                assert np.array_equal(dst.v[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstV"][0, :, :nl])
+        src, dst = dst, src
+    assert int(src.n.min()) == wl.budget
+    assert n_diff <= 8
+    eng.close()
