@@ -291,14 +291,6 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
   }
 }
 
-template <int kPass>
-__device__ __forceinline__ bool sub_takes_tile(const Work& w, int s, int j) {
-  if (kPass == 1) return j < w.ntiles_sub[s];
-  if (!w.sub_valid[s]) return false;
-  const int it = w.it0[0] + j % w.tiles_per_g;
-  return it >= w.it0[s];
-}
-
 template <int kPass, bool kEntropy>
 __global__ void __launch_bounds__(kThreads, 1)
 score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapKc,
@@ -337,9 +329,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 
   if (warp == 0) {
     // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
+    int it = kPass == 2 ? w.it0[0] : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
     for (int j = 0; j < w.ntiles; ++j) {
-      const int stage = j % kStages;
-      mbar_wait(bar_empty + 8 * stage, ((j / kStages) & 1) ^ 1);
+      mbar_wait(bar_empty + 8 * stage, sph);
       const CUtensorMap* mB;
       int row0, lh;
       if (kPass == 1) {
@@ -349,12 +341,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         lh = w.l * p.Hkv + w.h;
       } else {
         mB = &mapQ;
-        row0 = (w.it0[0] + j % w.tiles_per_g) * kTile;
-        lh = w.hq0 + j / w.tiles_per_g;
+        row0 = it * kTile;
+        lh = w.hq0 + g;
+        if (++it == w.it0[0] + w.tiles_per_g) { it = w.it0[0]; ++g; }
       }
 #ifdef OMNIMEM_DBG_NOTMA
-      if (elect_one()) { mbar_arrive(bar_full + 8 * stage); if (kPass == 2) mbar_arrive(bar_lse + 8 * (j % kLseSlots)); }
+      if (elect_one()) { mbar_arrive(bar_full + 8 * stage); if (kPass == 2) mbar_arrive(bar_lse + 8 * slot); }
       __syncwarp();
+      if (++stage == kStages) { stage = 0; sph ^= 1; }
+      if (++slot == kLseSlots) slot = 0;
       continue;
 #endif
       if (elect_one()) {
@@ -364,7 +359,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           // issued only after the MMAs of tile j - kStages completed, which needed the accumulator of a batch at most 3
           // batches (<= 3 tiles) older to be released, and an epilogue thread releases a batch only after it finished
           // computing all earlier ones: tile j - 16 is long done.
-          const int slot = j % kLseSlots;
           mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
           bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
         }
@@ -372,18 +366,20 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
       }
       __syncwarp();
+      if (++stage == kStages) { stage = 0; sph ^= 1; }
+      if (++slot == kLseSlots) slot = 0;
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     mbar_wait(bar_a, 0);  // stationary rows are in TMEM
     tc_fence_after();
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
+    int it = kPass == 2 ? w.it0[0] : 0, stage = 0, sph = 0;
     for (int j = 0; j < w.ntiles; ++j) {
-      const int stage = j % kStages;
-      mbar_wait(bar_full + 8 * stage, (j / kStages) & 1);
+      mbar_wait(bar_full + 8 * stage, sph);
       tc_fence_after();
       for (int s = 0; s < 2; ++s) {
-        if (!sub_takes_tile<kPass>(w, s, j)) continue;
+        if (!(kPass == 1 ? j < w.ntiles_sub[s] : (w.sub_valid[s] && it >= w.it0[s]))) continue;
         mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
@@ -405,6 +401,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       }
       if (elect_one()) tc_commit(bar_empty + 8 * stage);
       __syncwarp();
+      if (++stage == kStages) { stage = 0; sph ^= 1; }
+      if (kPass == 2 && ++it == w.it0[0] + w.tiles_per_g) it = w.it0[0];
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
@@ -449,9 +447,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
         const int n = p.n[w.l];
         float m_run = -1e30f, Z = 0.f, W = 0.f;
+        const int nt0 = w.ntiles_sub[0], nt1 = w.ntiles_sub[1], nt_mine = s == 0 ? nt0 : nt1;
         for (int j = 0; j < w.ntiles; ++j) {
-          if (s == 1 && j < w.ntiles_sub[0]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
-          if (j >= w.ntiles_sub[s]) { if (s == 0 && j < w.ntiles_sub[1]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          if (s == 1 && j < nt0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
+          if (j >= nt_mine) { if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // number of visible key columns of this tile for this row, relative to this thread's first column
           int limit;
           if (j < w.n_cache_tiles) limit = n - j * kTile;
@@ -472,7 +471,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);  // registers hold the tile: free the TMEM buffer
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-          if (s == 0 && j < w.ntiles_sub[1]) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
+          if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
           float x[kHalf];
           if (limit >= kHalf) {
 #pragma unroll
@@ -541,11 +540,15 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         uint64_t acc01 = 0ull, acc23 = 0ull;   // packed fp32x2 partial sums of the unmasked tiles
         const uint64_t c2c2 = pack2(c2, c2);
+        const int it_first = w.it0[0], it_end = w.it0[0] + w.tiles_per_g, it_mine = w.it0[s], it_other = w.it0[s ^ 1];
+        const bool other_valid = w.sub_valid[s ^ 1];
+        int it_next = it_first;
         for (int j = 0; j < w.ntiles; ++j) {
-          const int it = w.it0[0] + j % w.tiles_per_g;
-          const bool other = sub_takes_tile<kPass>(w, s ^ 1, j);
+          const int it = it_next, slot = j % kLseSlots, lse_parity = (j / kLseSlots) & 1;   // kLseSlots is a power of two
+          if (++it_next == it_end) it_next = it_first;                                       // no division in the tile loop
+          const bool other = other_valid && it >= it_other;
           if (s == 1 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j comes first
-          if (it < w.it0[s]) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          if (it < it_mine) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
           mbar_wait(bar_sfull + 8 * buf, ph);
@@ -560,8 +563,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
-          const int slot = j % kLseSlots;
-          mbar_wait(bar_lse + 8 * slot, (j / kLseSlots) & 1);
+          mbar_wait(bar_lse + 8 * slot, lse_parity);
           const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
           if (first <= 0) {
 #pragma unroll
