@@ -61,7 +61,7 @@ class ClockSampler:
     """Samples SM clock and throttle reasons with NVML during the timed region."""
 
     def __init__(self, index: int, period: float = 0.05):
-        self.index, self.period, self.samples, self.reasons = index, period, [], set()
+        self.index, self.period, self.samples, self.reasons, self.power = index, period, [], set(), []
         self.max_mhz, self._stop, self._thr, self.ok = None, threading.Event(), None, False
         try:
             import pynvml
@@ -80,6 +80,10 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+                except Exception:
+                    pass
                 try:
                     r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 except Exception:
@@ -106,7 +110,7 @@ class ClockSampler:
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(self.samples)}
+                "samples": len(self.samples), "power_w": float(np.median(self.power)) if self.power else None}
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm

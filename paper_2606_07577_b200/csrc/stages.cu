@@ -10,89 +10,108 @@ namespace omnimem {
 // Eq.7 (value rows per P:103, R8): cosn[t] = cos(x_t, x_{t+sigma}) inside the modality's appended sequence.
 // s_t is assembled from cosn[t] and cosn[t-sigma] in finalize.  kTPR threads (16 B each) cover one row.
 // ------------------------------------------------------------------------------------------------------------
-template <typename T> struct Row16;
-template <> struct Row16<float> {
-  static constexpr int N = 4;
-  __device__ static __forceinline__ void load(const float* p, float* o) {
-    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
-    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+// 16 bytes of a row and of its partner: dot += <x, y>, nx += <x, x>, ny += <y, y> in fp32.
+template <typename T> struct Vec16;
+template <> struct Vec16<float> {
+  __device__ static __forceinline__ void acc(const uint4& x, const uint4& y, float& dot, float& nx, float& ny) {
+    const float xs[4] = {__uint_as_float(x.x), __uint_as_float(x.y), __uint_as_float(x.z), __uint_as_float(x.w)};
+    const float ys[4] = {__uint_as_float(y.x), __uint_as_float(y.y), __uint_as_float(y.z), __uint_as_float(y.w)};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      dot = fmaf(xs[e], ys[e], dot);
+      nx = fmaf(xs[e], xs[e], nx);
+      ny = fmaf(ys[e], ys[e], ny);
+    }
   }
 };
-template <> struct Row16<__nv_bfloat16> {
-  static constexpr int N = 8;
-  __device__ static __forceinline__ void load(const __nv_bfloat16* p, float* o) {
-    const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
-    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+template <> struct Vec16<__nv_bfloat16> {
+  // mixed-precision FMA (bf16 x bf16 + fp32, exact products): no unpacking of the bf16 pairs
+  __device__ static __forceinline__ void fma_pair(float& d0, float& d1, uint32_t a, uint32_t b) {
+    asm("{\n\t.reg .b16 al, ah, bl, bh;\n\tmov.b32 {al, ah}, %2;\n\tmov.b32 {bl, bh}, %3;\n\t"
+        "fma.rn.f32.bf16 %0, al, bl, %0;\n\tfma.rn.f32.bf16 %1, ah, bh, %1;\n\t}" : "+f"(d0), "+f"(d1) : "r"(a), "r"(b));
+  }
+  __device__ static __forceinline__ void acc(const uint4& x, const uint4& y, float& dot, float& nx, float& ny) {
+    const uint32_t xs[4] = {x.x, x.y, x.z, x.w}, ys[4] = {y.x, y.y, y.z, y.w};
+    float d1 = 0.f, nx1 = 0.f, ny1 = 0.f;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      o[2 * i] = __uint_as_float(w[i] << 16);
-      o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    for (int e = 0; e < 4; ++e) {
+      fma_pair(dot, d1, xs[e], ys[e]);
+      fma_pair(nx, nx1, xs[e], xs[e]);
+      fma_pair(ny, ny1, ys[e], ys[e]);
     }
+    dot += d1; nx += nx1; ny += ny1;
   }
 };
 
-template <typename T, int kTPR>
+// kTPR = 4 threads cover one row, kVec 16-byte vectors each (vector j of the row goes to thread j % 4, so a warp's load
+// instruction touches 8 rows x 64 contiguous bytes).  One block = kUnroll * 64 consecutive items of one (layer, KV
+// head); every thread first issues all of its 2 * kUnroll * kVec loads (row t and its partner t + sigma, which a
+// neighbouring block reads again out of L2), then reduces: enough bytes in flight per SM to run at HBM speed, and
+// ~25 instructions per 16 bytes instead of ~115 (the first version was instruction-bound: ncu, profiles/).
+template <typename T, int kVec, int kUnroll>
 __global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __restrict__ cacheX,
                                                      const T* __restrict__ chunkX, float* __restrict__ cosn) {
-  constexpr int kRows = 256 / kTPR;
+  constexpr int kTPR = 4, kRows = 256 / kTPR;
   const int items = p.seg_cap_v + p.seg_cap_a;
-  const long long item = (long long)blockIdx.x * kRows + threadIdx.x / kTPR;
+  const int lh = blockIdx.y, l = lh / p.Hkv;
+  if (layer_skips_scoring(p, l)) return;
   const int sub = threadIdx.x % kTPR;
-  const long long total = (long long)p.L * p.Hkv * items;
-  bool active = item < total;
-  int l = 0, h = 0, m = 0, t = 0;
-  if (active) {
-    const int it = (int)(item % items);
-    h = (int)((item / items) % p.Hkv);
-    l = (int)(item / ((long long)items * p.Hkv));
-    m = it < p.seg_cap_v ? 0 : 1;
-    t = m == 0 ? it : it - p.seg_cap_v;
-  }
-  float dot = 0.f, nx = 0.f, ny = 0.f;
-  if (active) {
-    const int n_v = p.n_v[l], n = p.n[l];
+  const int n_v = p.n_v[l], n = p.n[l];
+  const uint4* cbase = reinterpret_cast<const uint4*>(cacheX + (long long)lh * p.cache_cap * p.D) + sub;
+  const uint4* kbase = reinterpret_cast<const uint4*>(chunkX + (long long)lh * p.Nn * p.D) + sub;
+  const int row_vecs = kVec * kTPR;
+  uint4 xv[kUnroll][kVec], yv[kUnroll][kVec];
+  bool active[kUnroll];
+  int it[kUnroll];
+#pragma unroll
+  for (int u = 0; u < kUnroll; ++u) {
+    it[u] = (blockIdx.x * kUnroll + u) * kRows + threadIdx.x / kTPR;
+    const int m = it[u] < p.seg_cap_v ? 0 : 1;
+    const int t = m == 0 ? it[u] : it[u] - p.seg_cap_v;
     const int sg = m == 0 ? p.stride_v : p.stride_a;
-    active = t + sg < seg_len(p, n_v, n, m);
-    if (active) {
+    active[u] = it[u] < items && t + sg < seg_len(p, n_v, n, m);
+    if (active[u]) {
       bool cx, cy;
       const int rx = seg_row(p, n_v, n, m, t, cx), ry = seg_row(p, n_v, n, m, t + sg, cy);
-      const long long lh = (long long)l * p.Hkv + h;
-      const T* x = (cx ? chunkX + (lh * p.Nn + rx) * p.D : cacheX + (lh * p.cache_cap + rx) * p.D) + sub * Row16<T>::N;
-      const T* y = (cy ? chunkX + (lh * p.Nn + ry) * p.D : cacheX + (lh * p.cache_cap + ry) * p.D) + sub * Row16<T>::N;
-      float xv[Row16<T>::N], yv[Row16<T>::N];
-      Row16<T>::load(x, xv);
-      Row16<T>::load(y, yv);
+      const uint4* x = (cx ? kbase : cbase) + (long long)rx * row_vecs;
+      const uint4* y = (cy ? kbase : cbase) + (long long)ry * row_vecs;
 #pragma unroll
-      for (int e = 0; e < Row16<T>::N; ++e) {
-        dot = fmaf(xv[e], yv[e], dot);
-        nx = fmaf(xv[e], xv[e], nx);
-        ny = fmaf(yv[e], yv[e], ny);
-      }
+      for (int i = 0; i < kVec; ++i) { xv[u][i] = __ldg(x + i * kTPR); yv[u][i] = __ldg(y + i * kTPR); }
     }
   }
 #pragma unroll
-  for (int o = kTPR / 2; o; o >>= 1) {
-    dot += __shfl_xor_sync(0xffffffffu, dot, o);
-    nx += __shfl_xor_sync(0xffffffffu, nx, o);
-    ny += __shfl_xor_sync(0xffffffffu, ny, o);
+  for (int u = 0; u < kUnroll; ++u) {
+    float dot = 0.f, nx = 0.f, ny = 0.f;
+    if (active[u]) {
+#pragma unroll
+      for (int i = 0; i < kVec; ++i) Vec16<T>::acc(xv[u][i], yv[u][i], dot, nx, ny);
+    }
+#pragma unroll
+    for (int o = kTPR / 2; o; o >>= 1) {
+      dot += __shfl_xor_sync(0xffffffffu, dot, o);
+      nx += __shfl_xor_sync(0xffffffffu, nx, o);
+      ny += __shfl_xor_sync(0xffffffffu, ny, o);
+    }
+    if (active[u] && sub == 0) cosn[(long long)lh * items + it[u]] = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
   }
-  if (active && sub == 0) cosn[item] = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
 }
 
 cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
                           int* launches) {
   const void* cx = ctx->cfg.sim_source == 0 ? b.cacheV : b.cacheK;
   const void* kx = ctx->cfg.sim_source == 0 ? b.chunkV : b.chunkK;
-  const long long total = (long long)p.L * p.Hkv * (p.seg_cap_v + p.seg_cap_a);
+  const int items = p.seg_cap_v + p.seg_cap_a;
   const int row_bytes = p.D * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2);
-  const int tpr = row_bytes / 16;
-  const unsigned grid = (unsigned)((total + 256 / tpr - 1) / (256 / tpr));
+  const int vec = row_bytes / 64;                      // 16-byte vectors per thread (4 threads per row): 2, 4 or 8
+  const int unroll = vec == 8 ? 1 : 2;
+  const int rows_per_block = unroll * 64;
+  const dim3 grid((unsigned)((items + rows_per_block - 1) / rows_per_block), (unsigned)(p.L * p.Hkv));
   ++*launches;
-#define OMNIMEM_COS(T, TPR) cosine_kernel<T, TPR><<<grid, 256, 0, st>>>(p, (const T*)cx, (const T*)kx, b.cosn)
+#define OMNIMEM_COS(T, V, U) cosine_kernel<T, V, U><<<grid, 256, 0, st>>>(p, (const T*)cx, (const T*)kx, b.cosn)
   if (ctx->cfg.dtype == OMNIMEM_FP32) {
-    if (tpr == 16) OMNIMEM_COS(float, 16); else OMNIMEM_COS(float, 32);
+    if (vec == 4) OMNIMEM_COS(float, 4, 2); else OMNIMEM_COS(float, 8, 1);
   } else {
-    if (tpr == 8) OMNIMEM_COS(__nv_bfloat16, 8); else OMNIMEM_COS(__nv_bfloat16, 16);
+    if (vec == 2) OMNIMEM_COS(__nv_bfloat16, 2, 2); else OMNIMEM_COS(__nv_bfloat16, 4, 2);
   }
 #undef OMNIMEM_COS
   return cudaGetLastError();
