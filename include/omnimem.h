@@ -160,9 +160,12 @@ OMNIMEM_API int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* sr
 /* ---- the fused step fed from HOST memory (end-to-end entry) --------------------------------------------------- */
 /* host_chunk->k/v/q (and ->lse if non-NULL) are HOST pointers (pinned memory for full copy speed) with the chunk
  * layout above; dev_chunk holds DEVICE staging buffers of the same shapes (caller-owned).  Copies the chunk to the
- * device, runs omnimem_compress_chunk, copies M_v, M_a (and dst n_v, n) back to the HOST arrays host_M_v, host_M_a
- * [L] (pinned) and synchronises `stream` before returning.  Returns the byte counts moved through
- * h2d_bytes / d2h_bytes (HOST, may be NULL). */
+ * device, runs the fused step, copies M_v, M_a back to the HOST arrays host_M_v, host_M_a [L] (pinned) and
+ * synchronises `stream` before returning.  Layers are independent through the whole step (the per-layer
+ * totals are an input, R21), so the chunk is copied and compressed in up to 8 groups of consecutive layers: the
+ * copies run on a stream owned by the context (ordered after everything already enqueued on `stream`) and the
+ * kernels of group g on `stream` overlap the copy of group g + 1.  Results are identical to omnimem_compress_chunk
+ * on the same inputs.  Returns the byte counts moved through h2d_bytes / d2h_bytes (HOST, may be NULL). */
 OMNIMEM_API int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
                                 const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,
                                 int32_t* host_M_v, int32_t* host_M_a, int64_t* h2d_bytes, int64_t* d2h_bytes,

@@ -48,10 +48,11 @@ int fail_cuda(omnimem_ctx* c, cudaError_t e) {
 }
 
 StepParams make_params(const omnimem_ctx* c, int Nn_v, int Nn_a, const int32_t* n_v, const int32_t* n,
-                       const int32_t* skip_budget) {
+                       const int32_t* skip_budget, int n_layers = -1) {
   const omnimem_config& g = c->cfg;
   StepParams p{};
-  p.L = g.n_layers; p.Hq = g.n_q_heads; p.Hkv = g.n_kv_heads; p.G = g.n_q_heads / g.n_kv_heads; p.D = g.head_dim;
+  // a layer range [l0, l0 + L): every per-layer pointer is offset by the caller
+  p.L = n_layers < 0 ? g.n_layers : n_layers; p.Hq = g.n_q_heads; p.Hkv = g.n_kv_heads; p.G = g.n_q_heads / g.n_kv_heads; p.D = g.head_dim;
   p.cache_cap = g.cache_cap;
   p.Nn_v = Nn_v; p.Nn_a = Nn_a; p.Nn = Nn_v + Nn_a;
   p.seg_cap_v = c->seg_cap_v; p.seg_cap_a = c->seg_cap_a;
@@ -139,6 +140,91 @@ int check_scores(const omnimem_scores* o) {
   return (o->a_v && o->a_a && o->s_v && o->s_a && o->psi_v && o->psi_a && o->stats) ? OMNIMEM_OK : OMNIMEM_INVALID_ARG;
 }
 
+int check_fused_args(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* layer_budget,
+                     omnimem_cache* dst, omnimem_scores* opt_out, void* ws, size_t ws_bytes) {
+  if (!ctx || !layer_budget || !ws) return OMNIMEM_INVALID_ARG;
+  int rc = check_cache(src);
+  if (rc) return rc;
+  rc = check_cache(dst);
+  if (rc) return rc;
+  rc = check_chunk(ctx, chunk, true);
+  if (rc) return rc;
+  if (opt_out && (rc = check_scores(opt_out))) return rc;
+  if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
+  if (ws_bytes < ws_layout(ctx).total) return OMNIMEM_WORKSPACE_TOO_SMALL;
+  return OMNIMEM_OK;
+}
+
+// The fused step on layers [l0, l0 + Lg).  Every buffer of the step is laid out [L, ...] with the layer outermost and
+// no stage looks across layers (the per-layer totals of Eq.14 are an input here, R21), so a layer range is the same
+// problem with every per-layer pointer advanced by l0 and L = Lg.  Arguments are already validated.
+int compress_layers(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* layer_budget,
+                    omnimem_cache* dst, omnimem_scores* opt_out, int32_t* opt_idx_v, int32_t* opt_idx_a,
+                    int32_t* opt_M_v, int32_t* opt_M_a, uint8_t* wsb, int l0, int Lg, cudaStream_t st) {
+  const omnimem_config& g = ctx->cfg;
+  const WsLayout w = ws_layout(ctx);
+  const size_t es = g.dtype == OMNIMEM_FP32 ? 4 : 2;
+  const size_t Nn = (size_t)chunk->Nn_v + chunk->Nn_a, Hq = g.n_q_heads, Hkv = g.n_kv_heads, D = g.head_dim;
+  const size_t lz = (size_t)l0;
+  auto adv = [](const void* p, size_t bytes) { return p ? (void*)((uint8_t*)const_cast<void*>(p) + bytes) : nullptr; };
+  const size_t cache_b = lz * Hkv * g.cache_cap * D * es, kv_b = lz * Hkv * Nn * D * es, q_b = lz * Hq * Nn * D * es;
+  const size_t segv_b = lz * Hkv * ctx->seg_cap_v * sizeof(float), sega_b = lz * Hkv * ctx->seg_cap_a * sizeof(float);
+  const size_t row_b = lz * Hq * Nn * sizeof(float), idx_b = lz * Hkv * g.cache_cap * sizeof(int32_t);
+  omnimem_cache s2{adv(src->k, cache_b), adv(src->v, cache_b), src->n_v + l0, src->n + l0};
+  omnimem_cache d2{adv(dst->k, cache_b), adv(dst->v, cache_b), dst->n_v + l0, dst->n + l0};
+  omnimem_chunk c2 = *chunk;
+  c2.k = adv(chunk->k, kv_b); c2.v = adv(chunk->v, kv_b); c2.q = adv(chunk->q, q_b);
+  c2.lse = (const float*)adv(chunk->lse, row_b);
+  omnimem_scores o2{};
+  if (opt_out) {
+    o2.a_v = (float*)adv(opt_out->a_v, segv_b); o2.a_a = (float*)adv(opt_out->a_a, sega_b);
+    o2.s_v = (float*)adv(opt_out->s_v, segv_b); o2.s_a = (float*)adv(opt_out->s_a, sega_b);
+    o2.psi_v = (float*)adv(opt_out->psi_v, segv_b); o2.psi_a = (float*)adv(opt_out->psi_a, sega_b);
+    o2.lse_out = (float*)adv(opt_out->lse_out, row_b); o2.row_entropy = (float*)adv(opt_out->row_entropy, row_b);
+    o2.stats = opt_out->stats + lz * 8;
+  }
+  // the workspace regions are [L, per-layer bytes] too
+  WsLayout w2 = w;
+  const size_t lse_stride = ((Nn + 127) / 128) * 128;   // the row stride the scoring kernels use for this chunk
+  w2.lse += lz * Hq * lse_stride * sizeof(float);
+  w2.cosn += lz * Hkv * ((size_t)ctx->seg_cap_v + ctx->seg_cap_a) * sizeof(float);
+  w2.partials += lz * 2 * (size_t)ctx->fin_blocks * 3 * sizeof(double);
+  w2.a_v += segv_b; w2.s_v += segv_b; w2.psi_v += segv_b;
+  w2.a_a += sega_b; w2.s_a += sega_b; w2.psi_a += sega_b;
+  w2.stats += lz * 8 * sizeof(double);
+  w2.M_v += lz * sizeof(int32_t); w2.M_a += lz * sizeof(int32_t);
+  w2.idx_v += idx_b; w2.idx_a += idx_b;
+  const int32_t* budget = layer_budget + l0;
+  // layers with nothing to evict skip scoring unless the caller asked for the scores
+  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, s2.n_v, s2.n, opt_out ? nullptr : budget, Lg);
+  StepBuffers b{};
+  fill_buffers(ctx, &s2, &c2, opt_out ? &o2 : nullptr, wsb, w2, b);
+  int rc = run_score(ctx, p, b, st);
+  if (rc) return rc;
+  int32_t* M_v = opt_M_v ? opt_M_v + l0 : (int32_t*)(wsb + w2.M_v);
+  int32_t* M_a = opt_M_a ? opt_M_a + l0 : (int32_t*)(wsb + w2.M_a);
+  int32_t* idx_v = opt_idx_v ? (int32_t*)adv(opt_idx_v, idx_b) : (int32_t*)(wsb + w2.idx_v);
+  int32_t* idx_a = opt_idx_a ? (int32_t*)adv(opt_idx_a, idx_b) : (int32_t*)(wsb + w2.idx_a);
+  cudaError_t e;
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_ALLOCATE);
+    e = launch_allocate(ctx, p, b.stats, budget, 0, M_v, M_a, nullptr, st, &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_SELECT);
+    e = launch_select(ctx, p, b.psi_v, b.psi_a, M_v, M_a, idx_v, idx_a, st, &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  {
+    StageTimer t(ctx, st, OMNIMEM_STAGE_COMPACT);
+    e = launch_compact(ctx, p, s2.k, s2.v, c2.k, c2.v, idx_v, idx_a, M_v, M_a, d2.k, d2.v, d2.n_v, d2.n, st,
+                       &ctx->launches);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
+  return OMNIMEM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -194,6 +280,11 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
     if (e != cudaSuccess) { delete c; return OMNIMEM_CUDA_ERROR; }
   }
   for (int s = 0; s < OMNIMEM_N_STAGES; ++s) c->ev_used[s] = false;
+  c->copy_stream = nullptr;
+  for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) c->ev_copy[i] = nullptr;
+  e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+  for (int i = 0; i <= OMNIMEM_HOST_GROUPS && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&c->ev_copy[i], cudaEventDisableTiming);
+  if (e != cudaSuccess) { omnimem_destroy(c); return OMNIMEM_CUDA_ERROR; }
   *out = c;
   return OMNIMEM_OK;
 }
@@ -201,6 +292,8 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
 int omnimem_destroy(omnimem_ctx* ctx) {
   if (!ctx) return OMNIMEM_INVALID_ARG;
   for (int i = 0; i < 2 * OMNIMEM_N_STAGES; ++i) cudaEventDestroy(ctx->ev[i]);
+  for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
   return OMNIMEM_OK;
 }
@@ -304,48 +397,11 @@ int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* src, const omn
                            const int32_t* layer_budget, omnimem_cache* dst, omnimem_scores* opt_out, int32_t* opt_idx_v,
                            int32_t* opt_idx_a, int32_t* opt_M_v, int32_t* opt_M_a, void* ws, size_t ws_bytes,
                            void* stream) {
-  if (!ctx || !layer_budget || !ws) return OMNIMEM_INVALID_ARG;
-  int rc = check_cache(src);
+  int rc = check_fused_args(ctx, src, chunk, layer_budget, dst, opt_out, ws, ws_bytes);
   if (rc) return rc;
-  rc = check_cache(dst);
-  if (rc) return rc;
-  rc = check_chunk(ctx, chunk, true);
-  if (rc) return rc;
-  if (opt_out && (rc = check_scores(opt_out))) return rc;
-  if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
-  const WsLayout w = ws_layout(ctx);
-  if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
-  cudaStream_t st = (cudaStream_t)stream;
-  uint8_t* wsb = (uint8_t*)ws;
   begin_call(ctx);
-  // layers with nothing to evict skip scoring unless the caller asked for the scores
-  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, opt_out ? nullptr : layer_budget);
-  StepBuffers b{};
-  fill_buffers(ctx, src, chunk, opt_out, wsb, w, b);
-  rc = run_score(ctx, p, b, st);
-  if (rc) return rc;
-  int32_t* M_v = opt_M_v ? opt_M_v : (int32_t*)(wsb + w.M_v);
-  int32_t* M_a = opt_M_a ? opt_M_a : (int32_t*)(wsb + w.M_a);
-  int32_t* idx_v = opt_idx_v ? opt_idx_v : (int32_t*)(wsb + w.idx_v);
-  int32_t* idx_a = opt_idx_a ? opt_idx_a : (int32_t*)(wsb + w.idx_a);
-  cudaError_t e;
-  {
-    StageTimer t(ctx, st, OMNIMEM_STAGE_ALLOCATE);
-    e = launch_allocate(ctx, p, b.stats, layer_budget, 0, M_v, M_a, nullptr, st, &ctx->launches);
-    if (e != cudaSuccess) return fail_cuda(ctx, e);
-  }
-  {
-    StageTimer t(ctx, st, OMNIMEM_STAGE_SELECT);
-    e = launch_select(ctx, p, b.psi_v, b.psi_a, M_v, M_a, idx_v, idx_a, st, &ctx->launches);
-    if (e != cudaSuccess) return fail_cuda(ctx, e);
-  }
-  {
-    StageTimer t(ctx, st, OMNIMEM_STAGE_COMPACT);
-    e = launch_compact(ctx, p, src->k, src->v, chunk->k, chunk->v, idx_v, idx_a, M_v, M_a, dst->k, dst->v, dst->n_v,
-                       dst->n, st, &ctx->launches);
-    if (e != cudaSuccess) return fail_cuda(ctx, e);
-  }
-  return OMNIMEM_OK;
+  return compress_layers(ctx, src, chunk, layer_budget, dst, opt_out, opt_idx_v, opt_idx_a, opt_M_v, opt_M_a,
+                         (uint8_t*)ws, 0, ctx->cfg.n_layers, (cudaStream_t)stream);
 }
 
 int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
@@ -356,39 +412,55 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   int rc = check_chunk(ctx, host_chunk, true);
   if (rc) return rc;
   if (!dev_chunk->k || !dev_chunk->v || !dev_chunk->q || (host_chunk->lse && !dev_chunk->lse)) return OMNIMEM_INVALID_ARG;
-  const WsLayout w = ws_layout(ctx);
-  if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
-  cudaStream_t st = (cudaStream_t)stream;
-  const omnimem_config& g = ctx->cfg;
-  const size_t es = g.dtype == OMNIMEM_FP32 ? 4 : 2;
-  const size_t Nn = (size_t)host_chunk->Nn_v + host_chunk->Nn_a;
-  const size_t kv_bytes = (size_t)g.n_layers * g.n_kv_heads * Nn * g.head_dim * es;
-  const size_t q_bytes = (size_t)g.n_layers * g.n_q_heads * Nn * g.head_dim * es;
-  const size_t lse_bytes = host_chunk->lse ? (size_t)g.n_layers * g.n_q_heads * Nn * sizeof(float) : 0;
-  cudaError_t e = cudaSuccess;
-  if (Nn > 0) {
-    e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->k), host_chunk->k, kv_bytes, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->v), host_chunk->v, kv_bytes, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<void*>(dev_chunk->q), host_chunk->q, q_bytes, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess && lse_bytes)
-      e = cudaMemcpyAsync(const_cast<float*>(dev_chunk->lse), host_chunk->lse, lse_bytes, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return fail_cuda(ctx, e);
-  }
   omnimem_chunk ch = *dev_chunk;
   ch.Nn_v = host_chunk->Nn_v;
   ch.Nn_a = host_chunk->Nn_a;
   if (!host_chunk->lse) ch.lse = nullptr;
-  uint8_t* wsb = (uint8_t*)ws;
-  int32_t* M_v = (int32_t*)(wsb + w.M_v);
-  int32_t* M_a = (int32_t*)(wsb + w.M_a);
-  rc = omnimem_compress_chunk(ctx, src, &ch, layer_budget, dst, nullptr, nullptr, nullptr, M_v, M_a, ws, ws_bytes, stream);
+  rc = check_fused_args(ctx, src, &ch, layer_budget, dst, nullptr, ws, ws_bytes);
   if (rc) return rc;
-  const size_t mb = (size_t)g.n_layers * sizeof(int32_t);
-  e = cudaMemcpyAsync(host_M_v, M_v, mb, cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(host_M_a, M_a, mb, cudaMemcpyDeviceToHost, st);
+  const WsLayout w = ws_layout(ctx);
+  cudaStream_t st = (cudaStream_t)stream;
+  const omnimem_config& g = ctx->cfg;
+  const int L = g.n_layers;
+  const size_t es = g.dtype == OMNIMEM_FP32 ? 4 : 2;
+  const size_t Nn = (size_t)host_chunk->Nn_v + host_chunk->Nn_a;
+  const size_t kv_layer = (size_t)g.n_kv_heads * Nn * g.head_dim * es;      // bytes per layer
+  const size_t q_layer = (size_t)g.n_q_heads * Nn * g.head_dim * es;
+  const size_t lse_layer = host_chunk->lse ? (size_t)g.n_q_heads * Nn * sizeof(float) : 0;
+  uint8_t* wsb = (uint8_t*)ws;
+  begin_call(ctx);
+  // Layers are independent through the whole step, so the chunk is copied and compressed in groups of layers: the
+  // copy of group g + 1 (on the context's copy stream) overlaps the kernels of group g (on `stream`).
+  const int per_group = (L + OMNIMEM_HOST_GROUPS - 1) / OMNIMEM_HOST_GROUPS;
+  cudaError_t e = cudaEventRecord(ctx->ev_copy[OMNIMEM_HOST_GROUPS], st);   // staging buffers are free once `stream` got here
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_copy[OMNIMEM_HOST_GROUPS], 0);
+  if (e != cudaSuccess) return fail_cuda(ctx, e);
+  auto at = [](const void* p, size_t bytes) { return (void*)((uint8_t*)const_cast<void*>(p) + bytes); };
+  int gi = 0;
+  for (int l0 = 0; l0 < L; l0 += per_group, ++gi) {
+    const int Lg = L - l0 < per_group ? L - l0 : per_group;
+    if (Nn > 0) {
+      cudaStream_t cs = ctx->copy_stream;
+      e = cudaMemcpyAsync(at(dev_chunk->k, l0 * kv_layer), at(host_chunk->k, l0 * kv_layer), Lg * kv_layer, cudaMemcpyHostToDevice, cs);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync(at(dev_chunk->q, l0 * q_layer), at(host_chunk->q, l0 * q_layer), Lg * q_layer, cudaMemcpyHostToDevice, cs);
+      if (e == cudaSuccess && lse_layer)
+        e = cudaMemcpyAsync(at(dev_chunk->lse, l0 * lse_layer), at(host_chunk->lse, l0 * lse_layer), Lg * lse_layer, cudaMemcpyHostToDevice, cs);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync(at(dev_chunk->v, l0 * kv_layer), at(host_chunk->v, l0 * kv_layer), Lg * kv_layer, cudaMemcpyHostToDevice, cs);
+      if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[gi], cs);
+      if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_copy[gi], 0);
+      if (e != cudaSuccess) return fail_cuda(ctx, e);
+    }
+    rc = compress_layers(ctx, src, &ch, layer_budget, dst, nullptr, nullptr, nullptr, nullptr, nullptr, wsb, l0, Lg, st);
+    if (rc) return rc;
+  }
+  const size_t mb = (size_t)L * sizeof(int32_t);
+  e = cudaMemcpyAsync(host_M_v, wsb + w.M_v, mb, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(host_M_a, wsb + w.M_a, mb, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) return fail_cuda(ctx, e);
-  if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? 2 * kv_bytes + q_bytes + lse_bytes : 0);
+  if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? (size_t)L * (2 * kv_layer + q_layer + lse_layer) : 0);
   if (d2h_bytes) *d2h_bytes = (int64_t)(2 * mb);
   return OMNIMEM_OK;
 }

@@ -69,6 +69,8 @@ struct TmaMaps;  // score_tc.cu
 
 }  // namespace omnimem
 
+#define OMNIMEM_HOST_GROUPS 8   // layer groups of the pipelined host entry
+
 struct omnimem_ctx {
   omnimem_config cfg;
   int device;
@@ -84,6 +86,8 @@ struct omnimem_ctx {
   bool ev_used[OMNIMEM_N_STAGES];
   int launches;
   void* encode_tiled;  // cuTensorMapEncodeTiled entry point
+  cudaStream_t copy_stream;                        // omnimem_compress_chunk_host: host -> device copies of the next layer group
+  cudaEvent_t ev_copy[OMNIMEM_HOST_GROUPS + 1];    // [g] group g is on the device; [last] `stream` reached the call
 };
 
 namespace omnimem {

@@ -299,3 +299,31 @@ def test_error_codes():
     with pytest.raises(OmniMemError, match="invalid"):
         eng.compress_chunk(src, chunk, Bt, src)                                                   # dst aliases src
     eng.close()
+
+
+def test_host_entry_matches_device_entry():
+    """omnimem_compress_chunk_host (chunk in pinned host memory, copied and compressed in layer groups on two streams)
+    must give exactly what omnimem_compress_chunk gives on the same inputs; 9 layers -> groups of 2 with a ragged tail."""
+    from paper_2606_07577_b200.omnimem import Chunk
+    for wl in (SMALL2.replace(L=9), I.CFG1.replace(L=3)):
+        x = I.full_inputs(wl, pin=True)
+        eng = engine_for(wl)
+        src, chunk = dev_objs(x, wl)
+        B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device="cuda")
+        dst = eng.new_cache()
+        M_v = torch.zeros(wl.L, dtype=torch.int32, device="cuda")
+        M_a = torch.zeros_like(M_v)
+        eng.compress_chunk(src, chunk, B, dst, M_v=M_v, M_a=M_a)
+        host_chunk = Chunk(x["chunkK"], x["chunkV"], x["Q"], wl.Nn_v, wl.Nn_a)
+        stage = Chunk(torch.zeros_like(chunk.k), torch.zeros_like(chunk.v), torch.zeros_like(chunk.q), wl.Nn_v, wl.Nn_a)
+        dst2 = eng.new_cache()
+        hM_v, hM_a = torch.zeros(wl.L, dtype=torch.int32).pin_memory(), torch.zeros(wl.L, dtype=torch.int32).pin_memory()
+        for _ in range(2):                                   # twice: the staging buffers are reused across calls
+            h2d, d2h = eng.compress_chunk_host(src, host_chunk, stage, B, dst2, hM_v, hM_a)
+        assert h2d == sum(t.numel() * t.element_size() for t in (x["chunkK"], x["chunkV"], x["Q"])) and d2h == 8 * wl.L
+        assert torch.equal(hM_v, M_v.cpu()) and torch.equal(hM_a, M_a.cpu())
+        assert torch.equal(dst2.n, dst.n) and torch.equal(dst2.n_v, dst.n_v)
+        for l in range(wl.L):
+            nl = int(dst.n[l])
+            assert torch.equal(dst2.k[l, :, :nl], dst.k[l, :, :nl]) and torch.equal(dst2.v[l, :, :nl], dst.v[l, :, :nl])
+        eng.close()
