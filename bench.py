@@ -206,6 +206,21 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     clocks = clk.summary()
     eng.set_profiling(False)
 
+    # ---- NEXT-1 context: the caller (the model's own attention forward, Eq.1) supplies the row LSE -> pass 1 is skipped
+    sc = eng.score(src, chunk, want_lse=True)
+    chunk_lse = Chunk(chunk.k, chunk.v, chunk.q, wl.Nn_v, wl.Nn_a, lse=sc.lse)
+    for _ in range(2):
+        eng.compress_chunk(src, chunk_lse, B, dst)
+    barrier()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record()
+    for _ in range(args.steps):
+        eng.compress_chunk(src, chunk_lse, B, dst)
+    ev3.record()
+    barrier()
+    t_one_pass = ev2.elapsed_time(ev3) / 1e3 / args.steps
+    del sc
+
     # ---- end to end through the C ABI with HOST buffers (H2D of the chunk + D2H of the budgets inside the region)
     h2d = d2h = 0
     for _ in range(2):
@@ -244,12 +259,14 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
         "roofline": {"bound": "tensor", "kernel": f"score_tc_kernel<{2 if dom == 'colsum' else 1}> ({dom})",
                      "achieved": achieved, "peak": peaks["tf_sust"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sust"],
                      "peak_source": f"{peaks['src']} bf16 sustained (kernel timed inside the step)",
-                     "frac_of_burst": achieved / peaks["tf_burst"], "traffic": NCU_TRAFFIC_BYTES.get(dom),
+                     "frac_of_burst": achieved / peaks["tf_burst"], "traffic": NCU_TRAFFIC_BYTES.get(dom) if wl.name == I.CFG2.name else None,
                      "algorithmic_flops_per_launch": work["f_pass"], "exps_per_launch": work["exps_pass"]},
         "step_roofline": {"t_roof_ms": t_roof * 1e3, "frac_two_pass": t_roof / t_step,
                           "frac_one_pass_normalised": t_roof / 2 / t_step, "bytes": work["bytes"]["total"],
                           "flops_two_pass": 2 * work["f_pass"]},
     }
+    out["supplied_lse"] = {"ms_per_step": t_one_pass * 1e3, "value": world * work["Nk"] / t_one_pass, "unit": "KV tok/s",
+                           "note": "row LSE supplied by the caller (chunk.lse): scoring pass 1 skipped; context, not the headline"}
     if world == 1 and not args.no_cpu_baseline:
         from oracle import ref
         secs = oracle_sample_seconds(wl, 0, [0, 1][: wl.Hkv])
@@ -262,8 +279,59 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     print(json.dumps(out), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------ streaming (cfg5)
+def run_stream(args, wl: I.Workload, local_rank: int):
+    """BASELINE.json configs[4]: `chunks` consecutive chunks from an empty cache, free-running on the device state
+    (ping-pong caches, no host sync inside a step).  Per-chunk CUDA-event times -> p50 / p99 over all chunks and over
+    the steady-state ones (cache full), total ingest tok/s = chunks * Nn / sum(t)."""
+    from paper_2606_07577_b200.omnimem import Chunk, OmniMem
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    eng = OmniMem.for_workload(wl, device=str(dev))
+    src, dst = eng.new_cache(), eng.new_cache()
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
+    n_chunks = args.chunks or wl.steps
+    x = I.full_inputs(wl, step=0, with_cache=False)
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+    scratch = eng.new_cache()
+    for _ in range(max(args.warmup, 3)):                      # warm-up on a scratch destination: the stream state is untouched
+        eng.compress_chunk(src, chunk, B, scratch)
+    del scratch
+    torch.cuda.synchronize(dev)
+    times, rows = [], []
+    with ClockSampler(local_rank) as clk:
+        for step in range(n_chunks):
+            if step:
+                x = I.full_inputs(wl, step=step, with_cache=False)
+                chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+            rows.append(int(src.n[0]) + wl.Nn)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record()
+            eng.compress_chunk(src, chunk, B, dst)
+            ev1.record()
+            torch.cuda.synchronize(dev)
+            times.append(ev0.elapsed_time(ev1))
+            src, dst = dst, src
+    t = np.array(times)
+    steady = t[np.array(rows) >= wl.budget + wl.Nn] if any(r >= wl.budget + wl.Nn for r in rows) else t
+    total_s = t.sum() / 1e3
+    pct = lambda a, q: float(np.percentile(a, q))
+    print(json.dumps({
+        "metric": "kv_tokens_per_s", "value": float(np.mean(rows)) / (t.mean() / 1e3), "unit": "KV tok/s", "n_gpus": 1,
+        "steps": n_chunks, "warmup": max(args.warmup, 3), "ms_per_step": float(t.mean()), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype, "data": "synthetic",
+        "config": {"workload": wl.name, "L": wl.L, "Hq": wl.Hq, "Hkv": wl.Hkv, "D": wl.D, "chunk_rows": wl.Nn,
+                   "budget": wl.budget, "chunks": n_chunks, "l2": "inputs larger than L2; no flush"},
+        "clocks": clk.summary(),
+        "stream": {"p50_ms": pct(t, 50), "p99_ms": pct(t, 99), "steady_p50_ms": pct(steady, 50),
+                   "steady_p99_ms": pct(steady, 99), "steady_chunks": int(len(steady)), "total_s": total_s,
+                   "ingest_tok_per_s": n_chunks * wl.Nn / total_s, "ms_per_chunk": [round(v, 3) for v in times],
+                   "rows_scored": rows},
+    }), flush=True)
+
+
 # per-launch DRAM bytes of the scoring kernels from the committed ncu --set full capture (profiles/); None = not captured
-NCU_TRAFFIC_BYTES = {"colsum": None, "lse": None}
+NCU_TRAFFIC_BYTES = {"colsum": 1.7907e9, "lse": 1.7817e9}   # profiles/r01_score_tc_full_cfg2.csv (CFG2 only)
 
 
 def main():
@@ -274,12 +342,16 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[i-1]; 2 = the config the metric is quoted on")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--chunks", type=int, default=0, help="config 5 only: chunks in the stream (default: the config's 60)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     wl = I.CONFIGS[args.config]
     rank, local_rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":
         run_reference(args, wl, rank, world)
+        return
+    if wl.steps > 1 and world == 1:
+        run_stream(args, wl, local_rank)
         return
     if world > 1:
         import torch.distributed as dist
