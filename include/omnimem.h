@@ -133,6 +133,18 @@ OMNIMEM_API int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const in
                      int32_t Nn_a, const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
                      int32_t* layer_budget_out, void* stream);
 
+/* ---- offline calibration of the per-layer totals (Eq.13-14; NEXT-2 of SURVEY.md section 8(f)) ---------- */
+/* "The budget is determined offline for each model based on a small calibration set of videos".  Reading R28:
+ * the statistics of every calibration chunk (stats [L,8] as written by omnimem_score) are summed into
+ * acc [(L+1)*8] doubles (DEVICE, zeroed by the caller before the first chunk; acc[8 l + i] = sum of statistic i of layer
+ * l, acc[8 L] = number of chunks); omnimem_calibrate_budgets writes their arithmetic means to mean_stats_out [L,8]
+ * (DEVICE) and B^(l) = Softmax_l(C^(l)/T) * total_budget with C^(l) = mean Hn_all * (1 - mean sbar_all) (Eq.13-14,
+ * clamp and rounding as in omnimem_allocate, R19-R20) to layer_budget_out [L] (DEVICE), the table that
+ * omnimem_compress_chunk takes as `layer_budget`.  Errors: INVALID_ARG, CUDA_ERROR. */
+OMNIMEM_API int omnimem_calibrate_accumulate(omnimem_ctx* ctx, const double* stats, double* acc, void* stream);
+OMNIMEM_API int omnimem_calibrate_budgets(omnimem_ctx* ctx, const double* acc, int64_t total_budget, double* mean_stats_out,
+                              int32_t* layer_budget_out, void* stream);
+
 /* ---- stage 4: segmented top-M (Eq.4-5) ---------------------------------------------------------------- */
 /* psi_m [L, Hkv, seg_cap_m] fp32 (finite); per (l, h, m) writes the segment-local indices of the M_m[l] largest
  * psi to idx_m[l, h, 0:M_m[l]) in ASCENDING index order; among equal psi the lowest index wins (R23).

@@ -186,6 +186,15 @@ def layer_budgets(p: RefParams, st, total: int):
     return out
 
 
+def calibrate_budgets(p: RefParams, stats_per_chunk, total: int):
+    """Offline per-layer totals ("determined offline ... based on a small calibration set", reading R28):
+    arithmetic mean over the calibration chunks of each layer's statistics, then Eq.13-14 on the means
+    (C^(l) = mean Hn_all * (1 - mean sbar_all)).  stats_per_chunk: [n_chunks, L, 8].  Returns (B [L] int32, mean [L,8])."""
+    st = np.asarray(stats_per_chunk, np.float64)
+    mean = st.sum(axis=0) / st.shape[0]
+    return layer_budgets(p, mean, total), mean
+
+
 def allocate(p: RefParams, st, n_v, n, layer_budget):
     st, n_v, n, layer_budget = f64(st), i32(n_v), i32(n), i32(layer_budget)
     M_v = np.zeros((p.L,), np.int32)

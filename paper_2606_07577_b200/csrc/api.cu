@@ -361,6 +361,25 @@ int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const int32_t* n_v, 
   return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
 }
 
+int omnimem_calibrate_accumulate(omnimem_ctx* ctx, const double* stats, double* acc, void* stream) {
+  if (!ctx || !stats || !acc) return OMNIMEM_INVALID_ARG;
+  begin_call(ctx);
+  cudaError_t e = launch_calib_accumulate(ctx->cfg.n_layers, stats, acc, (cudaStream_t)stream, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
+int omnimem_calibrate_budgets(omnimem_ctx* ctx, const double* acc, int64_t total_budget, double* mean_stats_out,
+                              int32_t* layer_budget_out, void* stream) {
+  if (!ctx || !acc || !mean_stats_out || !layer_budget_out || total_budget < 0) return OMNIMEM_INVALID_ARG;
+  begin_call(ctx);
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = launch_calib_mean(ctx->cfg.n_layers, acc, mean_stats_out, st, &ctx->launches);
+  if (e != cudaSuccess) return fail_cuda(ctx, e);
+  StepParams p = make_params(ctx, 0, 0, nullptr, nullptr, nullptr);
+  e = launch_allocate(ctx, p, mean_stats_out, nullptr, total_budget, nullptr, nullptr, layer_budget_out, st, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
 int omnimem_select(omnimem_ctx* ctx, const float* psi_v, const float* psi_a, const int32_t* n_v, const int32_t* n,
                    int32_t Nn_v, int32_t Nn_a, const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a,
                    void* ws, size_t ws_bytes, void* stream) {

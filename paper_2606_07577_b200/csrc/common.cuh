@@ -102,6 +102,8 @@ cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const S
 cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,
                             int64_t total_budget, int32_t* M_v, int32_t* M_a, int32_t* layer_budget_out, cudaStream_t st,
                             int* launches);
+cudaError_t launch_calib_accumulate(int L, const double* stats, double* acc, cudaStream_t st, int* launches);
+cudaError_t launch_calib_mean(int L, const double* acc, double* mean, cudaStream_t st, int* launches);
 cudaError_t launch_select(const omnimem_ctx* ctx, const StepParams& p, const float* psi_v, const float* psi_a,
                           const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a, cudaStream_t st,
                           int* launches);

@@ -289,10 +289,11 @@ __global__ void __launch_bounds__(128) allocate_kernel(StepParams p, AllocParams
   }
   __syncthreads();
   for (int l = threadIdx.x; l < L; l += blockDim.x) {
-    const int n_v = p.n_v[l], n = p.n[l];
-    const int Kv = seg_len(p, n_v, n, 0), Ka = seg_len(p, n_v, n, 1);
     const int Bl = B[l] < 0 ? 0 : B[l];
     if (layer_budget_out) layer_budget_out[l] = Bl;
+    if (M_v == nullptr) continue;   // calibration: only the per-layer totals are wanted
+    const int n_v = p.n_v[l], n = p.n[l];
+    const int Kv = seg_len(p, n_v, n, 0), Ka = seg_len(p, n_v, n, 1);
     if (Kv + Ka <= Bl) { M_v[l] = Kv; M_a[l] = Ka; continue; }
     const double Cv = stats[l * 8 + 4], Ca = stats[l * 8 + 5];
     const double den = ap.ratio_r * Cv + Ca;
@@ -312,6 +313,32 @@ cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const d
                  (long long)ctx->cfg.budget_min, (long long)ctx->cfg.budget_max};
   const size_t smem = (size_t)p.L * (2 * sizeof(double) + 2 * sizeof(int));
   allocate_kernel<<<1, 128, smem, st>>>(p, ap, stats, layer_budget, M_v, M_a, layer_budget_out);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Offline calibration of the per-layer totals ("determined offline ... on a small calibration set", R28):
+// acc[l][0..8) += stats[l][0..8) per calibration chunk, acc[L][0] counts the chunks; the budgets are Eq.13-14 on the
+// arithmetic means of the two layer measures (normalised entropy, mean similarity).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void calib_accumulate_kernel(int L, const double* __restrict__ stats, double* __restrict__ acc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < L * 8) acc[i] += stats[i];
+  if (i == 0) acc[L * 8] += 1.0;
+}
+__global__ void calib_mean_kernel(int L, const double* __restrict__ acc, double* __restrict__ mean) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const double cnt = acc[L * 8];
+  if (i < L * 8) mean[i] = cnt > 0.0 ? acc[i] / cnt : 0.0;
+}
+cudaError_t launch_calib_accumulate(int L, const double* stats, double* acc, cudaStream_t st, int* launches) {
+  calib_accumulate_kernel<<<(L * 8 + 127) / 128, 128, 0, st>>>(L, stats, acc);
+  ++*launches;
+  return cudaGetLastError();
+}
+cudaError_t launch_calib_mean(int L, const double* acc, double* mean, cudaStream_t st, int* launches) {
+  calib_mean_kernel<<<(L * 8 + 127) / 128, 128, 0, st>>>(L, acc, mean);
   ++*launches;
   return cudaGetLastError();
 }

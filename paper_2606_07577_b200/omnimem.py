@@ -21,7 +21,8 @@ STAGES = ("lse", "colsum", "cosine", "finalize", "allocate", "select", "compact"
 STAT_NAMES = ("Hn_v", "Hn_a", "sbar_v", "sbar_a", "C_v", "C_a", "Hn_all", "sbar_all")
 EXPORTS = ("omnimem_create", "omnimem_destroy", "omnimem_workspace_bytes", "omnimem_seg_cap", "omnimem_strerror",
            "omnimem_last_cuda_error", "omnimem_score", "omnimem_allocate", "omnimem_select", "omnimem_compact",
-           "omnimem_compress_chunk", "omnimem_compress_chunk_host", "omnimem_set_profiling", "omnimem_get_stage_ms")
+           "omnimem_compress_chunk", "omnimem_compress_chunk_host", "omnimem_set_profiling", "omnimem_get_stage_ms",
+           "omnimem_calibrate_accumulate", "omnimem_calibrate_budgets")
 
 
 class OmniMemError(RuntimeError):
@@ -76,6 +77,8 @@ def load_library() -> C.CDLL:
         lib.omnimem_score.argtypes = [vp, C.POINTER(omnimem_cache), C.POINTER(omnimem_chunk), C.POINTER(omnimem_scores),
                                       vp, C.c_size_t, vp]
         lib.omnimem_allocate.argtypes = [vp, vp, vp, vp, i32, i32, vp, i64, vp, vp, vp, vp]
+        lib.omnimem_calibrate_accumulate.argtypes = [vp, vp, vp, vp]
+        lib.omnimem_calibrate_budgets.argtypes = [vp, vp, i64, vp, vp, vp]
         lib.omnimem_select.argtypes = [vp, vp, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, C.c_size_t, vp]
         lib.omnimem_compact.argtypes = [vp, C.POINTER(omnimem_cache), C.POINTER(omnimem_chunk), vp, vp, vp, vp,
                                         C.POINTER(omnimem_cache), vp]
@@ -233,6 +236,22 @@ class OmniMem:
                     "omnimem_allocate")
         return M_v, M_a, B_out
 
+    def new_calibration(self) -> torch.Tensor:
+        """Zeroed accumulator of omnimem_calibrate_accumulate: [(L+1)*8] doubles on the device."""
+        return torch.zeros((self.L + 1) * 8, dtype=torch.float64, device=self.device)
+
+    def calibrate_accumulate(self, stats: torch.Tensor, acc: torch.Tensor) -> torch.Tensor:
+        self._check(self.lib.omnimem_calibrate_accumulate(self.ctx, _ptr(stats), _ptr(acc), _stream()),
+                    "omnimem_calibrate_accumulate")
+        return acc
+
+    def calibrate_budgets(self, acc: torch.Tensor, total_budget: int):
+        mean_stats = torch.zeros(self.L, 8, dtype=torch.float64, device=self.device)
+        B = torch.zeros(self.L, dtype=torch.int32, device=self.device)
+        self._check(self.lib.omnimem_calibrate_budgets(self.ctx, _ptr(acc), int(total_budget), _ptr(mean_stats), _ptr(B),
+                                                       _stream()), "omnimem_calibrate_budgets")
+        return B, mean_stats
+
     def select(self, psi_v: torch.Tensor, psi_a: torch.Tensor, n_v: torch.Tensor, n: torch.Tensor, Nn_v: int, Nn_a: int,
                M_v: torch.Tensor, M_a: torch.Tensor, idx_v: Optional[torch.Tensor] = None,
                idx_a: Optional[torch.Tensor] = None):
@@ -288,6 +307,8 @@ class OmniMem:
 def omnimem_score(ctx: OmniMem, *a, **k): return ctx.score(*a, **k)
 def omnimem_allocate(ctx: OmniMem, *a, **k): return ctx.allocate(*a, **k)
 def omnimem_select(ctx: OmniMem, *a, **k): return ctx.select(*a, **k)
+def omnimem_calibrate_accumulate(ctx: OmniMem, *a, **k): return ctx.calibrate_accumulate(*a, **k)
+def omnimem_calibrate_budgets(ctx: OmniMem, *a, **k): return ctx.calibrate_budgets(*a, **k)
 def omnimem_compact(ctx: OmniMem, *a, **k): return ctx.compact(*a, **k)
 def omnimem_compress_chunk(ctx: OmniMem, *a, **k): return ctx.compress_chunk(*a, **k)
 def omnimem_compress_chunk_host(ctx: OmniMem, *a, **k): return ctx.compress_chunk_host(*a, **k)

@@ -327,3 +327,52 @@ def test_host_entry_matches_device_entry():
             nl = int(dst.n[l])
             assert torch.equal(dst2.k[l, :, :nl], dst.k[l, :, :nl]) and torch.equal(dst2.v[l, :, :nl], dst.v[l, :, :nl])
         eng.close()
+
+
+def test_offline_calibration_and_ragged_layer_budgets():
+    """NEXT-2 (R28): statistics of several calibration chunks are accumulated on the device, Eq.13-14 on their
+    means give the per-layer table, and the fused step then runs with those RAGGED per-layer totals.  Layers get
+    different redundancy (AR(1) rho) so that the table is far from uniform."""
+    wl = I.CFG1.replace(L=6, cache_cap=700, budget=300)
+    L, n_cal = wl.L, 3
+    eng = engine_for(wl, budget_min=120, budget_max=520)
+    p = ref_params(wl, L, budget_min=120, budget_max=520)
+    acc = eng.new_calibration()
+    ref_stats = []
+    for c in range(n_cal):
+        x = I.full_inputs(wl, step=c)
+        for l in range(L):                                   # make the layers differ: a common offset raises the value
+            x["cacheV"][l] += 0.3 * l                        # similarity, a larger query scale lowers the entropy
+            x["chunkV"][l] += 0.3 * l
+            x["Q"][l] *= 0.3 + 0.5 * l
+        orc = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+        ref_stats.append(orc["stats"])
+        src, chunk = dev_objs(x, wl)
+        sc = eng.score(src, chunk)
+        eng.calibrate_accumulate(sc.stats, acc)
+    total = 300 * L
+    B_ref, mean_ref = ref.calibrate_budgets(p, np.stack(ref_stats), total)
+    B_gpu, mean_gpu = eng.calibrate_budgets(acc, total)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(mean_gpu.cpu().numpy()[:, 6:8], mean_ref[:, 6:8], rtol=1e-5, atol=1e-7)
+    Bg = B_gpu.cpu().numpy()
+    assert Bg.sum() == total == B_ref.sum() and Bg.min() >= 120 and Bg.max() <= 520
+    assert np.abs(Bg - B_ref).max() <= 1, f"{Bg} vs {B_ref}"          # statistics agree to 1e-6: at most a rounding flip
+    assert Bg.max() - Bg.min() > 50, "calibration inputs should give a visibly non-uniform table"
+    # the fused step under the oracle's ragged table: kept sets identical (fp32)
+    x = I.full_inputs(wl, step=n_cal)
+    orc = ref.compress_chunk(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"], B_ref)
+    src, chunk = dev_objs(x, wl)
+    dst = eng.new_cache()
+    idx_v, idx_a = eng.new_indices()
+    M_v = torch.zeros(L, dtype=torch.int32, device="cuda")
+    M_a = torch.zeros_like(M_v)
+    eng.compress_chunk(src, chunk, torch.from_numpy(B_ref).cuda(), dst, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+    torch.cuda.synchronize()
+    assert np.array_equal(M_v.cpu().numpy(), orc["M_v"]) and np.array_equal(dst.n.cpu().numpy(), orc["n_out"])
+    assert np.array_equal(dst.n.cpu().numpy(), np.minimum(B_ref, x["n"].numpy() + wl.Nn))
+    for l in range(L):
+        nl = int(orc["n_out"][l])
+        assert np.array_equal(idx_v[l, :, :orc["M_v"][l]].cpu().numpy(), orc["idx_v"][l, :, :orc["M_v"][l]])
+        assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][l, :, :nl])
+    eng.close()

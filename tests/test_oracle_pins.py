@@ -356,6 +356,33 @@ def test_layer_budgets_invariants():
     assert np.all(np.diff(b[np.argsort(C9)]) >= 0)            # monotone in compressibility
 
 
+def test_calibration_means_then_eq14():
+    """R28: budgets from the MEANS of the two layer measures over the calibration chunks.  Pins: one chunk ==
+    plain Eq.14; chunks that are permutations of each other give the same table; closed form of the two-layer case
+    B_0 / B_1 = exp((C_0 - C_1) / T); identical layers => uniform."""
+    L, total = 5, 5 * 1000
+    g = np.random.default_rng(11)
+    st = np.zeros((4, L, 8))
+    st[:, :, 6], st[:, :, 7] = g.uniform(0.6, 0.95, (4, L)), g.uniform(0.0, 0.4, (4, L))
+    p = ref.RefParams(L=L, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=0.2)
+    b1, m1 = ref.calibrate_budgets(p, st[:1], total)
+    assert np.array_equal(b1, ref.layer_budgets(p, st[0], total)) and np.array_equal(m1, st[0])
+    b, m = ref.calibrate_budgets(p, st, total)
+    b_perm, _ = ref.calibrate_budgets(p, st[[2, 0, 3, 1]], total)
+    assert np.array_equal(b, b_perm) and b.sum() == total
+    np.testing.assert_allclose(m[:, 6], st[:, :, 6].mean(0), rtol=1e-15)
+    C = st[:, :, 6].mean(0) * (1.0 - st[:, :, 7].mean(0))              # product of means, not mean of products
+    pi = np.exp(C / 0.2) / np.exp(C / 0.2).sum()
+    assert np.all(np.abs(b - pi * total) < 1.0)
+    p2 = ref.RefParams(L=2, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=0.2)
+    st2 = np.zeros((3, 2, 8))
+    st2[:, 0, 6], st2[:, 1, 6] = [0.9, 0.8, 0.7], [0.6, 0.7, 0.5]      # means 0.8 and 0.6, sbar = 0
+    b2, _ = ref.calibrate_budgets(p2, st2, 10**6)
+    assert abs(b2[0] / b2[1] - np.exp((0.8 - 0.6) / 0.2)) < 1e-4
+    st[:, :, 6], st[:, :, 7] = 0.8, 0.3
+    assert list(ref.calibrate_budgets(p, st, total)[0]) == [1000] * L
+
+
 # ------------------------------------------------------------------------------------------ O7 (Eq.4-5)
 def run_select(psi_row, M):
     K = len(psi_row)
