@@ -159,6 +159,23 @@ def run_reference(args, wl: I.Workload, rank: int, world: int):
     }), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------ rank plumbing
+def max_over_ranks(values, device, world: int):
+    """Every timing is reported as the MAX over ranks (reporting only: the data path has no collective, DESIGN.md
+    section 9).  Works on any backend (nccl on the GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch.distributed as dist
+    tt = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt]
+
+
+def job_value(world: int, units_per_rank: float, seconds: float) -> float:
+    """Whole-job throughput of N independent replicas (weak scaling): all ranks' units over the slowest rank's time."""
+    return world * units_per_rank / seconds
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     import torch.distributed as dist
@@ -218,7 +235,7 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
         eng.compress_chunk(src, chunk_lse, B, dst)
     ev3.record()
     barrier()
-    t_one_pass = ev2.elapsed_time(ev3) / 1e3 / args.steps
+    t_one_pass = ev2.elapsed_time(ev3) / 1e3
     del sc
 
     # ---- end to end through the C ABI with HOST buffers (H2D of the chunk + D2H of the budgets inside the region)
@@ -226,16 +243,15 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     for _ in range(2):
         h2d, d2h = eng.compress_chunk_host(src, host_chunk, chunk, B, dst, host_M_v, host_M_a)
     barrier()
-    t0 = time.perf_counter()
+    ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev4.record()
     for _ in range(args.steps):
-        eng.compress_chunk_host(src, host_chunk, chunk, B, dst, host_M_v, host_M_a)
-    torch.cuda.synchronize(dev)
-    t_e2e = time.perf_counter() - t0
+        eng.compress_chunk_host(src, host_chunk, chunk, B, dst, host_M_v, host_M_a)   # synchronises the stream itself
+    ev5.record()
+    barrier()
+    t_e2e = ev4.elapsed_time(ev5) / 1e3
 
-    if world > 1:
-        tt = torch.tensor([t_total, t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)          # max over ranks (reporting only; no data-path collective)
-        t_total, t_e2e = float(tt[0]), float(tt[1])
+    t_total, t_e2e, t_one_pass = max_over_ranks([t_total, t_e2e, t_one_pass], dev, world)
     if rank != 0:
         return
     t_step = t_total / args.steps
@@ -245,14 +261,14 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     achieved = work["f_pass"] / t_dom / 1e12 if t_dom > 0 else 0.0
     t_roof = max(2 * work["f_pass"] / (peaks["tf_sust"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
     out = {
-        "metric": "kv_tokens_per_s", "value": world * work["Nk"] / t_step, "unit": "KV tok/s", "n_gpus": world,
+        "metric": "kv_tokens_per_s", "value": job_value(world, work["Nk"], t_step), "unit": "KV tok/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype, "data": "synthetic",
         "config": {"workload": wl.name, "L": wl.L, "Hq": wl.Hq, "Hkv": wl.Hkv, "D": wl.D, "cache_rows": wl.n_v + wl.n_a,
                    "chunk_rows": wl.Nn, "budget": wl.budget, "parallelism": f"replicas x{world}",
                    "l2": "inputs larger than L2 (Q+K+V per step >> 126 MB); no flush", "gen_s": round(t_gen, 1)},
         "clocks": clocks,
-        "e2e": {"value": world * work["Nk"] / (t_e2e / args.steps), "unit": "KV tok/s", "ms_per_step": t_e2e / args.steps * 1e3,
+        "e2e": {"value": job_value(world, work["Nk"], t_e2e / args.steps), "unit": "KV tok/s", "ms_per_step": t_e2e / args.steps * 1e3,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": launches,
         "stage_ms": stage_ms,
@@ -265,7 +281,8 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
                           "frac_one_pass_normalised": t_roof / 2 / t_step, "bytes": work["bytes"]["total"],
                           "flops_two_pass": 2 * work["f_pass"]},
     }
-    out["supplied_lse"] = {"ms_per_step": t_one_pass * 1e3, "value": world * work["Nk"] / t_one_pass, "unit": "KV tok/s",
+    t_one_pass /= args.steps
+    out["supplied_lse"] = {"ms_per_step": t_one_pass * 1e3, "value": job_value(world, work["Nk"], t_one_pass), "unit": "KV tok/s",
                            "note": "row LSE supplied by the caller (chunk.lse): scoring pass 1 skipped; context, not the headline"}
     if world == 1 and not args.no_cpu_baseline:
         from oracle import ref
