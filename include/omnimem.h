@@ -76,6 +76,9 @@ typedef struct {
   int32_t sim_source;                      /* Eq.7 vectors: 0 = value rows (default), 1 = key rows            */
   int32_t sim_stride_v, sim_stride_a;      /* neighbour distance of Eq.7 per modality; 1 = paper literal (R11)       */
   int32_t score_path;                      /* 0 = auto (tcgen05 for bf16 D=128, SIMT otherwise), 1 = force SIMT      */
+  int32_t select_scope;                    /* 0 = one index set per (layer, KV head) (north_star, R5);
+                                              1 = one index set per layer, the paper-literal reading of P:68-74 where
+                                              I carries no head index (R29): psi = (sum_h a)^lambda (1 - mean_h s)         */
 } omnimem_config;
 
 typedef struct {     /* one pooled KV cache */

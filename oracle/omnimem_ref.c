@@ -215,6 +215,34 @@ int omnimem_ref_psi(const omnimem_ref_params* p, const int32_t* n_v, const int32
   return 0;
 }
 
+/* ---- O4': the paper-literal selection score, one per token and layer (R29) --------------------
+ * Eq.4-5 write the index sets I_{c,v}^{(l)}, I_{c,a}^{(l)} with no head index and Eq.6 an
+ * importance a_k with none either: the token is scored once per layer.  Reading R29: the importance is summed
+ * over ALL query heads (= the sum over KV heads of the per-group sums), the redundancy of Eq.7 taken on value
+ * rows is averaged over the KV heads, psi = A^lambda (1 - S) (Eq.8).  Every head's row of the output gets
+ * the same score, so Select returns the same index set for every head of the layer. */
+int omnimem_ref_psi_shared(const omnimem_ref_params* p, const int32_t* n_v, const int32_t* n, const double* a_v,
+                           const double* a_a, const double* s_v, const double* s_a, float* psi_v, float* psi_a) {
+  for (int l = 0; l < p->L; ++l)
+    for (int m = 0; m < 2; ++m) {
+      const int Km = seg_len(p, n_v[l], n[l], m);
+      const int cap = m == 0 ? p->seg_cap_v : p->seg_cap_a;
+      const double* a = m == 0 ? a_v : a_a;
+      const double* s = m == 0 ? s_v : s_a;
+      float* out = m == 0 ? psi_v : psi_a;
+      for (int t = 0; t < cap; ++t) {
+        double A = 0.0, S = 0.0;
+        for (int h = 0; h < p->Hkv; ++h) {
+          A += a[IDX3(l, h, t, p->Hkv, cap)];
+          S += s[IDX3(l, h, t, p->Hkv, cap)];
+        }
+        const float v = t < Km ? (float)(pow(A, p->lambda) * (1.0 - S / p->Hkv)) : 0.0f;
+        for (int h = 0; h < p->Hkv; ++h) out[IDX3(l, h, t, p->Hkv, cap)] = v;
+      }
+    }
+  return 0;
+}
+
 /* ---- O5: AVBA statistics (Eq.9-10; Eq.13) -------------------------------
  * Per layer and modality: A_m[t] = sum_h a[l,h,m,t]; abar = A_m / sum_t A_m (R16);
  * Hn_m = H[abar] / ln K_m (natural log, 0 ln 0 = 0, K_m <= 1 or empty mass => 0, R15);

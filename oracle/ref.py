@@ -153,14 +153,15 @@ def redundancy(p: RefParams, cacheX, n_v, n, chunkX):
 
 
 # ---- O4 ----------------------------------------------------------------------------------------
-def psi(p: RefParams, n_v, n, a_v, a_a, s_v, s_a):
+def psi(p: RefParams, n_v, n, a_v, a_a, s_v, s_a, select_scope: int = 0):
+    """select_scope 0: Eq.8 per (layer, KV head); 1: once per layer, paper-literal index sets (R29)."""
     n_v, n = i32(n_v), i32(n)
     a_v, a_a, s_v, s_a = f64(a_v), f64(a_a), f64(s_v), f64(s_a)
     psi_v = np.zeros((p.L, p.Hkv, p.seg_cap_v), np.float32)
     psi_a = np.zeros((p.L, p.Hkv, p.seg_cap_a), np.float32)
     cp = p.c()
-    _check(lib().omnimem_ref_psi(C.byref(cp), _p(n_v), _p(n), _p(a_v), _p(a_a), _p(s_v), _p(s_a), _p(psi_v),
-                                 _p(psi_a)), "psi")
+    fn = lib().omnimem_ref_psi_shared if select_scope == 1 else lib().omnimem_ref_psi
+    _check(fn(C.byref(cp), _p(n_v), _p(n), _p(a_v), _p(a_a), _p(s_v), _p(s_a), _p(psi_v), _p(psi_a)), "psi")
     return psi_v, psi_a
 
 
@@ -247,7 +248,8 @@ def compact(p: RefParams, cacheX, chunkX, n_v, n, idx_v, idx_a, M_v, M_a):
 
 
 # ---- the whole step, in the paper's order ------------------------------------------------------------
-def score(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source: int = 0, want_rowH: bool = False):
+def score(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source: int = 0, want_rowH: bool = False,
+          select_scope: int = 0):
     """Stages 1-3a: a, s, psi, statistics (Eq.6-10, 13).  Returns a dict of numpy arrays."""
     a_log, lse, rowH = attention(p, cacheK, n, chunkK, Q, want_rowH)
     a_v, a_a = split(p, a_log, n_v, n)
@@ -255,16 +257,16 @@ def score(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source: i
         s_v, s_a = redundancy(p, cacheV, n_v, n, chunkV)
     else:
         s_v, s_a = redundancy(p, cacheK, n_v, n, chunkK)
-    psi_v, psi_a = psi(p, n_v, n, a_v, a_a, s_v, s_a)
+    psi_v, psi_a = psi(p, n_v, n, a_v, a_a, s_v, s_a, select_scope)
     st = stats(p, n_v, n, a_v, a_a, s_v, s_a)
     return dict(a_log=a_log, lse=lse, rowH=rowH, a_v=a_v, a_a=a_a, s_v=s_v, s_a=s_a, psi_v=psi_v, psi_a=psi_a,
                 stats=st)
 
 
 def compress_chunk(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, layer_budget, sim_source: int = 0,
-                   want_rowH: bool = False):
+                   want_rowH: bool = False, select_scope: int = 0):
     """One full step: score -> allocate -> select -> compact.  `layer_budget` is an int array [L]."""
-    out = score(p, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source, want_rowH)
+    out = score(p, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source, want_rowH, select_scope)
     M_v, M_a = allocate(p, out["stats"], n_v, n, layer_budget)
     idx_v, idx_a = select(p, out["psi_v"], out["psi_a"], n_v, n, M_v, M_a)
     dstK, n_v2, n2 = compact(p, cacheK, chunkK, n_v, n, idx_v, idx_a, M_v, M_a)

@@ -61,6 +61,7 @@ StepParams make_params(const omnimem_ctx* c, int Nn_v, int Nn_a, const int32_t* 
   p.scale = c->scale;
   p.scale_log2e = (float)((double)c->scale * 1.4426950408889634);
   p.lambda = g.lambda;
+  p.shared_heads = g.select_scope == 1;
   p.n_v = n_v; p.n = n; p.skip_budget = skip_budget;
   return p;
 }
@@ -247,7 +248,7 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
   if (g.n_layers <= 0 || g.n_q_heads <= 0 || g.n_kv_heads <= 0 || g.cache_cap <= 0 || g.max_chunk_v < 0 ||
       g.max_chunk_a < 0 || g.n_q_heads % g.n_kv_heads != 0 || g.sim_stride_v < 1 || g.sim_stride_a < 1 ||
       g.softmax_scale < 0.f || g.lambda < 0.f || g.ratio_r <= 0.f || g.temperature <= 0.f || g.budget_min < 0 ||
-      g.budget_max < g.budget_min || (g.sim_source != 0 && g.sim_source != 1) || g.n_kv_heads > 65535)
+      g.budget_max < g.budget_min || (g.sim_source != 0 && g.sim_source != 1) || (g.select_scope != 0 && g.select_scope != 1) || g.n_kv_heads > 65535)
     return OMNIMEM_INVALID_ARG;
   if (g.dtype != OMNIMEM_FP32 && g.dtype != OMNIMEM_BF16) return OMNIMEM_UNSUPPORTED;
   if (g.head_dim != 64 && g.head_dim != 128) return OMNIMEM_UNSUPPORTED;

@@ -20,6 +20,7 @@ struct StepParams {
   float scale;               // c
   float scale_log2e;         // c * log2(e)
   float lambda;
+  int shared_heads;  // select_scope == 1: one score per token and layer (R29)
   // device state
   const int32_t* n_v;        // [L]
   const int32_t* n;          // [L]

@@ -147,9 +147,13 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams p, const float
       s = fminf(1.f, fmaxf(-1.f, s));
       const float a = (m == 0 ? a_v : a_a)[lh * cap + t];
       (m == 0 ? s_v : s_a)[lh * cap + t] = s;
-      (m == 0 ? psi_v : psi_a)[lh * cap + t] = powf(a, p.lambda) * (1.f - s);
+      if (!p.shared_heads) (m == 0 ? psi_v : psi_a)[lh * cap + t] = powf(a, p.lambda) * (1.f - s);
       A += a;
       ssum += s;
+    }
+    if (p.shared_heads) {  // R29: one score per token and layer, written to every head's row (identical index sets)
+      const float psi = powf(A, p.lambda) * (1.f - ssum / (float)p.Hkv);
+      for (int h = 0; h < p.Hkv; ++h) (m == 0 ? psi_v : psi_a)[((long long)l * p.Hkv + h) * cap + t] = psi;
     }
     v0 = (double)A;
     v1 = A > 0.f ? (double)A * log((double)A) : 0.0;

@@ -26,7 +26,7 @@ def dev_objs(x, wl):
     return Cache(d["cacheK"], d["cacheV"], d["n_v"], d["n"]), Chunk(d["chunkK"], d["chunkV"], d["Q"], wl.Nn_v, wl.Nn_a)
 
 
-def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=True, stats_tol=None):
+def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=True, stats_tol=None, select_scope=0):
     """All of rules (a), (b), (c) for one step of workload `wl` (L = number of layers in x)."""
     eng_kw, ref_kw = dict(eng_kw or {}), dict(ref_kw or {})
     x = x if x is not None else I.full_inputs(wl)
@@ -36,8 +36,8 @@ def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=Tr
     p = ref_params(wl, L, **ref_kw)
     B = np.full((L,), wl.budget, np.int32)
     orc = ref.compress_chunk(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"], B,
-                             sim_source=sim_source, want_rowH=check_rowH)
-    eng = engine_for(wl, sim_source=sim_source, **eng_kw)
+                             sim_source=sim_source, want_rowH=check_rowH, select_scope=select_scope)
+    eng = engine_for(wl, sim_source=sim_source, select_scope=select_scope, **eng_kw)
     src, chunk = dev_objs(x, wl)
     n_v, n = x["n_v"].numpy(), x["n"].numpy()
     Kv, Ka = seg_lens(wl, n_v, n)
@@ -375,4 +375,28 @@ def test_offline_calibration_and_ragged_layer_budgets():
         nl = int(orc["n_out"][l])
         assert np.array_equal(idx_v[l, :, :orc["M_v"][l]].cpu().numpy(), orc["idx_v"][l, :, :orc["M_v"][l]])
         assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][l, :, :nl])
+    eng.close()
+
+
+def test_shared_head_selection_paper_literal():
+    """select_scope = 1 (R29: the index sets carry no head index): one score per token and layer, identical
+    kept sets for every KV head; rules (a), (b), (c) as for the per-head mode."""
+    for wl in (I.CFG1, SMALL2, SMALL3.replace(Hq=8, Hkv=4)):
+        check_step(wl, select_scope=1)
+    from paper_2606_07577_b200.omnimem import OmniMem
+    wl = SMALL3.replace(Hq=8, Hkv=4)
+    x = I.full_inputs(wl)
+    eng = OmniMem.for_workload(wl, select_scope=1)
+    src, chunk = dev_objs(x, wl)
+    idx_v, idx_a = eng.new_indices()
+    M_v = torch.zeros(wl.L, dtype=torch.int32, device="cuda")
+    M_a = torch.zeros_like(M_v)
+    dst = eng.new_cache()
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device="cuda")
+    eng.compress_chunk(src, chunk, B, dst, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+    torch.cuda.synchronize()
+    for l in range(wl.L):
+        mv, ma = int(M_v[l]), int(M_a[l])
+        for h in range(1, wl.Hkv):
+            assert torch.equal(idx_v[l, h, :mv], idx_v[l, 0, :mv]) and torch.equal(idx_a[l, h, :ma], idx_a[l, 0, :ma])
     eng.close()

@@ -356,6 +356,41 @@ def test_layer_budgets_invariants():
     assert np.all(np.diff(b[np.argsort(C9)]) >= 0)            # monotone in compressibility
 
 
+def test_psi_shared_heads_paper_literal():
+    """R29: one score per token and layer.  Pins: Hkv = 1 reduces to Eq.8 per head; identical heads give
+    Hkv^lambda a^lambda (1 - s); permuting the heads changes nothing; every head's row carries the same score, so the
+    stable top-M of every head is the same set; against the formula written out with numpy."""
+    g = np.random.default_rng(4)
+    L, Hkv, cap_v, cap_a = 2, 3, 9, 5
+    p = ref.RefParams(L=L, Hq=Hkv, Hkv=Hkv, D=1, cache_cap=6, Nn_v=3, Nn_a=1, lam=0.3)
+    n_v, n = np.array([6, 4], np.int32), np.array([6, 6], np.int32)          # K_v = 9, 7 ; K_a = 1, 3
+    assert (p.seg_cap_v, p.seg_cap_a) == (cap_v, 7)
+    a_v, a_a = g.uniform(0.1, 3, (L, Hkv, p.seg_cap_v)), g.uniform(0.1, 3, (L, Hkv, p.seg_cap_a))
+    s_v, s_a = g.uniform(-0.5, 0.9, a_v.shape), g.uniform(-0.5, 0.9, a_a.shape)
+    pv, pa = ref.psi(p, n_v, n, a_v, a_a, s_v, s_a, select_scope=1)
+    want = (a_v.sum(1) ** 0.3 * (1 - s_v.mean(1))).astype(np.float32)
+    for l, Kv in enumerate((9, 7)):
+        for h in range(Hkv):
+            np.testing.assert_array_equal(pv[l, h, :Kv], want[l, :Kv])
+            assert np.all(pv[l, h, Kv:] == 0)
+    perm = [2, 0, 1]
+    pv2, pa2 = ref.psi(p, n_v, n, a_v[:, perm], a_a[:, perm], s_v[:, perm], s_a[:, perm], select_scope=1)
+    np.testing.assert_allclose(pv2, pv, rtol=1e-6)
+    np.testing.assert_allclose(pa2, pa, rtol=1e-6)
+    same = np.repeat(a_v[:, :1], Hkv, 1), np.repeat(a_a[:, :1], Hkv, 1), np.repeat(s_v[:, :1], Hkv, 1), np.repeat(s_a[:, :1], Hkv, 1)
+    ps, _ = ref.psi(p, n_v, n, *same, select_scope=1)
+    ph, _ = ref.psi(p, n_v, n, *same, select_scope=0)
+    np.testing.assert_allclose(ps[:, 0], ph[:, 0] * Hkv ** 0.3, rtol=1e-6)
+    p1 = ref.RefParams(L=L, Hq=1, Hkv=1, D=1, cache_cap=6, Nn_v=3, Nn_a=1, lam=0.3)
+    one = a_v[:, :1].copy(), a_a[:, :1].copy(), s_v[:, :1].copy(), s_a[:, :1].copy()
+    np.testing.assert_array_equal(ref.psi(p1, n_v, n, *one, select_scope=1)[0], ref.psi(p1, n_v, n, *one, select_scope=0)[0])
+    M_v, M_a = np.array([4, 3], np.int32), np.array([1, 2], np.int32)
+    iv, ia = ref.select(p, pv, pa, n_v, n, M_v, M_a)
+    for l in range(L):
+        for h in range(1, Hkv):
+            assert np.array_equal(iv[l, h, :M_v[l]], iv[l, 0, :M_v[l]]) and np.array_equal(ia[l, h, :M_a[l]], ia[l, 0, :M_a[l]])
+
+
 def test_calibration_means_then_eq14():
     """R28: budgets from the MEANS of the two layer measures over the calibration chunks.  Pins: one chunk ==
     plain Eq.14; chunks that are permutations of each other give the same table; closed form of the two-layer case
