@@ -73,12 +73,16 @@ typedef struct {
   float temperature;                       /* Eq.14 T; paper default 0.2                                     */
   int32_t budget_min, budget_max;          /* Eq.14 clamp [B_min, B_max]; 0,0 => no clamp                    */
   int32_t causal;                          /* 1 = causal inside the chunk (R3, default), 0 = every key visible       */
-  int32_t sim_source;                      /* Eq.7 vectors: 0 = value rows (default), 1 = key rows            */
+  int32_t sim_source;                      /* Eq.7 vectors: 0 = value rows (default), 1 = key rows,
+                                              2 = the layer's hidden states H (the paper's first form;
+                                              needs d_model > 0 and select_scope == 1, R30)                          */
   int32_t sim_stride_v, sim_stride_a;      /* neighbour distance of Eq.7 per modality; 1 = paper literal (R11)       */
   int32_t score_path;                      /* 0 = auto (tcgen05 for bf16 D=128, SIMT otherwise), 1 = force SIMT      */
   int32_t select_scope;                    /* 0 = one index set per (layer, KV head) (north_star, R5);
                                               1 = one index set per layer, the paper-literal reading of P:68-74 where
                                               I carries no head index (R29): psi = (sum_h a)^lambda (1 - mean_h s)         */
+  int32_t d_model;                         /* width of the retained hidden states (cache.h, chunk.h); 0 = none;
+                                              d_model * element size must be a multiple of 16 bytes                  */
 } omnimem_config;
 
 typedef struct {     /* one pooled KV cache */
@@ -86,6 +90,9 @@ typedef struct {     /* one pooled KV cache */
   void* v;           /* [L, Hkv, cache_cap, D] dtype                                          */
   int32_t* n_v;      /* [L] visual rows valid per layer                                       */
   int32_t* n;        /* [L] total rows valid per layer (visual + audio), n[l] <= cache_cap    */
+  void* h;           /* sim_source == 2 only, else NULL: [L, cache_cap, d_model] dtype, the retained hidden states
+                        H^(l) of the cached tokens, row r belongs to the token of K/V row r (one set of rows per
+                        layer: the kept set is the same for every head, select_scope == 1)          */
 } omnimem_cache;
 
 typedef struct {     /* one chunk, modality-blocked */
@@ -95,6 +102,7 @@ typedef struct {     /* one chunk, modality-blocked */
   const float* lse;  /* optional [L, Hq, Nn]: natural-log LSE of the scaled, masked logits of Eq.1 as produced by the
                         model's own attention forward; NULL => computed here (score pass 1)                        */
   int32_t Nn_v, Nn_a; /* HOST ints: rows of each modality in this chunk                       */
+  const void* h;     /* sim_source == 2 only, else NULL: [L, Nn, d_model] hidden states of the chunk's tokens */
 } omnimem_chunk;
 
 typedef struct {     /* outputs of the scoring stages; any pointer may be NULL except where noted */

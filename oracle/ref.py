@@ -15,6 +15,8 @@ import os
 import subprocess
 from dataclasses import dataclass
 
+import dataclasses
+
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -152,6 +154,23 @@ def redundancy(p: RefParams, cacheX, n_v, n, chunkX):
     return s_v, s_a
 
 
+def redundancy_hidden(p: RefParams, cacheH, n_v, n, chunkH):
+    """Eq.7 in the paper's first form: the vectors are the layer's hidden states H_k, one row per token and
+    layer (cacheH [L, cache_cap, d_model], chunkH [L, Nn, d_model]; reading R30).  The definition is the same adjacent
+    cosine as on value rows, with one "head" of width d_model, so the same plain routine is called on that shape; the
+    result [L, seg_cap_m] is the redundancy of the token in every KV head."""
+    p1 = dataclasses.replace(p, Hq=1, Hkv=1, D=int(cacheH.shape[-1]))
+    s_v, s_a = redundancy(p1, cacheH[:, None], n_v, n, chunkH[:, None])
+    return np.repeat(s_v, p.Hkv, axis=1), np.repeat(s_a, p.Hkv, axis=1)
+
+
+def compact_hidden(p: RefParams, cacheH, chunkH, n_v, n, idx_v, idx_a, M_v, M_a):
+    """The retained hidden states follow the kept tokens; the layer's index set is head 0's (select_scope = 1)."""
+    p1 = dataclasses.replace(p, Hq=1, Hkv=1, D=int(cacheH.shape[-1]))
+    dst, _, _ = compact(p1, cacheH[:, None], chunkH[:, None], n_v, n, i32(idx_v)[:, :1], i32(idx_a)[:, :1], M_v, M_a)
+    return dst[:, 0]
+
+
 # ---- O4 ----------------------------------------------------------------------------------------
 def psi(p: RefParams, n_v, n, a_v, a_a, s_v, s_a, select_scope: int = 0):
     """select_scope 0: Eq.8 per (layer, KV head); 1: once per layer, paper-literal index sets (R29)."""
@@ -249,14 +268,16 @@ def compact(p: RefParams, cacheX, chunkX, n_v, n, idx_v, idx_a, M_v, M_a):
 
 # ---- the whole step, in the paper's order ------------------------------------------------------------
 def score(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source: int = 0, want_rowH: bool = False,
-          select_scope: int = 0):
+          select_scope: int = 0, hidden=None):
     """Stages 1-3a: a, s, psi, statistics (Eq.6-10, 13).  Returns a dict of numpy arrays."""
     a_log, lse, rowH = attention(p, cacheK, n, chunkK, Q, want_rowH)
     a_v, a_a = split(p, a_log, n_v, n)
     if sim_source == 0:
         s_v, s_a = redundancy(p, cacheV, n_v, n, chunkV)
-    else:
+    elif sim_source == 1:
         s_v, s_a = redundancy(p, cacheK, n_v, n, chunkK)
+    else:
+        s_v, s_a = redundancy_hidden(p, hidden[0], n_v, n, hidden[1])
     psi_v, psi_a = psi(p, n_v, n, a_v, a_a, s_v, s_a, select_scope)
     st = stats(p, n_v, n, a_v, a_a, s_v, s_a)
     return dict(a_log=a_log, lse=lse, rowH=rowH, a_v=a_v, a_a=a_a, s_v=s_v, s_a=s_a, psi_v=psi_v, psi_a=psi_a,
@@ -264,12 +285,15 @@ def score(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source: i
 
 
 def compress_chunk(p: RefParams, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, layer_budget, sim_source: int = 0,
-                   want_rowH: bool = False, select_scope: int = 0):
-    """One full step: score -> allocate -> select -> compact.  `layer_budget` is an int array [L]."""
-    out = score(p, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source, want_rowH, select_scope)
+                   want_rowH: bool = False, select_scope: int = 0, hidden=None):
+    """One full step: score -> allocate -> select -> compact.  `layer_budget` is an int array [L].
+    hidden = (cacheH, chunkH) when sim_source == 2 (hidden-state redundancy, R30)."""
+    out = score(p, cacheK, cacheV, n_v, n, chunkK, chunkV, Q, sim_source, want_rowH, select_scope, hidden)
     M_v, M_a = allocate(p, out["stats"], n_v, n, layer_budget)
     idx_v, idx_a = select(p, out["psi_v"], out["psi_a"], n_v, n, M_v, M_a)
     dstK, n_v2, n2 = compact(p, cacheK, chunkK, n_v, n, idx_v, idx_a, M_v, M_a)
     dstV, _, _ = compact(p, cacheV, chunkV, n_v, n, idx_v, idx_a, M_v, M_a)
     out.update(M_v=M_v, M_a=M_a, idx_v=idx_v, idx_a=idx_a, dstK=dstK, dstV=dstV, n_v_out=n_v2, n_out=n2)
+    if hidden is not None:
+        out["dstH"] = compact_hidden(p, hidden[0], hidden[1], n_v, n, idx_v, idx_a, M_v, M_a)
     return out

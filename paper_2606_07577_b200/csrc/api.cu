@@ -62,6 +62,7 @@ StepParams make_params(const omnimem_ctx* c, int Nn_v, int Nn_a, const int32_t* 
   p.scale_log2e = (float)((double)c->scale * 1.4426950408889634);
   p.lambda = g.lambda;
   p.shared_heads = g.select_scope == 1;
+  p.d_model = g.sim_source == 2 ? g.d_model : 0;
   p.n_v = n_v; p.n = n; p.skip_budget = skip_budget;
   return p;
 }
@@ -75,6 +76,13 @@ int check_chunk(const omnimem_ctx* c, const omnimem_chunk* ch, bool need_q) {
 }
 int check_cache(const omnimem_cache* ca) {
   return (ca && ca->k && ca->v && ca->n_v && ca->n) ? OMNIMEM_OK : OMNIMEM_INVALID_ARG;
+}
+// sim_source == 2 (R30): the hidden-state buffers must be there
+int check_hidden(const omnimem_ctx* c, const omnimem_cache* ca, const omnimem_chunk* ch) {
+  if (c->cfg.sim_source != 2) return OMNIMEM_OK;
+  if (ca && !ca->h) return OMNIMEM_INVALID_ARG;
+  if (ch && ch->Nn_v + ch->Nn_a > 0 && !ch->h) return OMNIMEM_INVALID_ARG;
+  return OMNIMEM_OK;
 }
 
 struct StageTimer {
@@ -121,6 +129,7 @@ int run_score(omnimem_ctx* c, const StepParams& p, StepBuffers& b, cudaStream_t 
 void fill_buffers(const omnimem_ctx* c, const omnimem_cache* src, const omnimem_chunk* ch, const omnimem_scores* out,
                   uint8_t* ws, const WsLayout& w, StepBuffers& b) {
   b.cacheK = src->k; b.cacheV = src->v; b.chunkK = ch->k; b.chunkV = ch->v; b.Q = ch->q;
+  b.cacheH = src->h; b.chunkH = ch->h;
   b.lse_in = ch->lse;
   b.lse_out = out ? out->lse_out : nullptr;
   b.lse = ch->lse ? const_cast<float*>(ch->lse) : (b.lse_out ? b.lse_out : (float*)(ws + w.lse));
@@ -152,6 +161,8 @@ int check_fused_args(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_c
   if (rc) return rc;
   if (opt_out && (rc = check_scores(opt_out))) return rc;
   if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
+  if ((rc = check_hidden(ctx, src, chunk)) || (rc = check_hidden(ctx, dst, nullptr))) return rc;
+  if (ctx->cfg.sim_source == 2 && dst->h == src->h) return OMNIMEM_INVALID_ARG;
   if (ws_bytes < ws_layout(ctx).total) return OMNIMEM_WORKSPACE_TOO_SMALL;
   return OMNIMEM_OK;
 }
@@ -171,10 +182,11 @@ int compress_layers(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
   const size_t cache_b = lz * Hkv * g.cache_cap * D * es, kv_b = lz * Hkv * Nn * D * es, q_b = lz * Hq * Nn * D * es;
   const size_t segv_b = lz * Hkv * ctx->seg_cap_v * sizeof(float), sega_b = lz * Hkv * ctx->seg_cap_a * sizeof(float);
   const size_t row_b = lz * Hq * Nn * sizeof(float), idx_b = lz * Hkv * g.cache_cap * sizeof(int32_t);
-  omnimem_cache s2{adv(src->k, cache_b), adv(src->v, cache_b), src->n_v + l0, src->n + l0};
-  omnimem_cache d2{adv(dst->k, cache_b), adv(dst->v, cache_b), dst->n_v + l0, dst->n + l0};
+  const size_t hc_b = lz * g.cache_cap * (size_t)g.d_model * es, hn_b = lz * Nn * (size_t)g.d_model * es;
+  omnimem_cache s2{adv(src->k, cache_b), adv(src->v, cache_b), src->n_v + l0, src->n + l0, adv(src->h, hc_b)};
+  omnimem_cache d2{adv(dst->k, cache_b), adv(dst->v, cache_b), dst->n_v + l0, dst->n + l0, adv(dst->h, hc_b)};
   omnimem_chunk c2 = *chunk;
-  c2.k = adv(chunk->k, kv_b); c2.v = adv(chunk->v, kv_b); c2.q = adv(chunk->q, q_b);
+  c2.k = adv(chunk->k, kv_b); c2.v = adv(chunk->v, kv_b); c2.q = adv(chunk->q, q_b); c2.h = adv(chunk->h, hn_b);
   c2.lse = (const float*)adv(chunk->lse, row_b);
   omnimem_scores o2{};
   if (opt_out) {
@@ -221,6 +233,8 @@ int compress_layers(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
     StageTimer t(ctx, st, OMNIMEM_STAGE_COMPACT);
     e = launch_compact(ctx, p, s2.k, s2.v, c2.k, c2.v, idx_v, idx_a, M_v, M_a, d2.k, d2.v, d2.n_v, d2.n, st,
                        &ctx->launches);
+    if (e == cudaSuccess && p.d_model > 0)
+      e = launch_compact_hidden(ctx, p, s2.h, c2.h, idx_v, idx_a, M_v, M_a, d2.h, st, &ctx->launches);
     if (e != cudaSuccess) return fail_cuda(ctx, e);
   }
   return OMNIMEM_OK;
@@ -248,7 +262,8 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
   if (g.n_layers <= 0 || g.n_q_heads <= 0 || g.n_kv_heads <= 0 || g.cache_cap <= 0 || g.max_chunk_v < 0 ||
       g.max_chunk_a < 0 || g.n_q_heads % g.n_kv_heads != 0 || g.sim_stride_v < 1 || g.sim_stride_a < 1 ||
       g.softmax_scale < 0.f || g.lambda < 0.f || g.ratio_r <= 0.f || g.temperature <= 0.f || g.budget_min < 0 ||
-      g.budget_max < g.budget_min || (g.sim_source != 0 && g.sim_source != 1) || (g.select_scope != 0 && g.select_scope != 1) || g.n_kv_heads > 65535)
+      g.budget_max < g.budget_min || g.sim_source < 0 || g.sim_source > 2 || (g.select_scope != 0 && g.select_scope != 1) || g.d_model < 0 ||
+      (g.sim_source == 2 && (g.d_model == 0 || g.select_scope != 1 || (g.d_model * (g.dtype == OMNIMEM_FP32 ? 4 : 2)) % 16 != 0)) || g.n_kv_heads > 65535)
     return OMNIMEM_INVALID_ARG;
   if (g.dtype != OMNIMEM_FP32 && g.dtype != OMNIMEM_BF16) return OMNIMEM_UNSUPPORTED;
   if (g.head_dim != 64 && g.head_dim != 128) return OMNIMEM_UNSUPPORTED;
@@ -339,6 +354,8 @@ int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chun
   if (rc) return rc;
   rc = check_scores(out);
   if (rc) return rc;
+  rc = check_hidden(ctx, src, chunk);
+  if (rc) return rc;
   const WsLayout w = ws_layout(ctx);
   if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
   begin_call(ctx);
@@ -405,11 +422,14 @@ int omnimem_compact(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
   rc = check_chunk(ctx, chunk, false);
   if (rc) return rc;
   if (dst->k == src->k || dst->v == src->v || dst->n == src->n || dst->n_v == src->n_v) return OMNIMEM_INVALID_ARG;
+  if ((rc = check_hidden(ctx, src, chunk)) || (rc = check_hidden(ctx, dst, nullptr))) return rc;
   begin_call(ctx);
   StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
   StageTimer t(ctx, (cudaStream_t)stream, OMNIMEM_STAGE_COMPACT);
   cudaError_t e = launch_compact(ctx, p, src->k, src->v, chunk->k, chunk->v, idx_v, idx_a, M_v, M_a, dst->k, dst->v,
                                  dst->n_v, dst->n, (cudaStream_t)stream, &ctx->launches);
+  if (e == cudaSuccess && p.d_model > 0)   // the retained hidden states follow the kept tokens (R30)
+    e = launch_compact_hidden(ctx, p, src->h, chunk->h, idx_v, idx_a, M_v, M_a, dst->h, (cudaStream_t)stream, &ctx->launches);
   return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
 }
 
@@ -432,6 +452,7 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   int rc = check_chunk(ctx, host_chunk, true);
   if (rc) return rc;
   if (!dev_chunk->k || !dev_chunk->v || !dev_chunk->q || (host_chunk->lse && !dev_chunk->lse)) return OMNIMEM_INVALID_ARG;
+  if (ctx->cfg.sim_source == 2 && (!host_chunk->h || !dev_chunk->h)) return OMNIMEM_INVALID_ARG;
   omnimem_chunk ch = *dev_chunk;
   ch.Nn_v = host_chunk->Nn_v;
   ch.Nn_a = host_chunk->Nn_a;
@@ -447,6 +468,7 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   const size_t kv_layer = (size_t)g.n_kv_heads * Nn * g.head_dim * es;      // bytes per layer
   const size_t q_layer = (size_t)g.n_q_heads * Nn * g.head_dim * es;
   const size_t lse_layer = host_chunk->lse ? (size_t)g.n_q_heads * Nn * sizeof(float) : 0;
+  const size_t h_layer = g.sim_source == 2 ? Nn * (size_t)g.d_model * es : 0;
   uint8_t* wsb = (uint8_t*)ws;
   begin_call(ctx);
   // Layers are independent through the whole step, so the chunk is copied and compressed in groups of layers: the
@@ -468,6 +490,8 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
         e = cudaMemcpyAsync(at(dev_chunk->lse, l0 * lse_layer), at(host_chunk->lse, l0 * lse_layer), Lg * lse_layer, cudaMemcpyHostToDevice, cs);
       if (e == cudaSuccess)
         e = cudaMemcpyAsync(at(dev_chunk->v, l0 * kv_layer), at(host_chunk->v, l0 * kv_layer), Lg * kv_layer, cudaMemcpyHostToDevice, cs);
+      if (e == cudaSuccess && h_layer)
+        e = cudaMemcpyAsync(at(dev_chunk->h, l0 * h_layer), at(host_chunk->h, l0 * h_layer), Lg * h_layer, cudaMemcpyHostToDevice, cs);
       if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[gi], cs);
       if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_copy[gi], 0);
       if (e != cudaSuccess) return fail_cuda(ctx, e);
@@ -480,7 +504,7 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   if (e == cudaSuccess) e = cudaMemcpyAsync(host_M_a, wsb + w.M_a, mb, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) return fail_cuda(ctx, e);
-  if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? (size_t)L * (2 * kv_layer + q_layer + lse_layer) : 0);
+  if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? (size_t)L * (2 * kv_layer + q_layer + lse_layer + h_layer) : 0);
   if (d2h_bytes) *d2h_bytes = (int64_t)(2 * mb);
   return OMNIMEM_OK;
 }

@@ -21,6 +21,7 @@ struct StepParams {
   float scale_log2e;         // c * log2(e)
   float lambda;
   int shared_heads;  // select_scope == 1: one score per token and layer (R29)
+  int d_model;       // width of the hidden-state rows (sim_source == 2), else 0
   // device state
   const int32_t* n_v;        // [L]
   const int32_t* n;          // [L]
@@ -55,6 +56,7 @@ __device__ __forceinline__ bool layer_skips_scoring(const StepParams& p, int l) 
 // Buffers of one step (device pointers).
 struct StepBuffers {
   const void *cacheK, *cacheV, *chunkK, *chunkV, *Q;
+  const void *cacheH, *chunkH;  // hidden states (sim_source == 2) or nullptr
   const float* lse_in;   // caller-supplied natural-log LSE [L,Hq,Nn] or nullptr
   float* lse;            // SIMT path: natural-log LSE read by pass 2 (== lse_in when supplied)
   float* lse2;           // tcgen05 path: internal log2-domain LSE, rows padded to a multiple of 128
@@ -103,6 +105,9 @@ cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const S
 cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,
                             int64_t total_budget, int32_t* M_v, int32_t* M_a, int32_t* layer_budget_out, cudaStream_t st,
                             int* launches);
+cudaError_t launch_compact_hidden(const omnimem_ctx* ctx, const StepParams& p, const void* srcH, const void* chunkH,
+                                  const int32_t* idx_v, const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a,
+                                  void* dstH, cudaStream_t st, int* launches);
 cudaError_t launch_calib_accumulate(int L, const double* stats, double* acc, cudaStream_t st, int* launches);
 cudaError_t launch_calib_mean(int L, const double* acc, double* mean, cudaStream_t st, int* launches);
 cudaError_t launch_select(const omnimem_ctx* ctx, const StepParams& p, const float* psi_v, const float* psi_a,

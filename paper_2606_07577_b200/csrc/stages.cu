@@ -96,11 +96,67 @@ __global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __re
   }
 }
 
+// Eq.7 in the paper's first form: the vectors are the layer's hidden states H_k, one row of d_model elements
+// per token and layer ([L, cache_cap, d_model] / [L, Nn, d_model]; R30).  One warp per item streams row t and row
+// t + sigma in 512-byte steps (4 steps in flight), so the sweep is one pass over H at HBM speed; the cosine is written
+// to every KV head's slot of cosn, finalize then runs unchanged.
+template <typename T>
+__global__ void __launch_bounds__(256) cosine_hidden_kernel(StepParams p, const T* __restrict__ cacheH,
+                                                            const T* __restrict__ chunkH, float* __restrict__ cosn) {
+  const int items = p.seg_cap_v + p.seg_cap_a;
+  const int l = blockIdx.y;
+  if (layer_skips_scoring(p, l)) return;
+  const int lane = threadIdx.x & 31;
+  const int it = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (it >= items) return;
+  const int n_v = p.n_v[l], n = p.n[l];
+  const int m = it < p.seg_cap_v ? 0 : 1;
+  const int t = m == 0 ? it : it - p.seg_cap_v;
+  const int sg = m == 0 ? p.stride_v : p.stride_a;
+  if (t + sg >= seg_len(p, n_v, n, m)) return;
+  bool cx, cy;
+  const int rx = seg_row(p, n_v, n, m, t, cx), ry = seg_row(p, n_v, n, m, t + sg, cy);
+  const int row_vecs = p.d_model * (int)sizeof(T) / 16;
+  const uint4* x = reinterpret_cast<const uint4*>(cx ? chunkH + ((long long)l * p.Nn + rx) * p.d_model
+                                                     : cacheH + ((long long)l * p.cache_cap + rx) * p.d_model);
+  const uint4* y = reinterpret_cast<const uint4*>(cy ? chunkH + ((long long)l * p.Nn + ry) * p.d_model
+                                                     : cacheH + ((long long)l * p.cache_cap + ry) * p.d_model);
+  float dot = 0.f, nx = 0.f, ny = 0.f;
+  constexpr int kU = 4;
+  for (int v0 = lane; v0 < row_vecs; v0 += 32 * kU) {
+    uint4 xv[kU], yv[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u)
+      if (v0 + 32 * u < row_vecs) { xv[u] = __ldg(x + v0 + 32 * u); yv[u] = __ldg(y + v0 + 32 * u); }
+#pragma unroll
+    for (int u = 0; u < kU; ++u)
+      if (v0 + 32 * u < row_vecs) Vec16<T>::acc(xv[u], yv[u], dot, nx, ny);
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    nx += __shfl_xor_sync(0xffffffffu, nx, o);
+    ny += __shfl_xor_sync(0xffffffffu, ny, o);
+  }
+  const float c = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
+  for (int h = lane; h < p.Hkv; h += 32) cosn[((long long)l * p.Hkv + h) * items + it] = c;
+}
+
 cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
                           int* launches) {
+  const int items = p.seg_cap_v + p.seg_cap_a;
+  if (ctx->cfg.sim_source == 2) {
+    const dim3 grid((unsigned)((items + 7) / 8), (unsigned)p.L);
+    ++*launches;
+    if (ctx->cfg.dtype == OMNIMEM_FP32)
+      cosine_hidden_kernel<float><<<grid, 256, 0, st>>>(p, (const float*)b.cacheH, (const float*)b.chunkH, b.cosn);
+    else
+      cosine_hidden_kernel<__nv_bfloat16><<<grid, 256, 0, st>>>(p, (const __nv_bfloat16*)b.cacheH,
+                                                                 (const __nv_bfloat16*)b.chunkH, b.cosn);
+    return cudaGetLastError();
+  }
   const void* cx = ctx->cfg.sim_source == 0 ? b.cacheV : b.cacheK;
   const void* kx = ctx->cfg.sim_source == 0 ? b.chunkV : b.chunkK;
-  const int items = p.seg_cap_v + p.seg_cap_a;
   const int row_bytes = p.D * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2);
   const int vec = row_bytes / 64;                      // 16-byte vectors per thread (4 threads per row): 2, 4 or 8
   const int unroll = vec == 8 ? 1 : 2;
@@ -544,6 +600,46 @@ cudaError_t launch_compact(const omnimem_ctx* ctx, const StepParams& p, const vo
                                                 (uint4*)dstV, dst_n_v, dst_n)
   if (tpr == 8) OMNIMEM_CP(8); else if (tpr == 16) OMNIMEM_CP(16); else OMNIMEM_CP(32);
 #undef OMNIMEM_CP
+  return cudaGetLastError();
+}
+
+// The retained hidden states follow the kept tokens: dstH[l, j] = row of the j-th kept index of the layer
+// (select_scope == 1: every head keeps the same rows, head 0's index list is read).  One warp per row, 512-byte steps.
+__global__ void __launch_bounds__(256) compact_hidden_kernel(StepParams p, const uint4* __restrict__ srcH,
+                                                             const uint4* __restrict__ chunkH,
+                                                             const int32_t* __restrict__ idx_v,
+                                                             const int32_t* __restrict__ idx_a,
+                                                             const int32_t* __restrict__ M_v,
+                                                             const int32_t* __restrict__ M_a, uint4* __restrict__ dstH,
+                                                             int row_vecs) {
+  const int l = blockIdx.y, lane = threadIdx.x & 31;
+  const int j = blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int Mv = M_v[l], total = Mv + M_a[l];
+  if (j >= total) return;
+  const int m = j < Mv ? 0 : 1;
+  const long long lh0 = (long long)l * p.Hkv;  // head 0 of the layer
+  const int t = m == 0 ? idx_v[lh0 * p.cache_cap + j] : idx_a[lh0 * p.cache_cap + (j - Mv)];
+  bool in_chunk;
+  const int row = seg_row(p, p.n_v[l], p.n[l], m, t, in_chunk);
+  const uint4* src = in_chunk ? chunkH + ((long long)l * p.Nn + row) * row_vecs : srcH + ((long long)l * p.cache_cap + row) * row_vecs;
+  uint4* dst = dstH + ((long long)l * p.cache_cap + j) * row_vecs;
+  for (int v0 = lane; v0 < row_vecs; v0 += 128) {
+    uint4 r[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (v0 + 32 * u < row_vecs) r[u] = __ldg(src + v0 + 32 * u);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (v0 + 32 * u < row_vecs) dst[v0 + 32 * u] = r[u];
+  }
+}
+
+cudaError_t launch_compact_hidden(const omnimem_ctx* ctx, const StepParams& p, const void* srcH, const void* chunkH,
+                                  const int32_t* idx_v, const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a,
+                                  void* dstH, cudaStream_t st, int* launches) {
+  const int row_vecs = p.d_model * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2) / 16;
+  const dim3 grid((unsigned)((p.cache_cap + 7) / 8), (unsigned)p.L);
+  ++*launches;
+  compact_hidden_kernel<<<grid, 256, 0, st>>>(p, (const uint4*)srcH, (const uint4*)chunkH, idx_v, idx_a, M_v, M_a,
+                                              (uint4*)dstH, row_vecs);
   return cudaGetLastError();
 }
 

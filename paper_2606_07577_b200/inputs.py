@@ -201,6 +201,34 @@ def full_inputs(wl: Workload, step: int = 0, layers=None, with_cache: bool = Tru
     return out
 
 
+def hidden_inputs(wl: Workload, d_model: int, step: int = 0, with_cache: bool = True) -> dict:
+    """Synthetic hidden states for the hidden-state form of Eq.7 (NEXT-3): cacheH [L, cache_cap, d_model]
+    (zero-padded) and chunkH [L, Nn, d_model] in the config dtype.  Generator tid 6.  Visual rows: AR(1) across frames
+    of `wl.frame` tokens with the config's rho ("ar1" recipe), or a 16-centre mixture ("mixture"); audio rows i.i.d.
+    N(0, audio_std^2).  One row per token and layer (hidden states have no head index)."""
+    n_v, n_a = (wl.n_v, wl.n_a) if with_cache else (0, 0)
+    dt = wl.torch_dtype
+    cacheH = torch.zeros(wl.L, wl.cache_cap, d_model, dtype=dt)
+    chunkH = torch.zeros(wl.L, wl.Nn, d_model, dtype=dt)
+    for l in range(wl.L):
+        g = _gen(wl, step, l, 6)
+        if wl.recipe == "ar1":
+            cache_frames = -(-n_v // wl.frame) if n_v else 0
+            chunk_frames = -(-wl.Nn_v // wl.frame)
+            lead = cache_frames * wl.frame - n_v
+            x = _ar1_frames(g, 1, cache_frames + chunk_frames, wl.frame, d_model, wl.rho)[0]
+            vis_c, vis_n = x[lead:lead + n_v], x[cache_frames * wl.frame: cache_frames * wl.frame + wl.Nn_v]
+        else:
+            mu = _randn(_gen(wl, 0, l, 7), N_VISUAL_CENTRES, d_model)
+            c = torch.randint(0, N_VISUAL_CENTRES, (n_v + wl.Nn_v,), generator=g)
+            x = 0.7 * mu[c] + 0.7 * _randn(g, n_v + wl.Nn_v, d_model)
+            vis_c, vis_n = x[:n_v], x[n_v:]
+        aud = wl.audio_std * _randn(g, n_a + wl.Nn_a, d_model)
+        cacheH[l, :n_v], cacheH[l, n_v:n_v + n_a] = vis_c.to(dt), aud[:n_a].to(dt)
+        chunkH[l, :wl.Nn_v], chunkH[l, wl.Nn_v:] = vis_n.to(dt), aud[n_a:].to(dt)
+    return dict(cacheH=cacheH, chunkH=chunkH)
+
+
 def small(wl: Workload, **kw) -> Workload:
     """A reduced copy of a config (same recipe and value structure) for tests the oracle finishes in seconds."""
     return wl.replace(**kw)

@@ -35,16 +35,16 @@ class omnimem_config(C.Structure):
                 ("softmax_scale", C.c_float), ("lam", C.c_float), ("ratio_r", C.c_float), ("temperature", C.c_float),
                 ("budget_min", C.c_int32), ("budget_max", C.c_int32), ("causal", C.c_int32), ("sim_source", C.c_int32),
                 ("sim_stride_v", C.c_int32), ("sim_stride_a", C.c_int32), ("score_path", C.c_int32),
-                ("select_scope", C.c_int32)]
+                ("select_scope", C.c_int32), ("d_model", C.c_int32)]
 
 
 class omnimem_cache(C.Structure):
-    _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("n_v", C.c_void_p), ("n", C.c_void_p)]
+    _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("n_v", C.c_void_p), ("n", C.c_void_p), ("h", C.c_void_p)]
 
 
 class omnimem_chunk(C.Structure):
     _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("q", C.c_void_p), ("lse", C.c_void_p),
-                ("Nn_v", C.c_int32), ("Nn_a", C.c_int32)]
+                ("Nn_v", C.c_int32), ("Nn_a", C.c_int32), ("h", C.c_void_p)]
 
 
 class omnimem_scores(C.Structure):
@@ -110,9 +110,11 @@ class Cache:
     v: torch.Tensor
     n_v: torch.Tensor
     n: torch.Tensor
+    h: Optional[torch.Tensor] = None     # [L, cache_cap, d_model] retained hidden states (sim_source == 2)
 
     def c(self) -> omnimem_cache:
-        return omnimem_cache(self.k.data_ptr(), self.v.data_ptr(), self.n_v.data_ptr(), self.n.data_ptr())
+        return omnimem_cache(self.k.data_ptr(), self.v.data_ptr(), self.n_v.data_ptr(), self.n.data_ptr(),
+                             None if self.h is None else self.h.data_ptr())
 
 
 @dataclass
@@ -124,10 +126,12 @@ class Chunk:
     Nn_v: int
     Nn_a: int
     lse: Optional[torch.Tensor] = None
+    h: Optional[torch.Tensor] = None     # [L, Nn, d_model] hidden states of the chunk's tokens (sim_source == 2)
 
     def c(self) -> omnimem_chunk:
         return omnimem_chunk(self.k.data_ptr(), self.v.data_ptr(), self.q.data_ptr(),
-                             None if self.lse is None else self.lse.data_ptr(), self.Nn_v, self.Nn_a)
+                             None if self.lse is None else self.lse.data_ptr(), self.Nn_v, self.Nn_a,
+                             None if self.h is None else self.h.data_ptr())
 
 
 @dataclass
@@ -155,17 +159,18 @@ class OmniMem:
     def __init__(self, L: int, Hq: int, Hkv: int, D: int, dtype: str, cache_cap: int, max_chunk_v: int, max_chunk_a: int,
                  lam: float = 0.02, ratio_r: float = 5.0, temperature: float = 0.2, softmax_scale: float = 0.0,
                  budget_min: int = 0, budget_max: int = 0, causal: int = 1, sim_source: int = 0, sim_stride_v: int = 1,
-                 sim_stride_a: int = 1, score_path: int = 0, select_scope: int = 0, device: str = "cuda:0"):
+                 sim_stride_a: int = 1, score_path: int = 0, select_scope: int = 0, d_model: int = 0, device: str = "cuda:0"):
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise OmniMemError("no CUDA device: the OmniMem path has no CPU fallback")
         self.device = torch.device(device)
         self.L, self.Hq, self.Hkv, self.D = L, Hq, Hkv, D
         self.cache_cap, self.max_chunk_v, self.max_chunk_a = cache_cap, max_chunk_v, max_chunk_a
+        self.d_model, self.sim_source = d_model, sim_source
         self.torch_dtype = torch.float32 if dtype == "fp32" else torch.bfloat16
         self.cfg = omnimem_config(L, Hq, Hkv, D, OMNIMEM_FP32 if dtype == "fp32" else OMNIMEM_BF16, cache_cap, max_chunk_v,
                                   max_chunk_a, softmax_scale, lam, ratio_r, temperature, budget_min, budget_max, causal,
-                                  sim_source, sim_stride_v, sim_stride_a, score_path, select_scope)
+                                  sim_source, sim_stride_v, sim_stride_a, score_path, select_scope, d_model)
         self.ctx = C.c_void_p()
         with torch.cuda.device(self.device):
             self._check(self.lib.omnimem_create(C.byref(self.cfg), C.byref(self.ctx)), "omnimem_create")
@@ -204,7 +209,8 @@ class OmniMem:
         z = lambda *s, dt: torch.zeros(*s, dtype=dt, device=self.device)
         return Cache(z(self.L, self.Hkv, self.cache_cap, self.D, dt=self.torch_dtype),
                      z(self.L, self.Hkv, self.cache_cap, self.D, dt=self.torch_dtype),
-                     z(self.L, dt=torch.int32), z(self.L, dt=torch.int32))
+                     z(self.L, dt=torch.int32), z(self.L, dt=torch.int32),
+                     z(self.L, self.cache_cap, self.d_model, dt=self.torch_dtype) if self.sim_source == 2 else None)
 
     def new_scores(self, Nn: int, want_lse: bool = False, want_row_entropy: bool = False) -> Scores:
         f = lambda *s: torch.zeros(*s, dtype=torch.float32, device=self.device)

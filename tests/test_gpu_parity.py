@@ -400,3 +400,62 @@ def test_shared_head_selection_paper_literal():
         for h in range(1, wl.Hkv):
             assert torch.equal(idx_v[l, h, :mv], idx_v[l, 0, :mv]) and torch.equal(idx_a[l, h, :ma], idx_a[l, 0, :ma])
     eng.close()
+
+
+def test_hidden_state_redundancy_variant():
+    """NEXT-3 (R30): Eq.7 on the layer's hidden states (width d_model, one row per token and layer), the
+    retained hidden states compacted with the kept tokens.  Needs select_scope = 1.  Rules (a)/(c) on the fused step,
+    byte-exact K/V/H rows, and a second free-running step on the compacted state."""
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem, OmniMemError
+    for wl, d_model in ((I.CFG1, 96), (SMALL3.replace(Hq=8, Hkv=4), 328)):       # 328 * 2 B = 656 B: ragged 512-byte steps
+        tol = TOL[wl.dtype]
+        L = wl.L
+        p = ref_params(wl, L)
+        eng = OmniMem.for_workload(wl, select_scope=1, sim_source=2, d_model=d_model)
+        B = np.full((L,), wl.budget, np.int32)
+        x, hx = I.full_inputs(wl), I.hidden_inputs(wl, d_model)
+        rK, rV, rH, r_nv, r_n = x["cacheK"], x["cacheV"], hx["cacheH"], x["n_v"].numpy(), x["n"].numpy()
+        src = Cache(rK.cuda(), rV.cuda(), x["n_v"].cuda(), x["n"].cuda(), h=rH.cuda())
+        dst = eng.new_cache()
+        for step in range(2):
+            if step:
+                x, hx = I.full_inputs(wl, step=step, with_cache=False), I.hidden_inputs(wl, d_model, step=step, with_cache=False)
+            orc = ref.compress_chunk(p, rK, rV, r_nv, r_n, x["chunkK"], x["chunkV"], x["Q"], B, sim_source=2,
+                                     select_scope=1, hidden=(rH, hx["chunkH"]))
+            chunk = Chunk(x["chunkK"].cuda(), x["chunkV"].cuda(), x["Q"].cuda(), wl.Nn_v, wl.Nn_a, h=hx["chunkH"].cuda())
+            sc = eng.new_scores(wl.Nn, want_lse=True)
+            idx_v, idx_a = eng.new_indices()
+            M_v = torch.zeros(L, dtype=torch.int32, device="cuda")
+            M_a = torch.zeros_like(M_v)
+            eng.compress_chunk(src, chunk, torch.from_numpy(B).cuda(), dst, out=sc, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+            torch.cuda.synchronize()
+            compare_scores(wl, r_nv, r_n, scores_to_numpy(sc), orc, tol)
+            assert np.array_equal(M_v.cpu().numpy(), orc["M_v"])
+            Kv, Ka = seg_lens(wl, r_nv, r_n)
+            n_diff = 0
+            for l in range(L):
+                n_diff += kept_sets_rule_c(f"v[{l}]", idx_v[l, 0].cpu().numpy(), orc["idx_v"][l, 0], int(orc["M_v"][l]),
+                                           orc["psi_v"][l, 0, :Kv[l]], tol)
+                n_diff += kept_sets_rule_c(f"a[{l}]", idx_a[l, 0].cpu().numpy(), orc["idx_a"][l, 0], int(orc["M_a"][l]),
+                                           orc["psi_a"][l, 0, :Ka[l]], tol)
+            assert n_diff == 0, "these sizes are expected to agree exactly"
+            for l in range(L):
+                nl = int(orc["n_out"][l])
+                assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][l, :, :nl])
+                assert np.array_equal(dst.h[l, :nl].cpu().view(torch.uint8).numpy(), orc["dstH"][l, :nl]), f"hidden rows, layer {l}"
+            # carry the ORACLE's state into the next step on both sides (byte-identical to the GPU's, just asserted)
+            dt = wl.torch_dtype
+            rK = torch.from_numpy(orc["dstK"].copy()).view(dt).reshape(x["chunkK"].shape[0], wl.Hkv, wl.cache_cap, wl.D)
+            rV = torch.from_numpy(orc["dstV"].copy()).view(dt).reshape(rK.shape)
+            rH = torch.from_numpy(orc["dstH"].copy()).view(dt).reshape(L, wl.cache_cap, d_model)
+            r_nv, r_n = orc["n_v_out"], orc["n_out"]
+            src, dst = dst, src
+        eng.close()
+    with pytest.raises(OmniMemError):                          # hidden states have no head index: per-head sets are refused
+        OmniMem.for_workload(I.CFG1, select_scope=0, sim_source=2, d_model=96)
+    eng = OmniMem.for_workload(I.CFG1, select_scope=1, sim_source=2, d_model=96)
+    x = I.full_inputs(I.CFG1)
+    src, chunk = dev_objs(x, I.CFG1)
+    with pytest.raises(OmniMemError, match="invalid"):
+        eng.score(src, chunk)                                  # cache.h / chunk.h missing
+    eng.close()

@@ -391,6 +391,41 @@ def test_psi_shared_heads_paper_literal():
             assert np.array_equal(iv[l, h, :M_v[l]], iv[l, 0, :M_v[l]]) and np.array_equal(ia[l, h, :M_a[l]], ia[l, 0, :M_a[l]])
 
 
+def test_redundancy_hidden_states():
+    """R30: Eq.7 on hidden states.  Pins: against torch cosine_similarity on the rows; the same value in
+    every KV head; duplicate neighbours => 1; the compaction of H picks exactly the kept rows (numpy take)."""
+    g = torch.Generator().manual_seed(3)
+    L, cap, d = 2, 10, 24
+    p = ref.RefParams(L=L, Hq=4, Hkv=2, D=8, cache_cap=cap, Nn_v=4, Nn_a=2)
+    n_v, n = np.array([5, 3], np.int32), np.array([8, 6], np.int32)
+    cacheH, chunkH = torch.randn(L, cap, d, generator=g, dtype=torch.float64), torch.randn(L, 6, d, generator=g, dtype=torch.float64)
+    chunkH[0, 1] = chunkH[0, 0]                                  # duplicate neighbours
+    s_v, s_a = ref.redundancy_hidden(p, cacheH, n_v, n, chunkH)
+    assert s_v.shape == (L, 2, p.seg_cap_v) and np.array_equal(s_v[:, 0], s_v[:, 1]) and np.array_equal(s_a[:, 0], s_a[:, 1])
+    cos = torch.nn.functional.cosine_similarity
+    for l in range(L):
+        vis = torch.cat([cacheH[l, :n_v[l]], chunkH[l, :4]])
+        aud = torch.cat([cacheH[l, n_v[l]:n[l]], chunkH[l, 4:]])
+        for seq, s in ((vis, s_v[l, 0]), (aud, s_a[l, 0])):
+            c = cos(seq[:-1], seq[1:], dim=-1).numpy()
+            want = np.empty(len(seq))
+            want[0], want[-1] = c[0], c[-1]
+            want[1:-1] = 0.5 * (c[:-1] + c[1:])
+            np.testing.assert_allclose(s[:len(seq)], want, atol=1e-12)
+    Kv0 = n_v[0] + 4
+    assert abs(s_v[0, 0, n_v[0]] - 0.5 * (1.0 + cos(cacheH[0, n_v[0] - 1], chunkH[0, 0], dim=0).item())) < 1e-12 and Kv0 == 9
+    idx_v = np.full((L, 2, cap), -1, np.int32)
+    idx_a = np.full((L, 2, cap), -1, np.int32)
+    idx_v[0, :, :3], idx_v[1, :, :2] = [0, 5, 8], [2, 6]
+    idx_a[0, :, :2], idx_a[1, :, :1] = [1, 3], [4]
+    M_v, M_a = np.array([3, 2], np.int32), np.array([2, 1], np.int32)
+    dst = ref.compact_hidden(p, cacheH, chunkH, n_v, n, idx_v, idx_a, M_v, M_a).view(np.float64).reshape(L, cap, d)
+    vis0 = np.concatenate([cacheH[0, :5].numpy(), chunkH[0, :4].numpy()])
+    aud0 = np.concatenate([cacheH[0, 5:8].numpy(), chunkH[0, 4:].numpy()])
+    np.testing.assert_array_equal(dst[0, :3], vis0[[0, 5, 8]])
+    np.testing.assert_array_equal(dst[0, 3:5], aud0[[1, 3]])
+
+
 def test_calibration_means_then_eq14():
     """R28: budgets from the MEANS of the two layer measures over the calibration chunks.  Pins: one chunk ==
     plain Eq.14; chunks that are permutations of each other give the same table; closed form of the two-layer case
