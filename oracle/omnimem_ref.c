@@ -53,13 +53,17 @@ typedef struct {
   double temperature;       /* Eq.14 T (default 0.2 P:159)                           */
   int64_t budget_min;       /* Eq.14 clamp [B_min, B_max]; 0,0 = no clamp           */
   int64_t budget_max;
+  const int32_t* chunk_modality; /* R25': NULL = modality-blocked chunk (visual block then audio block); else
+                                    [Nn] with 0 = visual, 1 = audio for each chunk row in TRUE temporal order
+                                    (time-interleaved chunk, "a specific number of audio and visual tokens") */
 } omnimem_ref_params;
 
 #define IDX3(a, b, c, B, C) ((((int64_t)(a)) * (B) + (b)) * (int64_t)(C) + (c))
 
 /* ---- O1: logical sequences (Eq.2-3) ------------------------------------------
  * Key order seen by attention (R2: ONE joint softmax): cached visual, cached audio,
- * new visual, new audio.  Row k of that sequence for (l,h): */
+ * then the chunk's rows in storage order (new visual, new audio when blocked; true temporal
+ * order when chunk_modality is given; the causal mask of R3 follows that order).  Row k: */
 static const double* key_row(const omnimem_ref_params* p, const double* cacheX, const double* chunkX,
                              int l, int h, int Nc, int k) {
   const int Nn = p->Nn_v + p->Nn_a;
@@ -70,9 +74,14 @@ static const double* key_row(const omnimem_ref_params* p, const double* cacheX, 
 /* Per-modality appended sequence K~_m = [cache_m ; chunk_m] (Eq.3).  Segment-local index t of
  * modality m (0 = visual, 1 = audio) -> index in the logical sequence above. */
 static int seg_to_logical(const omnimem_ref_params* p, int n_v, int n, int m, int t) {
-  if (m == 0) return t < n_v ? t : n + (t - n_v);
-  const int n_a = n - n_v;
-  return t < n_a ? n_v + t : n + p->Nn_v + (t - n_a);
+  const int n_m = m == 0 ? n_v : n - n_v;
+  if (t < n_m) return m == 0 ? t : n_v + t;                  /* cached rows: visual block, then audio block  */
+  if (p->chunk_modality == NULL)                             /* blocked chunk (R25)                          */
+    return m == 0 ? n + (t - n_v) : n + p->Nn_v + (t - n_m);
+  int want = t - n_m;                                        /* interleaved chunk: the want-th row of modality m */
+  for (int r = 0; r < p->Nn_v + p->Nn_a; ++r)
+    if (p->chunk_modality[r] == m && want-- == 0) return n + r;
+  return -1;                                                 /* Nn_v / Nn_a do not match the map             */
 }
 static int seg_len(const omnimem_ref_params* p, int n_v, int n, int m) {
   return m == 0 ? n_v + p->Nn_v : (n - n_v) + p->Nn_a;

@@ -17,6 +17,8 @@ from dataclasses import dataclass
 
 import dataclasses
 
+from typing import Optional
+
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -39,7 +41,7 @@ class _Params(C.Structure):
         ("sim_stride_v", C.c_int32), ("sim_stride_a", C.c_int32),
         ("seg_cap_v", C.c_int32), ("seg_cap_a", C.c_int32),
         ("scale", C.c_double), ("lam", C.c_double), ("ratio_r", C.c_double), ("temperature", C.c_double),
-        ("budget_min", C.c_int64), ("budget_max", C.c_int64),
+        ("budget_min", C.c_int64), ("budget_max", C.c_int64), ("chunk_modality", C.c_void_p),
     ]
 
 
@@ -61,6 +63,7 @@ class RefParams:
     temperature: float = 0.2
     budget_min: int = 0
     budget_max: int = 0
+    chunk_modality: Optional[np.ndarray] = None   # [Nn] int32, 0 visual / 1 audio per chunk row (time-interleaved chunk)
 
     @property
     def Nn(self) -> int:
@@ -76,9 +79,14 @@ class RefParams:
 
     def c(self) -> _Params:
         sc = self.scale if self.scale > 0 else 1.0 / float(np.sqrt(np.float64(self.D)))
+        mod = None
+        if self.chunk_modality is not None:
+            self._mod = np.ascontiguousarray(self.chunk_modality, dtype=np.int32)   # kept alive by the dataclass instance
+            assert self._mod.shape == (self.Nn,) and int((self._mod == 0).sum()) == self.Nn_v
+            mod = self._mod.ctypes.data
         return _Params(self.L, self.Hq, self.Hkv, self.D, self.cache_cap, self.Nn_v, self.Nn_a, self.causal,
                        self.sim_stride_v, self.sim_stride_a, self.seg_cap_v, self.seg_cap_a,
-                       sc, self.lam, self.ratio_r, self.temperature, self.budget_min, self.budget_max)
+                       sc, self.lam, self.ratio_r, self.temperature, self.budget_min, self.budget_max, mod)
 
 
 _lib = None

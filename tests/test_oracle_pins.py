@@ -426,6 +426,47 @@ def test_redundancy_hidden_states():
     np.testing.assert_array_equal(dst[0, 3:5], aud0[[1, 3]])
 
 
+def test_time_interleaved_chunk():
+    """R25' (NEXT-4b): chunk rows in true temporal order with a per-row modality map.  Pins: (1) the attention itself
+    does not know the map (torch softmax, causal by storage order = true position) and the split takes the map's rows;
+    (2) Eq.7 neighbours are the adjacent tokens of the same modality, by torch cosine on sequences built with numpy;
+    (3) without the causal mask an interleaved chunk is a row permutation of the blocked chunk: every segment output,
+    the kept sets and the compacted bytes are the same."""
+    mod = np.array([0, 0, 1, 0, 1, 1, 0, 0], np.int32)                      # Nn_v = 5, Nn_a = 3
+    p, x = make(chunk_modality=mod)
+    Nc, n_v = 9, 6
+    out = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+    a_t = torch_attention(p, x, 0)[0]                                       # [Hkv, Nc + Nn], knows nothing of modalities
+    vis = np.concatenate([a_t[:, :n_v], a_t[:, Nc:][:, mod == 0]], 1)
+    aud = np.concatenate([a_t[:, n_v:Nc], a_t[:, Nc:][:, mod == 1]], 1)
+    np.testing.assert_allclose(out["a_v"][0, :, :11], vis, rtol=1e-12)
+    np.testing.assert_allclose(out["a_a"][0, :, :6], aud, rtol=1e-12)
+    cos = torch.nn.functional.cosine_similarity
+    for h in range(p.Hkv):
+        seq = torch.from_numpy(np.concatenate([x["cacheV"][0, h, :n_v], x["chunkV"][0, h][mod == 0]]))
+        c = cos(seq[:-1], seq[1:], dim=-1).numpy()
+        want = np.concatenate([[c[0]], 0.5 * (c[:-1] + c[1:]), [c[-1]]])
+        np.testing.assert_allclose(out["s_v"][0, h, :11], want, atol=1e-12)
+    # (3) permutation invariance without the causal mask
+    perm = np.concatenate([np.where(mod == 0)[0], np.where(mod == 1)[0]])   # interleaved row of each blocked row
+    pi, xi = make(chunk_modality=mod, causal=0)
+    pb, xb = make(causal=0)
+    for k in ("chunkK", "chunkV", "Q"):
+        xb[k] = np.ascontiguousarray(xi[k][:, :, perm])
+    B = np.array([7], np.int32)
+    oi = ref.compress_chunk(pi, xi["cacheK"], xi["cacheV"], xi["n_v"], xi["n"], xi["chunkK"], xi["chunkV"], xi["Q"], B)
+    ob = ref.compress_chunk(pb, xb["cacheK"], xb["cacheV"], xb["n_v"], xb["n"], xb["chunkK"], xb["chunkV"], xb["Q"], B)
+    for k in ("a_v", "a_a", "s_v", "s_a", "stats"):
+        np.testing.assert_allclose(oi[k], ob[k], rtol=1e-12, atol=1e-15)
+    assert np.array_equal(oi["M_v"], ob["M_v"]) and np.array_equal(oi["idx_v"], ob["idx_v"]) and np.array_equal(oi["idx_a"], ob["idx_a"])
+    assert np.array_equal(oi["dstK"], ob["dstK"]) and np.array_equal(oi["dstV"], ob["dstV"])
+    # with the causal mask the two layouts differ: an early audio row is seen by more queries than in the blocked order
+    oc = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+    pbc, _ = make(causal=1)
+    obc = ref.score(pbc, xb["cacheK"], xb["cacheV"], xb["n_v"], xb["n"], xb["chunkK"], xb["chunkV"], xb["Q"])
+    assert not np.allclose(oc["a_a"], obc["a_a"])
+
+
 def test_calibration_means_then_eq14():
     """R28: budgets from the MEANS of the two layer measures over the calibration chunks.  Pins: one chunk ==
     plain Eq.14; chunks that are permutations of each other give the same table; closed form of the two-layer case
