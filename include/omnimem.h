@@ -103,6 +103,11 @@ typedef struct {     /* one chunk, modality-blocked */
                         model's own attention forward; NULL => computed here (score pass 1)                        */
   int32_t Nn_v, Nn_a; /* HOST ints: rows of each modality in this chunk                       */
   const void* h;     /* sim_source == 2 only, else NULL: [L, Nn, d_model] hidden states of the chunk's tokens */
+  const int32_t* modality; /* NULL = modality-blocked chunk (visual rows [0, Nn_v), then audio rows; R25).  Else
+                        DEVICE [Nn]: 0 = visual, 1 = audio for every chunk row, rows in TRUE temporal order (a
+                        time-interleaved chunk, R25'); exactly Nn_v zeros.  The causal mask of R3 then follows the true
+                        position, and the j-th visual (audio) row of the chunk is entry n_v + j (n_a + j) of the
+                        appended visual (audio) sequence.  The same map serves every layer.                */
 } omnimem_chunk;
 
 typedef struct {     /* outputs of the scoring stages; any pointer may be NULL except where noted */
@@ -187,7 +192,8 @@ OMNIMEM_API int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* sr
  * synchronises `stream` before returning.  Layers are independent through the whole step (the per-layer
  * totals are an input, R21), so the chunk is copied and compressed in up to 8 groups of consecutive layers: the
  * copies run on a stream owned by the context (ordered after everything already enqueued on `stream`) and the
- * kernels of group g on `stream` overlap the copy of group g + 1.  Results are identical to omnimem_compress_chunk
+ * kernels of group g on `stream` overlap the copy of group g + 1.  host_chunk->h and host_chunk->modality, when set,
+ * are HOST arrays too and dev_chunk->h / dev_chunk->modality their DEVICE staging buffers.  Results are identical to omnimem_compress_chunk
  * on the same inputs.  Returns the byte counts moved through h2d_bytes / d2h_bytes (HOST, may be NULL). */
 OMNIMEM_API int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
                                 const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,

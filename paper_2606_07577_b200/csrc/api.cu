@@ -150,6 +150,20 @@ int check_scores(const omnimem_scores* o) {
   return (o->a_v && o->a_a && o->s_v && o->s_a && o->psi_v && o->psi_a && o->stats) ? OMNIMEM_OK : OMNIMEM_INVALID_ARG;
 }
 
+// Time-interleaved chunk (R25'): derive the row <-> segment maps on the stream and hang them on the step parameters.
+int set_chunk_maps(omnimem_ctx* c, const omnimem_chunk* ch, StepParams& p, cudaStream_t st) {
+  p.row_of_seg = nullptr;
+  p.seg_of_row = nullptr;
+  if (!ch->modality || p.Nn == 0) return OMNIMEM_OK;
+  int32_t* row_of_seg = c->chunk_maps;
+  int32_t* seg_of_row = c->chunk_maps + (c->cfg.max_chunk_v + c->cfg.max_chunk_a);
+  cudaError_t e = launch_chunk_maps(ch->modality, p.Nn, p.Nn_v, row_of_seg, seg_of_row, st, &c->launches);
+  if (e != cudaSuccess) return fail_cuda(c, e);
+  p.row_of_seg = row_of_seg;
+  p.seg_of_row = seg_of_row;
+  return OMNIMEM_OK;
+}
+
 int check_fused_args(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* layer_budget,
                      omnimem_cache* dst, omnimem_scores* opt_out, void* ws, size_t ws_bytes) {
   if (!ctx || !layer_budget || !ws) return OMNIMEM_INVALID_ARG;
@@ -210,9 +224,11 @@ int compress_layers(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
   const int32_t* budget = layer_budget + l0;
   // layers with nothing to evict skip scoring unless the caller asked for the scores
   StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, s2.n_v, s2.n, opt_out ? nullptr : budget, Lg);
+  int rc = set_chunk_maps(ctx, chunk, p, st);
+  if (rc) return rc;
   StepBuffers b{};
   fill_buffers(ctx, &s2, &c2, opt_out ? &o2 : nullptr, wsb, w2, b);
-  int rc = run_score(ctx, p, b, st);
+  rc = run_score(ctx, p, b, st);
   if (rc) return rc;
   int32_t* M_v = opt_M_v ? opt_M_v + l0 : (int32_t*)(wsb + w2.M_v);
   int32_t* M_a = opt_M_a ? opt_M_a + l0 : (int32_t*)(wsb + w2.M_a);
@@ -296,6 +312,13 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
     if (e != cudaSuccess) { delete c; return OMNIMEM_CUDA_ERROR; }
   }
   for (int s = 0; s < OMNIMEM_N_STAGES; ++s) c->ev_used[s] = false;
+  c->chunk_maps = nullptr;
+  c->copy_stream = nullptr;
+  for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) c->ev_copy[i] = nullptr;
+  if (g.max_chunk_v + g.max_chunk_a > 0) {
+    e = cudaMalloc((void**)&c->chunk_maps, 2 * sizeof(int32_t) * ((size_t)g.max_chunk_v + g.max_chunk_a));
+    if (e != cudaSuccess) { omnimem_destroy(c); return OMNIMEM_CUDA_ERROR; }
+  }
   c->copy_stream = nullptr;
   for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) c->ev_copy[i] = nullptr;
   e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
@@ -310,6 +333,7 @@ int omnimem_destroy(omnimem_ctx* ctx) {
   for (int i = 0; i < 2 * OMNIMEM_N_STAGES; ++i) cudaEventDestroy(ctx->ev[i]);
   for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  if (ctx->chunk_maps) cudaFree(ctx->chunk_maps);
   delete ctx;
   return OMNIMEM_OK;
 }
@@ -360,6 +384,7 @@ int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chun
   if (ws_bytes < w.total) return OMNIMEM_WORKSPACE_TOO_SMALL;
   begin_call(ctx);
   StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
+  if ((rc = set_chunk_maps(ctx, chunk, p, (cudaStream_t)stream))) return rc;
   StepBuffers b{};
   fill_buffers(ctx, src, chunk, out, (uint8_t*)ws, w, b);
   return run_score(ctx, p, b, (cudaStream_t)stream);
@@ -425,6 +450,7 @@ int omnimem_compact(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
   if ((rc = check_hidden(ctx, src, chunk)) || (rc = check_hidden(ctx, dst, nullptr))) return rc;
   begin_call(ctx);
   StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
+  if ((rc = set_chunk_maps(ctx, chunk, p, (cudaStream_t)stream))) return rc;
   StageTimer t(ctx, (cudaStream_t)stream, OMNIMEM_STAGE_COMPACT);
   cudaError_t e = launch_compact(ctx, p, src->k, src->v, chunk->k, chunk->v, idx_v, idx_a, M_v, M_a, dst->k, dst->v,
                                  dst->n_v, dst->n, (cudaStream_t)stream, &ctx->launches);
@@ -457,6 +483,7 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   ch.Nn_v = host_chunk->Nn_v;
   ch.Nn_a = host_chunk->Nn_a;
   if (!host_chunk->lse) ch.lse = nullptr;
+  if (!host_chunk->modality) ch.modality = nullptr;
   rc = check_fused_args(ctx, src, &ch, layer_budget, dst, nullptr, ws, ws_bytes);
   if (rc) return rc;
   const WsLayout w = ws_layout(ctx);
@@ -478,6 +505,12 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_copy[OMNIMEM_HOST_GROUPS], 0);
   if (e != cudaSuccess) return fail_cuda(ctx, e);
   auto at = [](const void* p, size_t bytes) { return (void*)((uint8_t*)const_cast<void*>(p) + bytes); };
+  if (host_chunk->modality && Nn > 0) {   // HOST [Nn] -> the device staging copy, ahead of the first group
+    if (!dev_chunk->modality) return OMNIMEM_INVALID_ARG;
+    e = cudaMemcpyAsync(const_cast<int32_t*>(dev_chunk->modality), host_chunk->modality, Nn * sizeof(int32_t),
+                        cudaMemcpyHostToDevice, ctx->copy_stream);
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+  }
   int gi = 0;
   for (int l0 = 0; l0 < L; l0 += per_group, ++gi) {
     const int Lg = L - l0 < per_group ? L - l0 : per_group;

@@ -26,6 +26,9 @@ struct StepParams {
   const int32_t* n_v;        // [L]
   const int32_t* n;          // [L]
   const int32_t* skip_budget;  // [L] or nullptr: layers with n[l] + Nn <= skip_budget[l] skip scoring
+  // time-interleaved chunk (chunk.modality != NULL, R25'), else nullptr = modality-blocked chunk:
+  const int32_t* row_of_seg;   // [Nn]: chunk rows of the visual tokens in order, then those of the audio tokens
+  const int32_t* seg_of_row;   // [Nn]: (modality << 30) | index among the chunk's tokens of that modality
 };
 
 // Segment maps (include/omnimem.h "Conventions"; Eq.3 appended sequences).
@@ -40,13 +43,20 @@ __device__ __forceinline__ int seg_row(const StepParams& p, int n_v, int n, int 
     return (m == 0 ? 0 : n_v) + t;
   }
   in_chunk = true;
-  return (m == 0 ? 0 : p.Nn_v) + (t - n_m);
+  const int j = (m == 0 ? 0 : p.Nn_v) + (t - n_m);
+  return p.row_of_seg ? p.row_of_seg[j] : j;
 }
 // logical key (cache row r < n, or chunk row) -> (modality, segment-local index)
 __device__ __forceinline__ void cache_row_to_seg(int n_v, int r, int& m, int& t) {
   if (r < n_v) { m = 0; t = r; } else { m = 1; t = r - n_v; }
 }
 __device__ __forceinline__ void chunk_row_to_seg(const StepParams& p, int n_v, int n, int r, int& m, int& t) {
+  if (p.seg_of_row) {
+    const int e = p.seg_of_row[r];
+    m = e >> 30;
+    t = (m == 0 ? n_v : n - n_v) + (e & 0x3FFFFFFF);
+    return;
+  }
   if (r < p.Nn_v) { m = 0; t = n_v + r; } else { m = 1; t = (n - n_v) + (r - p.Nn_v); }
 }
 __device__ __forceinline__ bool layer_skips_scoring(const StepParams& p, int l) {
@@ -89,6 +99,7 @@ struct omnimem_ctx {
   bool ev_used[OMNIMEM_N_STAGES];
   int launches;
   void* encode_tiled;  // cuTensorMapEncodeTiled entry point
+  int32_t* chunk_maps;   // device [2 * (max_chunk_v + max_chunk_a)]: row_of_seg, seg_of_row of an interleaved chunk
   cudaStream_t copy_stream;                        // omnimem_compress_chunk_host: host -> device copies of the next layer group
   cudaEvent_t ev_copy[OMNIMEM_HOST_GROUPS + 1];    // [g] group g is on the device; [last] `stream` reached the call
 };
@@ -105,6 +116,8 @@ cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const S
 cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,
                             int64_t total_budget, int32_t* M_v, int32_t* M_a, int32_t* layer_budget_out, cudaStream_t st,
                             int* launches);
+cudaError_t launch_chunk_maps(const int32_t* modality, int Nn, int Nn_v, int32_t* row_of_seg, int32_t* seg_of_row,
+                              cudaStream_t st, int* launches);
 cudaError_t launch_compact_hidden(const omnimem_ctx* ctx, const StepParams& p, const void* srcH, const void* chunkH,
                                   const int32_t* idx_v, const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a,
                                   void* dstH, cudaStream_t st, int* launches);

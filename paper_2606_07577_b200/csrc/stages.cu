@@ -603,6 +603,42 @@ cudaError_t launch_compact(const omnimem_ctx* ctx, const StepParams& p, const vo
   return cudaGetLastError();
 }
 
+// Time-interleaved chunk (R25'): from the per-row modality map (0 visual, 1 audio, rows in true temporal order) build
+// row_of_seg (rows of the visual tokens in order, then the audio tokens') and seg_of_row ((m << 30) | rank within m).
+// One block; thread i owns a contiguous slice, slice counts are scanned in shared memory.
+__global__ void __launch_bounds__(1024) chunk_maps_kernel(const int32_t* __restrict__ modality, int Nn, int Nn_v,
+                                                          int32_t* __restrict__ row_of_seg,
+                                                          int32_t* __restrict__ seg_of_row) {
+  __shared__ int cnt[1024];
+  const int per = (Nn + 1023) / 1024;
+  const int r0 = threadIdx.x * per, r1 = min(Nn, r0 + per);
+  int c = 0;
+  for (int r = r0; r < r1; ++r) c += modality[r] == 0;
+  cnt[threadIdx.x] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int i = 0; i < 1024; ++i) { const int v = cnt[i]; cnt[i] = run; run += v; }
+  }
+  __syncthreads();
+  int jv = cnt[threadIdx.x], ja = r0 < Nn ? r0 - jv : 0;   // visual / audio tokens before this slice
+  for (int r = r0; r < r1; ++r) {
+    const int m = modality[r] == 0 ? 0 : 1;
+    const int j = m == 0 ? jv++ : ja++;
+    seg_of_row[r] = (m << 30) | j;
+    const int slot = m == 0 ? j : Nn_v + j;
+    if (slot < Nn && (m == 1 || j < Nn_v)) row_of_seg[slot] = r;   // a map that disagrees with Nn_v cannot write out of bounds
+  }
+}
+
+cudaError_t launch_chunk_maps(const int32_t* modality, int Nn, int Nn_v, int32_t* row_of_seg, int32_t* seg_of_row,
+                              cudaStream_t st, int* launches) {
+  if (Nn == 0) return cudaSuccess;
+  chunk_maps_kernel<<<1, 1024, 0, st>>>(modality, Nn, Nn_v, row_of_seg, seg_of_row);
+  ++*launches;
+  return cudaGetLastError();
+}
+
 // The retained hidden states follow the kept tokens: dstH[l, j] = row of the j-th kept index of the layer
 // (select_scope == 1: every head keeps the same rows, head 0's index list is read).  One warp per row, 512-byte steps.
 __global__ void __launch_bounds__(256) compact_hidden_kernel(StepParams p, const uint4* __restrict__ srcH,

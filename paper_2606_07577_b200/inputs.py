@@ -229,6 +229,31 @@ def hidden_inputs(wl: Workload, d_model: int, step: int = 0, with_cache: bool = 
     return dict(cacheH=cacheH, chunkH=chunkH)
 
 
+def modality_pattern(wl: Workload, groups: int) -> torch.Tensor:
+    """Per-row modality map of a time-interleaved chunk (NEXT-4b, R25'): `groups` time slices (e.g. seconds), each holding
+    its share of the visual rows followed by its share of the audio rows.  int32 [Nn], 0 = visual, 1 = audio."""
+    groups = max(1, min(groups, max(wl.Nn_v, wl.Nn_a, 1)))
+    out = []
+    for g in range(groups):
+        nv = (g + 1) * wl.Nn_v // groups - g * wl.Nn_v // groups
+        na = (g + 1) * wl.Nn_a // groups - g * wl.Nn_a // groups
+        out += [0] * nv + [1] * na
+    return torch.tensor(out, dtype=torch.int32)
+
+
+def interleave(x: dict, modality: torch.Tensor, Nn_v: int) -> dict:
+    """Reorder the chunk tensors of a modality-blocked input dict (chunkK, chunkV, Q and chunkH if present; row axis -2)
+    into the temporal order of `modality`: the j-th visual (audio) row of the result is blocked row j (Nn_v + j)."""
+    m = modality.long()
+    rank_v, rank_a = torch.cumsum(1 - m, 0) - 1, torch.cumsum(m, 0) - 1
+    src = torch.where(m == 0, rank_v, Nn_v + rank_a)
+    y = dict(x)
+    for k in ("chunkK", "chunkV", "Q", "chunkH"):
+        if k in x:
+            y[k] = x[k].index_select(-2, src).contiguous()
+    return y
+
+
 def small(wl: Workload, **kw) -> Workload:
     """A reduced copy of a config (same recipe and value structure) for tests the oracle finishes in seconds."""
     return wl.replace(**kw)

@@ -44,7 +44,7 @@ class omnimem_cache(C.Structure):
 
 class omnimem_chunk(C.Structure):
     _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("q", C.c_void_p), ("lse", C.c_void_p),
-                ("Nn_v", C.c_int32), ("Nn_a", C.c_int32), ("h", C.c_void_p)]
+                ("Nn_v", C.c_int32), ("Nn_a", C.c_int32), ("h", C.c_void_p), ("modality", C.c_void_p)]
 
 
 class omnimem_scores(C.Structure):
@@ -127,11 +127,13 @@ class Chunk:
     Nn_a: int
     lse: Optional[torch.Tensor] = None
     h: Optional[torch.Tensor] = None     # [L, Nn, d_model] hidden states of the chunk's tokens (sim_source == 2)
+    modality: Optional[torch.Tensor] = None   # int32 [Nn], 0 visual / 1 audio per row: time-interleaved chunk (R25')
 
     def c(self) -> omnimem_chunk:
         return omnimem_chunk(self.k.data_ptr(), self.v.data_ptr(), self.q.data_ptr(),
                              None if self.lse is None else self.lse.data_ptr(), self.Nn_v, self.Nn_a,
-                             None if self.h is None else self.h.data_ptr())
+                             None if self.h is None else self.h.data_ptr(),
+                             None if self.modality is None else self.modality.data_ptr())
 
 
 @dataclass

@@ -26,19 +26,25 @@ def dev_objs(x, wl):
     return Cache(d["cacheK"], d["cacheV"], d["n_v"], d["n"]), Chunk(d["chunkK"], d["chunkV"], d["Q"], wl.Nn_v, wl.Nn_a)
 
 
-def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=True, stats_tol=None, select_scope=0):
+def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=True, stats_tol=None, select_scope=0,
+               modality=None):
     """All of rules (a), (b), (c) for one step of workload `wl` (L = number of layers in x)."""
     eng_kw, ref_kw = dict(eng_kw or {}), dict(ref_kw or {})
     x = x if x is not None else I.full_inputs(wl)
     L = x["Q"].shape[0]
     wl = wl.replace(L=L)
     tol = TOL[wl.dtype]
+    if modality is not None:                       # time-interleaved chunk: both sides get the reordered rows + the map
+        x = I.interleave(x, modality, wl.Nn_v)
+        ref_kw["chunk_modality"] = modality.numpy()
     p = ref_params(wl, L, **ref_kw)
     B = np.full((L,), wl.budget, np.int32)
     orc = ref.compress_chunk(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"], B,
                              sim_source=sim_source, want_rowH=check_rowH, select_scope=select_scope)
     eng = engine_for(wl, sim_source=sim_source, select_scope=select_scope, **eng_kw)
     src, chunk = dev_objs(x, wl)
+    if modality is not None:
+        chunk.modality = modality.cuda()
     n_v, n = x["n_v"].numpy(), x["n"].numpy()
     Kv, Ka = seg_lens(wl, n_v, n)
 
@@ -102,8 +108,9 @@ def check_step(wl, x=None, eng_kw=None, ref_kw=None, sim_source=0, check_rowH=Tr
     rawc, rawk = x["cacheK"].view(torch.uint8).numpy(), x["chunkK"].view(torch.uint8).numpy()
     for l in range(L):
         for h in range(wl.Hkv):
-            vis = np.concatenate([rawc[l, h, :n_v[l]], rawk[l, h, :wl.Nn_v]])
-            aud = np.concatenate([rawc[l, h, n_v[l]:n[l]], rawk[l, h, wl.Nn_v:]])
+            mv_rows = np.arange(wl.Nn) < wl.Nn_v if modality is None else modality.numpy() == 0
+            vis = np.concatenate([rawc[l, h, :n_v[l]], rawk[l, h][mv_rows]])
+            aud = np.concatenate([rawc[l, h, n_v[l]:n[l]], rawk[l, h][~mv_rows]])
             assert np.array_equal(dK2[l, h, :mv[l]], vis[iv[l, h, :mv[l]]])
             assert np.array_equal(dK2[l, h, mv[l]:mv[l] + ma[l]], aud[ia[l, h, :ma[l]]])
     eng.close()
@@ -458,4 +465,32 @@ def test_hidden_state_redundancy_variant():
     src, chunk = dev_objs(x, I.CFG1)
     with pytest.raises(OmniMemError, match="invalid"):
         eng.score(src, chunk)                                  # cache.h / chunk.h missing
+    eng.close()
+
+
+def test_time_interleaved_chunk():
+    """NEXT-4b (R25'): chunk rows in true temporal order with a per-row modality map: causal mask by true position,
+    segments gathered through the map.  All of rules (a), (b), (c) on the tcgen05, SIMT and fp32 paths, plus the host
+    entry (the map travels from host memory)."""
+    check_step(I.CFG1, modality=I.modality_pattern(I.CFG1, 7))
+    check_step(SMALL2, modality=I.modality_pattern(SMALL2, 9))
+    check_step(SMALL3, modality=I.modality_pattern(SMALL3, 1000))                  # alternating single rows
+    check_step(SMALL2, modality=I.modality_pattern(SMALL2, 5), eng_kw=dict(score_path=1))
+    check_step(SMALL4, modality=I.modality_pattern(SMALL4, 3), eng_kw=dict(causal=0), ref_kw=dict(causal=0))
+    from paper_2606_07577_b200.omnimem import Chunk
+    wl = SMALL2.replace(L=3)
+    mod = I.modality_pattern(wl, 6)
+    x = I.interleave(I.full_inputs(wl, pin=True), mod, wl.Nn_v)
+    eng = engine_for(wl)
+    src, chunk = dev_objs(x, wl)
+    chunk.modality = mod.cuda()
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device="cuda")
+    dst, dst2 = eng.new_cache(), eng.new_cache()
+    eng.compress_chunk(src, chunk, B, dst)
+    host_chunk = Chunk(x["chunkK"].pin_memory(), x["chunkV"].pin_memory(), x["Q"].pin_memory(), wl.Nn_v, wl.Nn_a, modality=mod.pin_memory())
+    stage = Chunk(torch.zeros_like(chunk.k), torch.zeros_like(chunk.v), torch.zeros_like(chunk.q), wl.Nn_v, wl.Nn_a,
+                  modality=torch.zeros_like(chunk.modality))
+    hM_v, hM_a = torch.zeros(wl.L, dtype=torch.int32).pin_memory(), torch.zeros(wl.L, dtype=torch.int32).pin_memory()
+    eng.compress_chunk_host(src, host_chunk, stage, B, dst2, hM_v, hM_a)
+    assert torch.equal(dst2.n, dst.n) and torch.equal(dst2.k, dst.k) and torch.equal(dst2.v, dst.v)
     eng.close()
