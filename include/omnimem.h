@@ -190,7 +190,7 @@ OMNIMEM_API int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* sr
  * layout above; dev_chunk holds DEVICE staging buffers of the same shapes (caller-owned).  Copies the chunk to the
  * device, runs the fused step, copies M_v, M_a back to the HOST arrays host_M_v, host_M_a [L] (pinned) and
  * synchronises `stream` before returning.  Layers are independent through the whole step (the per-layer
- * totals are an input, R21), so the chunk is copied and compressed in up to 8 groups of consecutive layers: the
+ * totals are an input, R21), so the chunk is copied and compressed in up to 8 groups of consecutive layers (1, 2, 3, 4, 6, 9, ... layers): the
  * copies run on a stream owned by the context (ordered after everything already enqueued on `stream`) and the
  * kernels of group g on `stream` overlap the copy of group g + 1.  host_chunk->h and host_chunk->modality, when set,
  * are HOST arrays too and dev_chunk->h / dev_chunk->modality their DEVICE staging buffers.  Results are identical to omnimem_compress_chunk

@@ -500,7 +500,17 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   begin_call(ctx);
   // Layers are independent through the whole step, so the chunk is copied and compressed in groups of layers: the
   // copy of group g + 1 (on the context's copy stream) overlaps the kernels of group g (on `stream`).
-  const int per_group = (L + OMNIMEM_HOST_GROUPS - 1) / OMNIMEM_HOST_GROUPS;
+  // Group sizes grow geometrically (1, 2, 3, 4, 6, 9, ... layers): only the first, one-layer copy is exposed, each later
+  // copy is shorter than the kernels it hides behind (a layer computes for longer than it copies), and the big late
+  // groups keep the scoring kernels' tail waves few.  The last of the OMNIMEM_HOST_GROUPS groups takes the rest.
+  int group_size[OMNIMEM_HOST_GROUPS];
+  int n_groups = 0;
+  for (int left = L, sz = 1; left > 0; ++n_groups) {
+    const int take = (n_groups == OMNIMEM_HOST_GROUPS - 1 || sz > left) ? left : sz;
+    group_size[n_groups] = take;
+    left -= take;
+    sz = sz + 1 > sz * 3 / 2 ? sz + 1 : sz * 3 / 2;
+  }
   cudaError_t e = cudaEventRecord(ctx->ev_copy[OMNIMEM_HOST_GROUPS], st);   // staging buffers are free once `stream` got here
   if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_copy[OMNIMEM_HOST_GROUPS], 0);
   if (e != cudaSuccess) return fail_cuda(ctx, e);
@@ -512,8 +522,8 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
     if (e != cudaSuccess) return fail_cuda(ctx, e);
   }
   int gi = 0;
-  for (int l0 = 0; l0 < L; l0 += per_group, ++gi) {
-    const int Lg = L - l0 < per_group ? L - l0 : per_group;
+  for (int l0 = 0; gi < n_groups; l0 += group_size[gi], ++gi) {
+    const int Lg = group_size[gi];
     if (Nn > 0) {
       cudaStream_t cs = ctx->copy_stream;
       e = cudaMemcpyAsync(at(dev_chunk->k, l0 * kv_layer), at(host_chunk->k, l0 * kv_layer), Lg * kv_layer, cudaMemcpyHostToDevice, cs);
