@@ -35,6 +35,14 @@ constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 
 constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
+// Two CTAs of a cluster (one TPC) work on neighbouring stationary blocks and stream the SAME tiles: each loads one
+// 64-column K-block of every tile and multicasts it into both shared memories, which halves the L2 -> SM read traffic
+// of the streamed operand (96 GB per pass at CFG2; its removal was worth ~8 % of a pass under the power cap).
+#ifndef OMNIMEM_CLUSTER
+#define OMNIMEM_CLUSTER 1
+#endif
+constexpr int kCluster = OMNIMEM_CLUSTER;   // 1 or 2
+
 // ---- PTX wrappers -------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -59,6 +67,24 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
           "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar,
+                                               uint16_t cta_mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, "
+      "%3, %4}], [%5], %6;" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void tc_commit_mc(uint32_t bar, uint16_t cta_mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+               "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
 }
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
@@ -238,10 +264,11 @@ struct Work {
   int n_cache_tiles, ntiles_sub[2], h;
   // pass 2
   int it0[2], tiles_per_g, hq0;
+  int seq0;              // first query tile of the streamed sequence (== it0[0] unless a cluster peer starts earlier)
 };
 
 template <int kPass>
-__device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
+__device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int bx) {   // bx: x index of the CTA described
   const StepParams& p = a.p;
   w.l = blockIdx.z;
   // values loaded from memory are made provably warp-uniform (shfl) so that the control warps stay on the uniform datapath
@@ -251,7 +278,7 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
     const int j = blockIdx.y;  // query head
     w.h = j / p.G;
     w.lhA = w.l * p.Hq + j;
-    w.rowA0 = blockIdx.x * 2 * kTile;
+    w.rowA0 = bx * 2 * kTile;
     w.a_chunk = false;
     w.n_cache_tiles = (n + kTile - 1) / kTile;
     const int nct = (p.Nn + kTile - 1) / kTile;
@@ -270,13 +297,13 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
     w.lhA = w.l * p.Hkv + h;
     w.hq0 = w.l * p.Hq + h * p.G;
     int valid_rows;
-    if ((int)blockIdx.x < a.n_cache_pairs) {
+    if (bx < a.n_cache_pairs) {
       w.a_chunk = false;
-      w.rowA0 = blockIdx.x * 2 * kTile;
+      w.rowA0 = bx * 2 * kTile;
       valid_rows = n;
     } else {
       w.a_chunk = true;
-      w.rowA0 = (blockIdx.x - a.n_cache_pairs) * 2 * kTile;
+      w.rowA0 = (bx - a.n_cache_pairs) * 2 * kTile;
       valid_rows = p.Nn;
     }
     const int nqt = (p.Nn + kTile - 1) / kTile;
@@ -285,9 +312,11 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w) {
       w.sub_valid[s] = r0 < valid_rows;
       w.it0[s] = (p.causal && w.a_chunk) ? r0 / kTile : 0;  // first query tile that can see this key sub-tile
     }
-    w.tiles_per_g = nqt - w.it0[0];
+    w.seq0 = w.it0[0];
+    w.tiles_per_g = nqt - w.seq0;
     w.ntiles = w.sub_valid[0] ? p.G * w.tiles_per_g : 0;
-    return w.sub_valid[0] && w.ntiles > 0;
+    if (w.ntiles <= 0) { w.ntiles = 0; w.sub_valid[0] = w.sub_valid[1] = false; }
+    return w.sub_valid[0];
   }
 }
 
@@ -298,7 +327,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   extern __shared__ uint8_t smem_raw[];
   const StepParams& p = a.p;
   Work w;
-  if (!make_work<kPass>(a, w)) return;  // uniform across the CTA
+  const bool mine = make_work<kPass>(a, w, (int)blockIdx.x);
+  if (kCluster == 2) {
+    // the pair streams one sequence: the union of what its two CTAs need (a CTA skips the tiles that are not its own)
+    Work wp;
+    const bool peer = make_work<kPass>(a, wp, (int)blockIdx.x ^ 1);
+    if (!mine && !peer) return;           // uniform across the cluster
+    if (kPass == 1) {
+      w.ntiles = max(mine ? w.ntiles : 0, peer ? wp.ntiles : 0);
+    } else {
+      w.seq0 = min(mine ? w.seq0 : 1 << 30, peer ? wp.seq0 : 1 << 30);
+      w.tiles_per_g = (p.Nn + kTile - 1) / kTile - w.seq0;
+      w.ntiles = p.G * w.tiles_per_g;
+    }
+  } else if (!mine) {
+    return;                               // uniform across the CTA
+  }
+  const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
 
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const uint32_t sB = smem_u32(smem);                    // [kStages][2 kb][16 KB]
@@ -312,7 +357,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, kCluster); }
     mbar_init(bar_a, w.sub_valid[1] ? 16 : 8);  // one arrival per epilogue warp that stages stationary rows
     for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
@@ -324,12 +369,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
+  if (kCluster == 2) cluster_sync_all();   // the peer's barriers exist before anything is multicast into them
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
   if (warp == 0) {
     // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
-    int it = kPass == 2 ? w.it0[0] : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
+    int it = kPass == 2 ? w.seq0 : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_empty + 8 * stage, sph);
       const CUtensorMap* mB;
@@ -343,7 +389,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         mB = &mapQ;
         row0 = it * kTile;
         lh = w.hq0 + g;
-        if (++it == w.it0[0] + w.tiles_per_g) { it = w.it0[0]; ++g; }
+        if (++it == w.seq0 + w.tiles_per_g) { it = w.seq0; ++g; }
       }
 #ifdef OMNIMEM_DBG_NOTMA
       if (elect_one()) { mbar_arrive(bar_full + 8 * stage); if (kPass == 2) mbar_arrive(bar_lse + 8 * slot); }
@@ -362,19 +408,28 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
           bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
         }
-        for (int kb = 0; kb < 2; ++kb)
-          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
+        if (kCluster == 2) {
+          const int kb = (int)cta_rank;   // this CTA's K-block, delivered to both CTAs; the peer sends the other one
+          tma_load_3d_mc(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage, 3);
+        } else {
+          for (int kb = 0; kb < 2; ++kb)
+            tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
+        }
       }
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
       if (++slot == kLseSlots) slot = 0;
     }
+    if (kCluster == 2) {
+      // drain: every stage released by BOTH CTAs, i.e. no remote arrival is still on its way to this CTA's barriers
+      for (int j = max(0, w.ntiles - kStages); j < w.ntiles; ++j) mbar_wait(bar_empty + 8 * (j % kStages), (j / kStages) & 1);
+    }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    mbar_wait(bar_a, 0);  // stationary rows are in TMEM
+    if (mine) mbar_wait(bar_a, 0);  // stationary rows are in TMEM (a CTA that only serves its peer has none)
     tc_fence_after();
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
-    int it = kPass == 2 ? w.it0[0] : 0, stage = 0, sph = 0;
+    int it = kPass == 2 ? w.seq0 : 0, stage = 0, sph = 0;
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_full + 8 * stage, sph);
       tc_fence_after();
@@ -399,10 +454,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         __syncwarp();
         if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
       }
-      if (elect_one()) tc_commit(bar_empty + 8 * stage);
+      if (elect_one()) { if (kCluster == 2) tc_commit_mc(bar_empty + 8 * stage, 3); else tc_commit(bar_empty + 8 * stage); }
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
-      if (kPass == 2 && ++it == w.it0[0] + w.tiles_per_g) it = w.it0[0];
+      if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
@@ -540,7 +595,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         uint64_t acc01 = 0ull, acc23 = 0ull;   // packed fp32x2 partial sums of the unmasked tiles
         const uint64_t c2c2 = pack2(c2, c2);
-        const int it_first = w.it0[0], it_end = w.it0[0] + w.tiles_per_g, it_mine = w.it0[s], it_other = w.it0[s ^ 1];
+        const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s], it_other = w.it0[s ^ 1];
         const bool other_valid = w.sub_valid[s ^ 1];
         int it_next = it_first;
         for (int j = 0; j < w.ntiles; ++j) {
@@ -611,6 +666,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
+  if (kCluster == 2) cluster_sync_all();   // nobody leaves while the peer may still write into this CTA
   if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
@@ -684,6 +740,32 @@ static TcArgs make_args(const StepParams& p, const StepBuffers& b) {
   return a;
 }
 
+// One launch of a scoring kernel: 211 KB of dynamic shared memory, and a (2,1,1) cluster when kCluster == 2 (grid.x is
+// rounded up to even; the extra CTA has no rows of its own and only serves its peer, or exits with it).
+typedef void (*ScoreKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const TcArgs);
+static cudaError_t launch_score(ScoreKernel k, dim3 grid, cudaStream_t st, const Maps& m, const TcArgs& a) {
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  if (kCluster == 1) {
+    k<<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
+    return cudaGetLastError();
+  }
+  grid.x = (grid.x + kCluster - 1) / kCluster * kCluster;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = kSmemBytes;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = kCluster;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, k, m.q, m.kc, m.kn, a);
+}
+
 cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
   if (p.Nn == 0) return cudaSuccess;
   Maps m;
@@ -692,16 +774,8 @@ cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const Ste
   const TcArgs a = make_args(p, b);
   dim3 grid((p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hq, p.L);
   ++*launches;
-  if (b.row_entropy) {
-    e = cudaFuncSetAttribute(score_tc_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    score_tc_kernel<1, true><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
-  } else {
-    e = cudaFuncSetAttribute(score_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    score_tc_kernel<1, false><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
-  }
-  return cudaGetLastError();
+  if (b.row_entropy) return launch_score(score_tc_kernel<1, true>, grid, st, m, a);
+  return launch_score(score_tc_kernel<1, false>, grid, st, m, a);
 }
 
 cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
@@ -720,11 +794,8 @@ cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const 
     ++*launches;
   }
   dim3 grid(a.n_cache_pairs + (p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hkv, p.L);
-  e = cudaFuncSetAttribute(score_tc_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-  if (e != cudaSuccess) return e;
   ++*launches;
-  score_tc_kernel<2, false><<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
-  return cudaGetLastError();
+  return launch_score(score_tc_kernel<2, false>, grid, st, m, a);
 }
 
 }  // namespace omnimem
