@@ -54,6 +54,13 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+#ifdef OMNIMEM_DBG_FREERUN
+#define EPI_WAIT(bar, parity) ((void)0)
+#define EPI_ARRIVE(bar) ((void)0)
+#else
+#define EPI_WAIT(bar, parity) mbar_wait(bar, parity)
+#define EPI_ARRIVE(bar) mbar_arrive(bar)
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
@@ -345,8 +352,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   }
   const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
 
-  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  const uint32_t sB = smem_u32(smem);                    // [kStages][2 kb][16 KB]
+  // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
+  // array is a link-time constant, so every barrier / stage address below folds into an immediate
+  const uint32_t s_raw = smem_u32(smem_raw);
+  const uint32_t sB = (s_raw + 1023u) & ~1023u;          // [kStages][2 kb][16 KB]
+  uint8_t* smem = smem_raw + (sB - s_raw);
   const uint32_t sLse = sB + kOffLse;                    // [kLseSlots][128] float (pass 2)
   float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 sub][128]
   const uint32_t bars = sB + kOffBars;
@@ -373,6 +383,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
+#ifdef OMNIMEM_DBG_FREERUN
+  if (warp < 4) goto done;   // timing experiment only: the epilogue reads whatever tensor memory holds, nobody feeds it
+#endif
   if (warp == 0) {
     // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
     int it = kPass == 2 ? w.seq0 : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
@@ -515,7 +528,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             if (p.causal) limit = min(limit, i - t0 + 1);
           }
           limit -= col0;
-          mbar_wait(bar_sfull + 8 * buf, ph);
+          EPI_WAIT(bar_sfull + 8 * buf, ph);
           tc_fence_after();
           const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
           uint32_t v0[32], v1[32];
@@ -524,7 +537,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);  // registers hold the tile: free the TMEM buffer
+          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * buf);  // registers hold the tile: free the TMEM buffer
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
           float x[kHalf];
@@ -606,7 +619,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (it < it_mine) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
-          mbar_wait(bar_sfull + 8 * buf, ph);
+          EPI_WAIT(bar_sfull + 8 * buf, ph);
           tc_fence_after();
           const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
           uint32_t v0[32], v1[32];
@@ -615,10 +628,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_sempty + 8 * buf);
+          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * buf);
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
-          mbar_wait(bar_lse + 8 * slot, lse_parity);
+          EPI_WAIT(bar_lse + 8 * slot, lse_parity);
           const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
           if (first <= 0) {
 #pragma unroll
@@ -664,6 +677,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       }
     }
   }
+#ifdef OMNIMEM_DBG_FREERUN
+done:
+#endif
   tc_fence_before();
   __syncthreads();
   if (kCluster == 2) cluster_sync_all();   // nobody leaves while the peer may still write into this CTA
