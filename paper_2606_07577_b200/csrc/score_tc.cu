@@ -351,6 +351,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     return;                               // uniform across the CTA
   }
   const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
+#ifdef OMNIMEM_DBG_MAXTILES   // timing experiment only: cap the streamed sequence to expose the per-CTA fixed cost
+  w.ntiles = min(w.ntiles, OMNIMEM_DBG_MAXTILES);
+  w.ntiles_sub[0] = min(w.ntiles_sub[0], OMNIMEM_DBG_MAXTILES);
+  w.ntiles_sub[1] = min(w.ntiles_sub[1], OMNIMEM_DBG_MAXTILES);
+#endif
 
   // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
   // array is a link-time constant, so every barrier / stage address below folds into an immediate
@@ -516,30 +521,20 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const int n = p.n[w.l];
         float m_run = -1e30f, Z = 0.f, W = 0.f;
         const int nt0 = w.ntiles_sub[0], nt1 = w.ntiles_sub[1], nt_mine = s == 0 ? nt0 : nt1;
-        for (int j = 0; j < w.ntiles; ++j) {
-          if (s == 1 && j < nt0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
-          if (j >= nt_mine) { if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
-          // number of visible key columns of this tile for this row, relative to this thread's first column
-          int limit;
-          if (j < w.n_cache_tiles) limit = n - j * kTile;
-          else {
-            const int t0 = (j - w.n_cache_tiles) * kTile;
-            limit = p.Nn - t0;
-            if (p.causal) limit = min(limit, i - t0 + 1);
-          }
-          limit -= col0;
-          EPI_WAIT(bar_sfull + 8 * buf, ph);
+        // accumulator batch at ring position (b, bph) -> registers; the TMEM buffer is released as soon as they hold it
+        auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
+          EPI_WAIT(bar_sfull + 8 * b, bph);
           tc_fence_after();
-          const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
-          uint32_t v0[32], v1[32];
+          const uint32_t t_addr = t_col + (uint32_t)(b * kTile);
           tc_ld32(t_addr, v0);
           tc_ld32(t_addr + 32, v1);
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * buf);  // registers hold the tile: free the TMEM buffer
-          if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-          if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
+          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * b);
+        };
+        // online softmax statistics of this thread's 64 columns of one tile; limit = visible columns (>= 64: all)
+        auto row_update = [&](const uint32_t (&v0)[32], const uint32_t (&v1)[32], int limit) {
           float x[kHalf];
           if (limit >= kHalf) {
 #pragma unroll
@@ -567,12 +562,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             const uint64_t P01 = ex2_pair(A01, e / 2), P23 = ex2_pair(A23, e / 2 + 1);
             z01 = add2(z01, P01);
             z23 = add2(z23, P23);
-            float a0, a1, a2, a3, p0, p1, p2, p3;
-            unpack2(A01, a0, a1);
-            unpack2(A23, a2, a3);
-            unpack2(P01, p0, p1);
-            unpack2(P23, p2, p3);
             if (kEntropy) {  // sum p z2 over visible columns (masked ones have p = 0 but z2 = -inf)
+              float a0, a1, a2, a3, p0, p1, p2, p3;
+              unpack2(A01, a0, a1);
+              unpack2(A23, a2, a3);
+              unpack2(P01, p0, p1);
+              unpack2(P23, p2, p3);
               wz[0] = fmaf(p0, limit > e ? a0 + m_new : 0.f, wz[0]);
               wz[1] = fmaf(p1, limit > e + 1 ? a1 + m_new : 0.f, wz[1]);
               wz[2] = fmaf(p2, limit > e + 2 ? a2 + m_new : 0.f, wz[2]);
@@ -584,6 +579,37 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           unpack2(z23, z2, z3);
           Z = fmaf(Z, rs, (z0 + z1) + (z2 + z3));
           if (kEntropy) W = fmaf(W, rs, (wz[0] + wz[1]) + (wz[2] + wz[3]));
+        };
+        int j = 0;
+        // Steady state: tiles that lie fully inside the cache are taken by both sub-tiles and need no mask, so the ring
+        // position advances by two batches per tile and the loop carries no other bookkeeping.
+        const int n_simple = (w.sub_valid[0] && w.sub_valid[1]) ? min(n / kTile, w.ntiles) : 0;
+        for (; j < n_simple; ++j) {
+          int own = buf + s, oph = ph;
+          if (own >= kAccBufs) { own -= kAccBufs; oph ^= 1; }
+          uint32_t v0[32], v1[32];
+          load_tile(own, oph, v0, v1);
+          buf += 2;
+          if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
+          row_update(v0, v1, kHalf);
+        }
+        for (; j < w.ntiles; ++j) {   // last cache tile, chunk tiles (causal edge), sub-tiles of unequal length
+          if (s == 1 && j < nt0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
+          if (j >= nt_mine) { if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          // number of visible key columns of this tile for this row, relative to this thread's first column
+          int limit;
+          if (j < w.n_cache_tiles) limit = n - j * kTile;
+          else {
+            const int t0 = (j - w.n_cache_tiles) * kTile;
+            limit = p.Nn - t0;
+            if (p.causal) limit = min(limit, i - t0 + 1);
+          }
+          limit -= col0;
+          uint32_t v0[32], v1[32];
+          load_tile(buf, ph, v0, v1);
+          if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+          if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
+          row_update(v0, v1, limit);
         }
         // merge the two column halves of each row (online-softmax partials), then publish
         if (half == 1) sMerge[s * kTile + r] = make_float4(m_run, Z, W, 0.f);
@@ -610,6 +636,47 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const uint64_t c2c2 = pack2(c2, c2);
         const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s], it_other = w.it0[s ^ 1];
         const bool other_valid = w.sub_valid[s ^ 1];
+        auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
+          EPI_WAIT(bar_sfull + 8 * b, bph);
+          tc_fence_after();
+          const uint32_t t_addr = t_col + (uint32_t)(b * kTile);
+          tc_ld32(t_addr, v0);
+          tc_ld32(t_addr + 32, v1);
+          tc_wait_ld();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * b);
+        };
+        // a_k += sum over this thread's 64 query columns of 2^(c2 s - lse2); every column visible
+        auto col_update = [&](const uint32_t (&v0)[32], const uint32_t (&v1)[32], uint32_t l_addr) {
+#pragma unroll
+          for (int e4 = 0; e4 < 8; ++e4) {
+            const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
+            const uint64_t x0 = fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y));
+            const uint64_t x1 = fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w));
+            const uint64_t x2 = fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y));
+            const uint64_t x3 = fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w));
+            acc01 = add2(acc01, ex2_pair(x0, 4 * e4));
+            acc23 = add2(acc23, ex2_pair(x1, 4 * e4 + 1));
+            acc01 = add2(acc01, ex2_pair(x2, 4 * e4 + 2));
+            acc23 = add2(acc23, ex2_pair(x3, 4 * e4 + 3));
+          }
+        };
+        if (w.sub_valid[0] && w.sub_valid[1] && !(p.causal && w.a_chunk)) {
+          // Steady state (cached keys, or no causal mask): both sub-tiles take every tile of the sequence and nothing is
+          // masked; the ring position advances by two batches per tile.
+          for (int j = 0; j < w.ntiles; ++j) {
+            int own = buf + s, oph = ph;
+            if (own >= kAccBufs) { own -= kAccBufs; oph ^= 1; }
+            uint32_t v0[32], v1[32];
+            load_tile(own, oph, v0, v1);
+            buf += 2;
+            if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
+            const int slot = j % kLseSlots;
+            EPI_WAIT(bar_lse + 8 * slot, (j / kLseSlots) & 1);
+            col_update(v0, v1, sLse + (uint32_t)(slot * kTile + col0) * 4);
+          }
+        } else {
         int it_next = it_first;
         for (int j = 0; j < w.ntiles; ++j) {
           const int it = it_next, slot = j % kLseSlots, lse_parity = (j / kLseSlots) & 1;   // kLseSlots is a power of two
@@ -619,33 +686,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (it < it_mine) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
-          EPI_WAIT(bar_sfull + 8 * buf, ph);
-          tc_fence_after();
-          const uint32_t t_addr = t_col + (uint32_t)(buf * kTile);
           uint32_t v0[32], v1[32];
-          tc_ld32(t_addr, v0);
-          tc_ld32(t_addr + 32, v1);
-          tc_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * buf);
+          load_tile(buf, ph, v0, v1);
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
           EPI_WAIT(bar_lse + 8 * slot, lse_parity);
           const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
           if (first <= 0) {
-#pragma unroll
-            for (int e4 = 0; e4 < 8; ++e4) {
-              const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
-              const uint64_t x0 = fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y));
-              const uint64_t x1 = fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w));
-              const uint64_t x2 = fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y));
-              const uint64_t x3 = fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w));
-              acc01 = add2(acc01, ex2_pair(x0, 4 * e4));
-              acc23 = add2(acc23, ex2_pair(x1, 4 * e4 + 1));
-              acc01 = add2(acc01, ex2_pair(x2, 4 * e4 + 2));
-              acc23 = add2(acc23, ex2_pair(x3, 4 * e4 + 3));
-            }
+            col_update(v0, v1, l_addr);
           } else {
 #pragma unroll
             for (int e4 = 0; e4 < 8; ++e4) {
@@ -659,6 +707,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
               }
             }
           }
+        }
         }
         float q0, q1, q2, q3;
         unpack2(acc01, q0, q1);
