@@ -5,11 +5,14 @@
 //                        accumulator, keeps an online max / sum and writes lse2 = log2 sum_k 2^(c2 s_k).
 //   pass 2 (kPass == 2)  S^T = K Q^T, M = 128 keys per sub-tile: each thread owns one KEY row, the sum over
 //                        queries is thread-local: a_k = sum_{g,i} 2^(c2 s - lse2_i).  No atomics, no shuffles.
-// One CTA holds two stationary 128-row sub-tiles (A operand, 64 KB) and streams 128-row tiles of the other
-// operand (B, 32 KB stages) by TMA; one thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile) into a
-// double-buffered 128-column TMEM accumulator per sub-tile; four 4-warp epilogue groups (sub-tile x column half)
-// drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns, frees the TMEM buffer
-// as soon as its registers hold the data, and merges with its partner thread once, at the end.
+// One CTA holds two stationary 128-row sub-tiles, staged once by the epilogue threads from global memory into tensor
+// memory (tcgen05.st: the A operand of a TS-mode tcgen05.mma, 64 TMEM columns each), and streams 128-row tiles of the
+// other operand (B, six 32 KB stages) by TMA; one elected thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile and
+// sub-tile) into a ring of three 128-column TMEM accumulators shared by both sub-tiles; four 4-warp epilogue groups
+// (sub-tile x column half) drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns,
+// frees the TMEM buffer as soon as its registers hold the data, and merges with its partner thread once, at the end.
+// The epilogue is bound by the MUFU ex2 pipe and by instruction dispatch: 2 of every 8
+// exponential pairs run as a packed fp32x2 polynomial on the FMA pipe, and the tile loops carry as little else as possible.
 // Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-19 = epilogue.
 #include <cuda.h>
 #include <math.h>
