@@ -4,6 +4,8 @@ north_star matching rules: (a) scores, entropies, budgets within 2e-3 relative (
 (b) selection and compaction bit-exact when fed the oracle's score array; (c) end-to-end kept-index sets
 identical except where adjacent scores differ by less than that tolerance.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -494,3 +496,30 @@ def test_time_interleaved_chunk():
     eng.compress_chunk_host(src, host_chunk, stage, B, dst2, hM_v, hM_a)
     assert torch.equal(dst2.n, dst.n) and torch.equal(dst2.k, dst.k) and torch.equal(dst2.v, dst.v)
     eng.close()
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("OMNIMEM_FUZZ_SEEDS", "8"))))
+def test_random_shapes_fuzz(seed):
+    """Seeded random shapes around the tile edges (128-row tiles, 256-row CTAs, the 16-slot lse ring, ragged caches,
+    tiny budgets, strides, both modalities possibly empty, optional interleaving / shared selection): rules (a)-(c)."""
+    g = np.random.default_rng(1000 + seed)
+    for rep in range(4):
+        bf16 = bool(g.integers(0, 2))
+        Hkv = int(g.integers(1, 4))
+        G = int(g.choice([1, 2, 4, 7]))
+        big = rep == 3                                     # one larger case per seed: several CTAs along x, > 16 tiles
+        Nn_v, Nn_a = int(g.integers(0, 1400 if big else 600)), int(g.integers(0, 200))
+        if Nn_v + Nn_a == 0:
+            Nn_v = 1
+        n_v, n_a = int(g.integers(0, 2600 if big else 900)), int(g.integers(0, 300))
+        cap = n_v + n_a + int(g.integers(0, 64))
+        budget = int(g.integers(1, max(2, cap + 1)))
+        cap = max(cap, budget, 1)
+        base = SMALL3 if bf16 else I.CFG1
+        wl = base.replace(L=int(g.integers(1, 3)), Hq=Hkv * G, Hkv=Hkv, n_v=n_v, n_a=n_a, Nn_v=Nn_v, Nn_a=Nn_a, budget=budget,
+                          cache_cap=cap, sim_stride_v=int(g.choice([1, 1, 16, 256])), sim_stride_a=int(g.choice([1, 3])))
+        causal = int(g.integers(0, 2))
+        scope = int(g.integers(0, 2))
+        mod = I.modality_pattern(wl, int(g.integers(1, 12))) if g.integers(0, 2) and Nn_v and Nn_a else None
+        check_step(wl, eng_kw=dict(causal=causal), ref_kw=dict(causal=causal), select_scope=scope, modality=mod,
+                   check_rowH=bool(g.integers(0, 2)))
