@@ -45,6 +45,10 @@ constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers +
 #define OMNIMEM_CLUSTER 1
 #endif
 constexpr int kCluster = OMNIMEM_CLUSTER;   // 1 or 2
+#ifndef OMNIMEM_LAZY_MAX
+#define OMNIMEM_LAZY_MAX 1
+#endif
+constexpr bool kLazyMax = OMNIMEM_LAZY_MAX != 0;   // pass 1: running reference instead of a per-tile maximum (see the loop)
 
 // ---- PTX wrappers -------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -587,14 +591,67 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         // Steady state: tiles that lie fully inside the cache are taken by both sub-tiles and need no mask, so the ring
         // position advances by two batches per tile and the loop carries no other bookkeeping.
         const int n_simple = (w.sub_valid[0] && w.sub_valid[1]) ? min(n / kTile, w.ntiles) : 0;
+        // Lazy reference (kLazyMax): the exponentials of a steady-state tile are taken against the running reference
+        // m_run AS IT STANDS -- no tile maximum, no rescale of Z -- which is exact as long as nothing overflows (fp32
+        // sums are scale-free; m_run only has to stay within ~2^100 of the row maximum).  Each warp then votes on
+        // "tile sum and Z finite and below 2^100"; a warp that fails (first tile of a row, or a jump of the maximum by
+        // more than 100 in the log2 domain) discards its tile sums, re-reads the tile from tensor memory (the buffer is
+        // released only after the vote) and takes the exact path, which also re-bases m_run and Z.
         for (; j < n_simple; ++j) {
           int own = buf + s, oph = ph;
           if (own >= kAccBufs) { own -= kAccBufs; oph ^= 1; }
-          uint32_t v0[32], v1[32];
-          load_tile(own, oph, v0, v1);
           buf += 2;
           if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
-          row_update(v0, v1, kHalf);
+          uint32_t v0[32], v1[32];
+          if (!kLazyMax || kEntropy) {
+            load_tile(own, oph, v0, v1);
+            row_update(v0, v1, kHalf);
+            continue;
+          }
+          EPI_WAIT(bar_sfull + 8 * own, oph);
+          tc_fence_after();
+          const uint32_t t_addr = t_col + (uint32_t)(own * kTile);
+          tc_ld32(t_addr, v0);
+          tc_ld32(t_addr + 32, v1);
+          tc_wait_ld();
+          // the polynomial exponentials are only valid up to 2^127 and, unlike the MUFU ones, do not overflow to inf:
+          // their largest raw score takes part in the vote (c2 > 0)
+          float pmax = -INFINITY;
+#pragma unroll
+          for (int pi = 0; pi < 32; ++pi)
+            if (pair_is_poly(pi)) {
+              const uint32_t* v = pi < 16 ? v0 : v1;
+              pmax = fmaxf(pmax, fmaxf(__uint_as_float(v[(2 * pi) & 31]), __uint_as_float(v[(2 * pi + 1) & 31])));
+            }
+          uint64_t z01 = 0ull, z23 = 0ull;
+          const uint64_t c2c2 = pack2(c2, c2), nm = pack2(-m_run, -m_run);
+#pragma unroll
+          for (int e = 0; e < 32; e += 4) {
+            z01 = add2(z01, ex2_pair(fma2(pack2u(v0[e], v0[e + 1]), c2c2, nm), e / 2));
+            z23 = add2(z23, ex2_pair(fma2(pack2u(v0[e + 2], v0[e + 3]), c2c2, nm), e / 2 + 1));
+          }
+#pragma unroll
+          for (int e = 0; e < 32; e += 4) {
+            z01 = add2(z01, ex2_pair(fma2(pack2u(v1[e], v1[e + 1]), c2c2, nm), 16 + e / 2));
+            z23 = add2(z23, ex2_pair(fma2(pack2u(v1[e + 2], v1[e + 3]), c2c2, nm), 16 + e / 2 + 1));
+          }
+          float z0, z1, z2, z3;
+          unpack2(z01, z0, z1);
+          unpack2(z23, z2, z3);
+          const float zt = (z0 + z1) + (z2 + z3);
+          const bool ok = zt < 1.2676506e30f && Z < 1.2676506e30f &&   // 2^100; false for inf and NaN too
+                          fmaf(pmax, c2, -m_run) < 100.f;
+          if (__all_sync(0xffffffffu, ok)) {
+            Z += zt;
+          } else {
+            tc_ld32(t_addr, v0);   // the fast path consumed the registers in place
+            tc_ld32(t_addr + 32, v1);
+            tc_wait_ld();
+            row_update(v0, v1, kHalf);
+          }
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * own);
         }
         for (; j < w.ntiles; ++j) {   // last cache tile, chunk tiles (causal edge), sub-tiles of unequal length
           if (s == 1 && j < nt0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
