@@ -172,7 +172,10 @@ OMNIMEM_API int omnimem_select(omnimem_ctx* ctx, const float* psi_v, const float
 /* ---- stage 5: prune / gather-compaction ---------------------------------------------------------- */
 /* dst[l,h,0:M_v] = visual rows idx_v, dst[l,h,M_v:M_v+M_a] = audio rows idx_a, K and V, byte-exact;
  * dst->n_v[l] = M_v[l], dst->n[l] = M_v[l] + M_a[l].  dst buffers must not alias src's (INVALID_ARG if
- * dst->k == src->k or dst->v == src->v): the caller ping-pongs two caches. */
+ * dst->k == src->k or dst->v == src->v): the caller ping-pongs two caches.  With sim_source == 2 the retained hidden
+ * states follow the kept tokens too: dst->h[l, j] = the hidden row of the j-th kept token of layer l (head 0's index
+ * list; select_scope == 1 makes every head's list the same).  chunk->modality, when set, is honoured (R25').
+ * The context's small device scratch for the interleaving maps is reused by every call: one stream per context. */
 OMNIMEM_API int omnimem_compact(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, const int32_t* idx_v,
                     const int32_t* idx_a, const int32_t* M_v, const int32_t* M_a, omnimem_cache* dst, void* stream);
 
