@@ -416,7 +416,8 @@ def test_hidden_state_redundancy_variant():
     retained hidden states compacted with the kept tokens.  Needs select_scope = 1.  Rules (a)/(c) on the fused step,
     byte-exact K/V/H rows, and a second free-running step on the compacted state."""
     from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem, OmniMemError
-    for wl, d_model in ((I.CFG1, 96), (SMALL3.replace(Hq=8, Hkv=4), 328)):       # 328 * 2 B = 656 B: ragged 512-byte steps
+    for wl, d_model in ((I.CFG1, 96), (SMALL3.replace(Hq=8, Hkv=4), 328),        # 328 * 2 B = 656 B: ragged 512-byte steps
+                        (SMALL2.replace(Hq=8, Hkv=4), 328), (SMALL2, 3584)):      # neighbour distance 1: the streaming kernel
         tol = TOL[wl.dtype]
         L = wl.L
         p = ref_params(wl, L)
