@@ -524,3 +524,32 @@ def test_random_shapes_fuzz(seed):
         mod = I.modality_pattern(wl, int(g.integers(1, 12))) if g.integers(0, 2) and Nn_v and Nn_a else None
         check_step(wl, eng_kw=dict(causal=causal), ref_kw=dict(causal=causal), select_scope=scope, modality=mod,
                    check_rowH=bool(g.integers(0, 2)))
+
+
+def test_fused_step_captures_into_a_cuda_graph():
+    """The fused call only enqueues work on the given stream (no host synchronisation, no allocation): it can be
+    captured once and replayed; the replay must reproduce the eager result byte for byte, also after the inputs changed."""
+    for wl in (I.CFG1, SMALL2):
+        eng = engine_for(wl)
+        x = I.full_inputs(wl)
+        src, chunk = dev_objs(x, wl)
+        B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device="cuda")
+        dst_e, dst_g = eng.new_cache(), eng.new_cache()
+        eng.compress_chunk(src, chunk, B, dst_g)                      # warm-up outside the capture (attributes, tensor maps)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            eng.compress_chunk(src, chunk, B, dst_g)
+        for step in (0, 1):
+            if step:                                                  # new chunk contents in the SAME buffers
+                y = I.full_inputs(wl, step=1)
+                chunk.k.copy_(y["chunkK"].cuda()); chunk.v.copy_(y["chunkV"].cuda()); chunk.q.copy_(y["Q"].cuda())
+            dst_g.k.zero_(); dst_g.v.zero_()
+            g.replay()
+            eng.compress_chunk(src, chunk, B, dst_e)
+            torch.cuda.synchronize()
+            assert torch.equal(dst_g.n, dst_e.n) and torch.equal(dst_g.n_v, dst_e.n_v)
+            for l in range(wl.L):
+                nl = int(dst_e.n[l])
+                assert torch.equal(dst_g.k[l, :, :nl], dst_e.k[l, :, :nl]) and torch.equal(dst_g.v[l, :, :nl], dst_e.v[l, :, :nl])
+        eng.close()
