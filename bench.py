@@ -373,7 +373,7 @@ def run_stream(args, wl: I.Workload, local_rank: int):
 
 
 # per-launch DRAM bytes of the scoring kernels from the committed ncu --set full capture (profiles/); None = not captured
-NCU_TRAFFIC_BYTES = {"colsum": 1.7925e9, "lse": 1.7778e9}   # profiles/r01c_score_tc_full_cfg2.csv (CFG2 only)
+NCU_TRAFFIC_BYTES = {"colsum": 1.7913e9, "lse": 1.7789e9}   # profiles/r01c_score_tc_full_cfg2.csv (CFG2 only)
 
 
 def main():
