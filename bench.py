@@ -306,6 +306,8 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     t_one_pass /= args.steps
     out["supplied_lse"] = {"ms_per_step": t_one_pass * 1e3, "value": job_value(world, work["Nk"], t_one_pass), "unit": "KV tok/s",
                            "note": "row LSE supplied by the caller (chunk.lse): scoring pass 1 skipped; context, not the headline"}
+    out["derived"] = {"ingest_tok_per_s": world * wl.Nn / t_step, "layer_entries_per_s": world * wl.L * work["Nk"] / t_step,
+                      "note": "SURVEY.md 8(d): chunk tokens ingested per second; (layer, KV entry) pairs scored and compacted per second"}
     if t_graph is not None:
         out["cuda_graph"] = {"ms_per_step": t_graph / args.steps * 1e3,
                              "note": "one omnimem_compress_chunk captured once and replayed (no profiling events)"}
