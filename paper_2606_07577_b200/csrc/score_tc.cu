@@ -25,7 +25,7 @@ constexpr int kTile = 128;         // rows per operand tile (UMMA M and N)
 constexpr int kHeadDim = 128;      // D
 constexpr int kKBlock = 64;        // bf16 elements per 128-byte swizzle atom row
 constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16 KB K-blocks
-constexpr int kKBlockBytes = kTile * kKBlock * 2; // 16 KB
+
 constexpr int kStages = 6;          // B ring (32 KB stages)
 constexpr int kThreads = 640;       // 4 control warps + 16 epilogue warps (4 groups: sub-tile x column half)
 constexpr int kTmemCols = 512;
@@ -38,13 +38,19 @@ constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 
 constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
-// Two CTAs of a cluster (one TPC) work on neighbouring stationary blocks and stream the SAME tiles: each loads one
-// 64-column K-block of every tile and multicasts it into both shared memories, which halves the L2 -> SM read traffic
-// of the streamed operand (96 GB per pass at CFG2; its removal was worth ~8 % of a pass under the power cap).
+// OMNIMEM_CLUSTER == 2: the two CTAs of a cluster (one TPC) take neighbouring stationary blocks, stream ONE tile
+// sequence (the union of what both need) and run it as tcgen05.mma.cta_group::2: M = 256 (128 stationary rows of
+// each CTA, out of its own tensor memory), N = 128 with each CTA holding HALF of every streamed tile (64 rows, 16 KB)
+// in its shared memory.  That halves the L2 -> SM traffic, the shared-memory writes and the tensor-pipe reads of the
+// streamed operand.  Only the leader CTA (rank 0) issues MMAs; completion is multicast to both CTAs' barriers; the
+// peer's "my half has landed", "stationary rows staged" and "accumulator read" signals reach the leader's barriers
+// by remote mbarrier arrives.
 #ifndef OMNIMEM_CLUSTER
 #define OMNIMEM_CLUSTER 1
 #endif
 constexpr int kCluster = OMNIMEM_CLUSTER;   // 1 or 2
+constexpr int kRowsB = 128 / kCluster;       // rows of a streamed tile in this CTA's shared memory
+constexpr int kKBlockBytesB = kRowsB * 128;  // one 64-element K-block of them
 #ifndef OMNIMEM_LAZY_MAX
 #define OMNIMEM_LAZY_MAX 1
 #endif
@@ -82,15 +88,32 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
           "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar,
-                                               uint16_t cta_mask) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, "
-      "%3, %4}], [%5], %6;" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "h"(cta_mask) : "memory");
+// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t bar, uint32_t rank) {
+  uint32_t remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
 }
-__device__ __forceinline__ void tc_commit_mc(uint32_t bar, uint16_t cta_mask) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
-               "h"(cta_mask) : "memory");
+// wait that also acquires what other CTAs of the cluster released (remote arrives)
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAITC_LOOP:\n\t"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1, %2;\n\t"
+      "@p bra WAITC_DONE;\n\t"
+      "bra WAITC_LOOP;\n\t"
+      "WAITC_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+}
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {   // both CTAs' barriers at this offset
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+               "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16_ts_pair(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
+      "r"(acc) : "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -253,6 +276,7 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   return d;
 }
 // Instruction descriptor: D = f32 (bit 4), A = B = bf16 (bits 7, 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
+constexpr uint32_t kIdescPair = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(2 * kTile >> 4) << 24);  // M = 256
 constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
 
 struct TcArgs {
@@ -279,6 +303,9 @@ struct Work {
   // pass 2
   int it0[2], tiles_per_g, hq0;
   int seq0;              // first query tile of the streamed sequence (== it0[0] unless a cluster peer starts earlier)
+  // pair level (== the CTA's own values without a cluster): which batches exist for sub-tile s
+  int ntp[2], it0p[2];
+  bool validp[2];
 };
 
 template <int kPass>
@@ -342,20 +369,34 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const StepParams& p = a.p;
   Work w;
   const bool mine = make_work<kPass>(a, w, (int)blockIdx.x);
+  // Pair level (kCluster == 2): the two CTAs stream one sequence, the union of what they need, and every MMA covers
+  // sub-tile s of BOTH.  ntp[s] (pass 1) / it0p[s], validp[s] (pass 2) say which batches exist; a CTA whose own sub-tile
+  // does not take a batch still has to release the accumulator ("ghost" consumption in the epilogue).
+  int peer_stage_warps = 0;
   if (kCluster == 2) {
-    // the pair streams one sequence: the union of what its two CTAs need (a CTA skips the tiles that are not its own)
     Work wp;
     const bool peer = make_work<kPass>(a, wp, (int)blockIdx.x ^ 1);
     if (!mine && !peer) return;           // uniform across the cluster
+    for (int s = 0; s < 2; ++s) {
+      if (kPass == 1) {
+        w.ntp[s] = max(w.sub_valid[s] ? w.ntiles_sub[s] : 0, wp.sub_valid[s] ? wp.ntiles_sub[s] : 0);
+      } else {
+        w.it0p[s] = min(w.sub_valid[s] ? w.it0[s] : 1 << 30, wp.sub_valid[s] ? wp.it0[s] : 1 << 30);
+      }
+      w.validp[s] = w.sub_valid[s] || wp.sub_valid[s];
+      peer_stage_warps += wp.sub_valid[s] ? 8 : 0;
+    }
     if (kPass == 1) {
-      w.ntiles = max(mine ? w.ntiles : 0, peer ? wp.ntiles : 0);
+      w.ntiles = max(w.ntp[0], w.ntp[1]);
     } else {
-      w.seq0 = min(mine ? w.seq0 : 1 << 30, peer ? wp.seq0 : 1 << 30);
+      w.seq0 = min(w.it0p[0], w.it0p[1]);
       w.tiles_per_g = (p.Nn + kTile - 1) / kTile - w.seq0;
       w.ntiles = p.G * w.tiles_per_g;
     }
-  } else if (!mine) {
-    return;                               // uniform across the CTA
+  } else {
+    if (!mine) return;                    // uniform across the CTA
+    // (set AFTER the early exit: written before it, ptxas stopped using the uniform datapath in the tile loops)
+    for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
   }
   const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
 #ifdef OMNIMEM_DBG_MAXTILES   // timing experiment only: cap the streamed sequence to expose the per-CTA fixed cost
@@ -375,19 +416,29 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages, bar_a = bar_empty + 8 * kStages;
   const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
   const uint32_t bar_lse = bar_sempty + 8 * kAccBufs;                           // [kLseSlots]
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots);
+  const uint32_t bar_pfull = bar_lse + 8 * kLseSlots;                           // [kStages] leader only: the peer's half of a stage has landed
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots + 8 * kStages);
+  const bool leader = cta_rank == 0;
+  const int my_stage_warps = (w.sub_valid[0] ? 8 : 0) + (w.sub_valid[1] ? 8 : 0);
 
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, kCluster); }
-    mbar_init(bar_a, w.sub_valid[1] ? 16 : 8);  // one arrival per epilogue warp that stages stationary rows
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); mbar_init(bar_pfull + 8 * s, 1); }
+    // one arrival per epilogue warp that stages stationary rows (the leader also collects the peer's, remotely)
+    mbar_init(bar_a, max(1, my_stage_warps + (kCluster == 2 ? peer_stage_warps : 0)));
+    // an accumulator buffer is free when the 8 warps of its sub-tile's group have read it -- in BOTH CTAs for a pair
+    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8 * kCluster); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (kCluster == 2) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tc_fence_before();
   __syncthreads();
@@ -424,7 +475,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       continue;
 #endif
       if (elect_one()) {
-        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
+        mbar_expect_tx(bar_full + 8 * stage, kTileBytes / kCluster);
         if (kPass == 2) {
           // lse2 of these 128 queries: its own ring + barrier.  Slot j % 16 was last read for tile j - 16; this load is
           // issued only after the MMAs of tile j - kStages completed, which needed the accumulator of a batch at most 3
@@ -433,34 +484,43 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
           bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
         }
-        if (kCluster == 2) {
-          const int kb = (int)cta_rank;   // this CTA's K-block, delivered to both CTAs; the peer sends the other one
-          tma_load_3d_mc(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage, 3);
-        } else {
-          for (int kb = 0; kb < 2; ++kb)
-            tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
-        }
+        // pair: this CTA's 64 rows of the tile (the peer loads the other 64 into ITS shared memory)
+        for (int kb = 0; kb < 2; ++kb)
+          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytesB, mB, kb * kKBlock, row0 + (int)cta_rank * kRowsB, lh,
+                      bar_full + 8 * stage);
       }
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
       if (++slot == kLseSlots) slot = 0;
     }
     if (kCluster == 2) {
-      // drain: every stage released by BOTH CTAs, i.e. no remote arrival is still on its way to this CTA's barriers
+      // drain: the leader's last commits have reached this CTA's barriers before anybody leaves
       for (int j = max(0, w.ntiles - kStages); j < w.ntiles; ++j) mbar_wait(bar_empty + 8 * (j % kStages), (j / kStages) & 1);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (mine) mbar_wait(bar_a, 0);  // stationary rows are in TMEM (a CTA that only serves its peer has none)
+    if (kCluster == 2 && !leader) {
+      // peer of a pair: no MMAs of its own; it tells the leader when its half of a stage has landed
+      int stage = 0, sph = 0;
+      for (int j = 0; j < w.ntiles; ++j) {
+        mbar_wait(bar_full + 8 * stage, sph);
+        if (elect_one()) mbar_arrive_remote(bar_pfull + 8 * stage, 0);
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; sph ^= 1; }
+      }
+    } else {
+    if (kCluster == 2) { if (my_stage_warps + peer_stage_warps > 0) mbar_wait_cluster(bar_a, 0); }
+    else if (mine) mbar_wait(bar_a, 0);  // stationary rows are in TMEM
     tc_fence_after();
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
     int it = kPass == 2 ? w.seq0 : 0, stage = 0, sph = 0;
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_full + 8 * stage, sph);
+      if (kCluster == 2) mbar_wait_cluster(bar_pfull + 8 * stage, sph);
       tc_fence_after();
       for (int s = 0; s < 2; ++s) {
-        if (!(kPass == 1 ? j < w.ntiles_sub[s] : (w.sub_valid[s] && it >= w.it0[s]))) continue;
-        mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
+        if (!(kPass == 1 ? j < w.ntp[s] : (w.validp[s] && it >= w.it0p[s]))) continue;
+        if (kCluster == 2) mbar_wait_cluster(bar_sempty + 8 * buf, ph ^ 1); else mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
         const uint32_t a_tmem = tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2));
@@ -469,20 +529,22 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
             // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
-            const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
+            const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytesB + (kk & 3) * 32) >> 4);
 #ifndef OMNIMEM_DBG_NOMMA
-            tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, OMNIMEM_DBG_ACC(kk));
+            if (kCluster == 2) tc_mma_bf16_ts_pair(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdescPair, OMNIMEM_DBG_ACC(kk));
+            else tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, OMNIMEM_DBG_ACC(kk));
 #endif
           }
-          tc_commit(bar_sfull + 8 * buf);
+          if (kCluster == 2) tc_commit_pair(bar_sfull + 8 * buf); else tc_commit(bar_sfull + 8 * buf);
         }
         __syncwarp();
         if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
       }
-      if (elect_one()) { if (kCluster == 2) tc_commit_mc(bar_empty + 8 * stage, 3); else tc_commit(bar_empty + 8 * stage); }
+      if (elect_one()) { if (kCluster == 2) tc_commit_pair(bar_empty + 8 * stage); else tc_commit(bar_empty + 8 * stage); }
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
       if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
+    }
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
@@ -493,7 +555,32 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     const int r = q4 * 32 + lane;        // row of the sub-tile == TMEM lane
     const int col0 = half * kHalf;
     const float c2 = p.scale_log2e;
-    if (w.sub_valid[s]) {
+    // "this warp has read accumulator buffer b": the leader of a pair collects its peer's arrivals remotely
+    auto release = [&](int b) {
+      if (lane == 0) {
+        if (kCluster == 2 && !leader) mbar_arrive_remote(bar_sempty + 8 * b, 0);
+        else EPI_ARRIVE(bar_sempty + 8 * b);
+      }
+    };
+    if (!w.sub_valid[s]) {
+      // pair only: this CTA has no rows in sub-tile s but its peer does; every MMA still writes this CTA's accumulator
+      // buffer, which has to be handed back in ring order
+      if (kCluster == 2 && (s == 0 ? w.validp[0] : w.validp[1])) {
+        int buf = 0, ph = 0, it = kPass == 2 ? w.seq0 : 0;
+        for (int j = 0; j < w.ntiles; ++j) {
+          const bool tk0 = kPass == 1 ? j < w.ntp[0] : (w.validp[0] && it >= w.it0p[0]);
+          const bool tk1 = kPass == 1 ? j < w.ntp[1] : (w.validp[1] && it >= w.it0p[1]);
+          if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
+          if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
+          if (s == 0 ? tk0 : tk1) {
+            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            release(buf);
+            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+          }
+          if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
+        }
+      }
+    } else {
       const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
       {
         // Stage this thread's share of the stationary operand: row r of the sub-tile, bf16 elements [64 half, 64 half + 64)
@@ -519,7 +606,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar_a);
+        if (lane == 0) { if (kCluster == 2 && !leader) mbar_arrive_remote(bar_a, 0); else mbar_arrive(bar_a); }
       }
       const uint32_t t_col = t_lane + (uint32_t)col0;
       int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile
@@ -527,7 +614,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
         const int n = p.n[w.l];
         float m_run = -1e30f, Z = 0.f, W = 0.f;
-        const int nt0 = w.ntiles_sub[0], nt1 = w.ntiles_sub[1], nt_mine = s == 0 ? nt0 : nt1;
+        const int nt_mine = s == 0 ? w.ntiles_sub[0] : w.ntiles_sub[1];
         // accumulator batch at ring position (b, bph) -> registers; the TMEM buffer is released as soon as they hold it
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
           EPI_WAIT(bar_sfull + 8 * b, bph);
@@ -538,7 +625,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * b);
+          release(b);
         };
         // online softmax statistics of this thread's 64 columns of one tile; limit = visible columns (>= 64: all)
         auto row_update = [&](const uint32_t (&v0)[32], const uint32_t (&v1)[32], int limit) {
@@ -651,11 +738,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           }
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * own);
+          release(own);
         }
+        // selects on the warp-uniform s, not dynamic indexing: a local-memory load would take the ring bookkeeping off the
+        // uniform datapath (it did: +7 % cycles)
+        const int ntp_mine = uniform(s == 0 ? w.ntp[0] : w.ntp[1]), ntp_other = uniform(s == 0 ? w.ntp[1] : w.ntp[0]);
         for (; j < w.ntiles; ++j) {   // last cache tile, chunk tiles (causal edge), sub-tiles of unequal length
-          if (s == 1 && j < nt0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
-          if (j >= nt_mine) { if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          const bool tk_mine = j < ntp_mine, tk_other = j < ntp_other;   // the batches of tile j that exist (pair level)
+          const bool tk0 = s == 0 ? tk_mine : tk_other, tk1 = s == 0 ? tk_other : tk_mine;
+          if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
+          if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          if (kCluster == 2 && j >= nt_mine) {   // the peer's rows take this tile, mine do not: hand the buffer back unread
+            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            release(buf);
+            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+            if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
+            continue;
+          }
           // number of visible key columns of this tile for this row, relative to this thread's first column
           int limit;
           if (j < w.n_cache_tiles) limit = n - j * kTile;
@@ -668,7 +767,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           uint32_t v0[32], v1[32];
           load_tile(buf, ph, v0, v1);
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-          if (s == 0 && j < nt1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
+          if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }    // sub-tile 1's batch of tile j
           row_update(v0, v1, limit);
         }
         // merge the two column halves of each row (online-softmax partials), then publish
@@ -694,8 +793,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         uint64_t acc01 = 0ull, acc23 = 0ull;   // packed fp32x2 partial sums of the unmasked tiles
         const uint64_t c2c2 = pack2(c2, c2);
-        const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s], it_other = w.it0[s ^ 1];
-        const bool other_valid = w.sub_valid[s ^ 1];
+        const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s];
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
           EPI_WAIT(bar_sfull + 8 * b, bph);
           tc_fence_after();
@@ -705,7 +803,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           tc_wait_ld();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) EPI_ARRIVE(bar_sempty + 8 * b);
+          release(b);
         };
         // a_k += sum over this thread's 64 query columns of 2^(c2 s - lse2); every column visible
         auto col_update = [&](const uint32_t (&v0)[32], const uint32_t (&v1)[32], uint32_t l_addr) {
@@ -738,12 +836,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           }
         } else {
         int it_next = it_first;
+        const int it0p_mine = uniform(s == 0 ? w.it0p[0] : w.it0p[1]), it0p_other = uniform(s == 0 ? w.it0p[1] : w.it0p[0]);
+        const bool validp_mine = uniform(s == 0 ? w.validp[0] : w.validp[1]) != 0, validp_other = uniform(s == 0 ? w.validp[1] : w.validp[0]) != 0;
         for (int j = 0; j < w.ntiles; ++j) {
           const int it = it_next, slot = j % kLseSlots, lse_parity = (j / kLseSlots) & 1;   // kLseSlots is a power of two
           if (++it_next == it_end) it_next = it_first;                                       // no division in the tile loop
-          const bool other = other_valid && it >= it_other;
+          const bool tk_mine = validp_mine && it >= it0p_mine, tk_other = validp_other && it >= it0p_other;   // pair level
+          const bool tk0 = s == 0 ? tk_mine : tk_other, tk1 = s == 0 ? tk_other : tk_mine;
+          const bool other = s == 0 ? tk1 : tk0;
           if (s == 1 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j comes first
-          if (it < it_mine) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
+          if (kCluster == 2 && it < it_mine) {   // the peer's keys see this query tile, mine do not yet: hand the buffer back unread
+            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            release(buf);
+            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+            if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
+            continue;
+          }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
           uint32_t v0[32], v1[32];
@@ -794,7 +903,8 @@ done:
   if (kCluster == 2) cluster_sync_all();   // nobody leaves while the peer may still write into this CTA
   if (warp == 2) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    if (kCluster == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
   }
 }
 
@@ -830,7 +940,7 @@ static cudaError_t make_map(EncodeTiledFn enc, CUtensorMap* m, const void* base,
   if (rows == 0 || outer == 0 || base == nullptr) { memset(m, 0, sizeof(*m)); return cudaSuccess; }
   const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, outer};
   const cuuint64_t strides[2] = {(cuuint64_t)kHeadDim * 2, rows * kHeadDim * 2};
-  const cuuint32_t box[3] = {(cuuint32_t)kKBlock, (cuuint32_t)kTile, 1};
+  const cuuint32_t box[3] = {(cuuint32_t)kKBlock, (cuuint32_t)kRowsB, 1};   // a CTA of a pair loads half of the tile's rows
   const cuuint32_t es[3] = {1, 1, 1};
   const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
