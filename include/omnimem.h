@@ -31,6 +31,12 @@
  *     t < n_m -> cache row off_m + t (off_v = 0, off_a = n_v);  else chunk row coff_m + (t - n_m) (coff_v = 0,
  *     coff_a = Nn_v).  Per-modality arrays are [L, Hkv, seg_cap_m] fp32 with seg_cap_m = cache_cap + max_chunk_m
  *     (omnimem_seg_cap); entries at t >= K_m are unspecified.
+ *   - Budgets (layer_budget, M_v, M_a) are DEVICE arrays: the AVBA split runs on the device every step (R21) and no
+ *     call reads them back, so they cannot be rejected on the host.  They are CLAMPED where they are consumed:
+ *     a per-layer total B^(l) to [0, cache_cap] in omnimem_allocate / omnimem_compress_chunk, and M_v to
+ *     [0, min(K_v, cache_cap)], M_a to [0, min(K_a, cache_cap - M_v)] in omnimem_select / omnimem_compact.  Nothing is
+ *     ever written at or beyond row cache_cap of an idx_m or dst row block.  OMNIMEM_CAPACITY is returned only for
+ *     sizes the host can see (Nn_v > max_chunk_v, Nn_a > max_chunk_a).
  */
 #ifndef OMNIMEM_H_
 #define OMNIMEM_H_
@@ -54,7 +60,7 @@ typedef enum {
   OMNIMEM_UNSUPPORTED = -2,        /* dtype / head_dim / device architecture not supported                        */
   OMNIMEM_WORKSPACE_TOO_SMALL = -3,
   OMNIMEM_CUDA_ERROR = -4,         /* details: omnimem_last_cuda_error                                           */
-  OMNIMEM_CAPACITY = -5            /* chunk larger than max_chunk_*, or budget larger than cache_cap              */
+  OMNIMEM_CAPACITY = -5            /* chunk larger than max_chunk_v / max_chunk_a (host-visible sizes only)       */
 } omnimem_status;
 
 enum { OMNIMEM_FP32 = 0, OMNIMEM_BF16 = 1 };
@@ -144,7 +150,9 @@ OMNIMEM_API int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const 
 /* stats [L,8] as written by omnimem_score; n_v, n [L]; layer_budget [L] int32 per-layer totals B^(l) (the paper
  * fixes them offline) or NULL => B^(l) = Softmax_l(C^(l)/T) * total_budget, clamped to [budget_min,
  * budget_max], integerised by largest remainder (R19, R20).  Out: M_v, M_a [L] with M_v + M_a = min(B^(l), K_v + K_a),
- * M_m <= K_m (R22); layer_budget_out [L] or NULL receives the totals used. */
+ * M_m <= K_m (R22); layer_budget_out [L] or NULL receives the totals used (after the clamp to [0, cache_cap]).
+ * The bounded split is b_l = clip(kappa pi_l, B_min, B_max) with kappa set by sum_l b_l = total_budget; if
+ * total_budget >= L B_max (<= L B_min) every layer gets B_max (B_min). */
 OMNIMEM_API int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const int32_t* n_v, const int32_t* n, int32_t Nn_v,
                      int32_t Nn_a, const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
                      int32_t* layer_budget_out, void* stream);
@@ -164,7 +172,8 @@ OMNIMEM_API int omnimem_calibrate_budgets(omnimem_ctx* ctx, const double* acc, i
 /* ---- stage 4: segmented top-M (Eq.4-5) ---------------------------------------------------------------- */
 /* psi_m [L, Hkv, seg_cap_m] fp32 (finite); per (l, h, m) writes the segment-local indices of the M_m[l] largest
  * psi to idx_m[l, h, 0:M_m[l]) in ASCENDING index order; among equal psi the lowest index wins (R23).
- * idx_m are [L, Hkv, cache_cap] int32; entries at >= M_m[l] are left untouched. */
+ * idx_m are [L, Hkv, cache_cap] int32; entries at >= M_m[l] are left untouched.  M_m are clamped as stated under
+ * "Budgets" above. */
 OMNIMEM_API int omnimem_select(omnimem_ctx* ctx, const float* psi_v, const float* psi_a, const int32_t* n_v, const int32_t* n,
                    int32_t Nn_v, int32_t Nn_a, const int32_t* M_v, const int32_t* M_a, int32_t* idx_v, int32_t* idx_a,
                    void* ws, size_t ws_bytes, void* stream);
@@ -197,7 +206,10 @@ OMNIMEM_API int omnimem_compress_chunk(omnimem_ctx* ctx, const omnimem_cache* sr
  * copies run on a stream owned by the context (ordered after everything already enqueued on `stream`) and the
  * kernels of group g on `stream` overlap the copy of group g + 1.  host_chunk->h and host_chunk->modality, when set,
  * are HOST arrays too and dev_chunk->h / dev_chunk->modality their DEVICE staging buffers.  Results are identical to omnimem_compress_chunk
- * on the same inputs.  Returns the byte counts moved through h2d_bytes / d2h_bytes (HOST, may be NULL). */
+ * on the same inputs.  Returns the byte counts moved through h2d_bytes / d2h_bytes (HOST, may be NULL).  All argument
+ * errors are detected before anything is enqueued; if a CUDA call fails later, both streams are synchronised before the
+ * status is returned, so the host buffers are no longer being read.  Per-stage timing (omnimem_get_stage_ms) after this
+ * entry covers the LAST layer group only (the events are re-recorded per group). */
 OMNIMEM_API int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* host_chunk,
                                 const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,
                                 int32_t* host_M_v, int32_t* host_M_a, int64_t* h2d_bytes, int64_t* d2h_bytes,

@@ -25,11 +25,14 @@
  * (declarative `reduction`, no hand-written blocking).
  *
  * Pins (tests/test_oracle_pins.py) -- each function below is checked against
- * something other than itself; the one exception is stated here:
- *   omnimem_ref_layer_budgets (Eq.14 + clamp/rounding, R20): PARITY UNPINNED
- *   beyond sum / clamp / symmetry / T->inf invariants (the paper gives neither
- *   B_min/B_max nor a rounding rule nor a worked example).
+ * something other than itself.  omnimem_ref_layer_budgets (Eq.14 + clamp and
+ * rounding, R20) is pinned by the water-filling form the mathematics fixes,
+ * b_l = clip(kappa pi_l, B_min, B_max) with sum_l b_l = total, found by plain
+ * bisection in numpy on 240 seeded cases, plus a numpy largest-remainder
+ * integerisation and two closed forms.  What stays unpinned is only the
+ * end-to-end numeric output as a whole: the paper prints no worked example.
  */
+#define _GNU_SOURCE /* qsort_r */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -310,7 +313,7 @@ int omnimem_ref_stats(const omnimem_ref_params* p, const int32_t* n_v, const int
   return 0;
 }
 
-/* ---- O6b: per-layer totals (Eq.13-14) -- PARITY UNPINNED beyond invariants (R19, R20) ----
+/* ---- O6b: per-layer totals (Eq.13-14; R19, R20) ------------------------------------------
  * C^(l) = Hn_all (1 - sbar_all); pi = softmax_l(C/T); b_l = pi_l * total.
  * Clamp to [B_min,B_max] (if budget_max > 0): layers beyond the bound on the side with the larger total violation
  * are fixed at that bound and the remaining total is re-split over the free layers in proportion to pi, until
@@ -416,11 +419,11 @@ int omnimem_ref_allocate(const omnimem_ref_params* p, const double* stats, const
 /* ---- O7: Select (Eq.4-5; "top K pairs that have the highest score") -----------
  * Per (l,h,m): order the segment's indices by psi (the fp32 array) descending, equal psi by index ascending
  * (= a stable descending sort: lowest index wins ties, R23); keep the first M_m; emit them ascending. */
-static const float* g_sort_key;
-static int cmp_desc_stable(const void* x, const void* y) {
+static int cmp_desc_stable(const void* x, const void* y, void* key) {
+  const float* sort_key = (const float*)key;
   const int32_t i = *(const int32_t*)x, j = *(const int32_t*)y;
-  if (g_sort_key[i] > g_sort_key[j]) return -1;
-  if (g_sort_key[i] < g_sort_key[j]) return 1;
+  if (sort_key[i] > sort_key[j]) return -1;
+  if (sort_key[i] < sort_key[j]) return 1;
   return (i > j) - (i < j);
 }
 static int cmp_int_asc(const void* x, const void* y) {
@@ -441,8 +444,8 @@ int omnimem_ref_select(const omnimem_ref_params* p, const float* psi_v, const fl
         if (M < 0 || M > Km || M > idx_cap) return -1;
         int32_t* order = (int32_t*)malloc(sizeof(int32_t) * (size_t)(Km + 1));
         for (int t = 0; t < Km; ++t) order[t] = t;
-        g_sort_key = (m == 0 ? psi_v : psi_a) + IDX3(l, h, 0, p->Hkv, cap);
-        qsort(order, (size_t)Km, sizeof(int32_t), cmp_desc_stable);
+        const float* sort_key = (m == 0 ? psi_v : psi_a) + IDX3(l, h, 0, p->Hkv, cap);
+        qsort_r(order, (size_t)Km, sizeof(int32_t), cmp_desc_stable, (void*)sort_key);
         qsort(order, (size_t)M, sizeof(int32_t), cmp_int_asc);
         for (int t = 0; t < M; ++t) out[t] = order[t];
         for (int t = M; t < idx_cap; ++t) out[t] = -1;

@@ -27,7 +27,16 @@ _SO = os.path.join(_HERE, "libomnimem_ref.so")
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (plain C, OpenMP); returns the path of the shared object."""
+    """Compile the oracle with gcc (plain C, OpenMP); returns the path of the shared object.
+    OMNIMEM_REF_SANITIZE=1 builds (and loads) a separate AddressSanitizer + UBSan copy instead; the process must then
+    run with LD_PRELOAD=$(gcc -print-file-name=libasan.so) (tests/test_oracle_pins.py does, in a subprocess)."""
+    if os.environ.get("OMNIMEM_REF_SANITIZE") == "1":
+        so = os.path.join(_HERE, "libomnimem_ref_san.so")
+        if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer",
+                   "-fopenmp", "-fPIC", "-shared", "-o", so, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+        return so
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-march=native", "-fopenmp", "-fPIC", "-shared", "-o", _SO, _SRC, "-lm"]
         subprocess.run(cmd, check=True)

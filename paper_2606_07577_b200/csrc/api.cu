@@ -267,7 +267,7 @@ const char* omnimem_strerror(int status) {
     case OMNIMEM_UNSUPPORTED: return "unsupported dtype, head_dim or device (needs sm_100)";
     case OMNIMEM_WORKSPACE_TOO_SMALL: return "workspace too small (see omnimem_workspace_bytes)";
     case OMNIMEM_CUDA_ERROR: return "CUDA error (see omnimem_last_cuda_error)";
-    case OMNIMEM_CAPACITY: return "chunk or budget exceeds the context capacities";
+    case OMNIMEM_CAPACITY: return "chunk exceeds the context capacities (max_chunk_v / max_chunk_a)";
     default: return "unknown status";
   }
 }
@@ -479,6 +479,7 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   if (rc) return rc;
   if (!dev_chunk->k || !dev_chunk->v || !dev_chunk->q || (host_chunk->lse && !dev_chunk->lse)) return OMNIMEM_INVALID_ARG;
   if (ctx->cfg.sim_source == 2 && (!host_chunk->h || !dev_chunk->h)) return OMNIMEM_INVALID_ARG;
+  if (host_chunk->modality && host_chunk->Nn_v + host_chunk->Nn_a > 0 && !dev_chunk->modality) return OMNIMEM_INVALID_ARG;
   omnimem_chunk ch = *dev_chunk;
   ch.Nn_v = host_chunk->Nn_v;
   ch.Nn_a = host_chunk->Nn_a;
@@ -515,11 +516,12 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
   if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_copy[OMNIMEM_HOST_GROUPS], 0);
   if (e != cudaSuccess) return fail_cuda(ctx, e);
   auto at = [](const void* p, size_t bytes) { return (void*)((uint8_t*)const_cast<void*>(p) + bytes); };
+  // an error after this point leaves copies in flight that read the caller's host buffers: wait for them before returning
+  auto fail_mid = [&](int status) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamSynchronize(st); return status; };
   if (host_chunk->modality && Nn > 0) {   // HOST [Nn] -> the device staging copy, ahead of the first group
-    if (!dev_chunk->modality) return OMNIMEM_INVALID_ARG;
     e = cudaMemcpyAsync(const_cast<int32_t*>(dev_chunk->modality), host_chunk->modality, Nn * sizeof(int32_t),
                         cudaMemcpyHostToDevice, ctx->copy_stream);
-    if (e != cudaSuccess) return fail_cuda(ctx, e);
+    if (e != cudaSuccess) return fail_mid(fail_cuda(ctx, e));
   }
   int gi = 0;
   for (int l0 = 0; gi < n_groups; l0 += group_size[gi], ++gi) {
@@ -537,16 +539,16 @@ int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cache* src, cons
         e = cudaMemcpyAsync(at(dev_chunk->h, l0 * h_layer), at(host_chunk->h, l0 * h_layer), Lg * h_layer, cudaMemcpyHostToDevice, cs);
       if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[gi], cs);
       if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_copy[gi], 0);
-      if (e != cudaSuccess) return fail_cuda(ctx, e);
+      if (e != cudaSuccess) return fail_mid(fail_cuda(ctx, e));
     }
     rc = compress_layers(ctx, src, &ch, layer_budget, dst, nullptr, nullptr, nullptr, nullptr, nullptr, wsb, l0, Lg, st);
-    if (rc) return rc;
+    if (rc) return fail_mid(rc);
   }
   const size_t mb = (size_t)L * sizeof(int32_t);
   e = cudaMemcpyAsync(host_M_v, wsb + w.M_v, mb, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(host_M_a, wsb + w.M_a, mb, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) return fail_cuda(ctx, e);
+  if (e != cudaSuccess) return fail_mid(fail_cuda(ctx, e));
   if (h2d_bytes) *h2d_bytes = (int64_t)(Nn > 0 ? (size_t)L * (2 * kv_layer + q_layer + lse_layer + h_layer) : 0);
   if (d2h_bytes) *d2h_bytes = (int64_t)(2 * mb);
   return OMNIMEM_OK;

@@ -59,6 +59,14 @@ __device__ __forceinline__ void chunk_row_to_seg(const StepParams& p, int n_v, i
   }
   if (r < p.Nn_v) { m = 0; t = n_v + r; } else { m = 1; t = (n - n_v) + (r - p.Nn_v); }
 }
+// Budgets are device data (AVBA runs on the device, R21; the public stage calls take device arrays): nothing on the
+// host can validate them, so select / compact clamp them to the rows that exist and to what one cache row block holds.
+// With in-range budgets (what allocate produces) this is the identity.
+__device__ __forceinline__ void clamp_budgets(const StepParams& p, int n_v, int n, int mv_in, int ma_in, int& Mv, int& Ma) {
+  const int Kv = seg_len(p, n_v, n, 0), Ka = seg_len(p, n_v, n, 1);
+  Mv = min(max(mv_in, 0), min(Kv, p.cache_cap));
+  Ma = min(max(ma_in, 0), min(Ka, p.cache_cap - Mv));
+}
 __device__ __forceinline__ bool layer_skips_scoring(const StepParams& p, int l) {
   return p.skip_budget != nullptr && p.n[l] + p.Nn <= p.skip_budget[l];
 }

@@ -290,66 +290,111 @@ struct AllocParams {
   long long total_budget, budget_min, budget_max;
 };
 
+// Eq.14 with the range [B_min, B_max] of P:137 (R20) is the bounded proportional split
+//     b_l = clip(kappa pi_l, B_min, B_max),   kappa such that sum_l b_l = total          ("water-filling").
+// f(kappa) = sum_l clip(kappa pi_l, lo, hi) is continuous, non-decreasing and piecewise linear with breakpoints lo / pi_l
+// and hi / pi_l.  Thread t evaluates f at breakpoint t (2L of them); the crossing f = total lies between the largest
+// breakpoint with f <= total and the smallest with f >= total; between two neighbouring breakpoints the set of layers
+// strictly inside the range is constant, so there kappa = (total - mass of the clamped layers) / (pi of the free ones).
+// Integerisation is by largest remainder, computed as a RANK: layer l gets one of the `left` spare units iff fewer than
+// `left` eligible layers have a larger fractional part (equal parts: the lower layer first) -- no sequential hand-out.
+__device__ __forceinline__ double clip_share(double kappa, double pi, double lo, double hi) {
+  if (!(pi > 0.0)) return lo;                 // a layer whose softmax weight underflowed sits at the lower bound
+  const double v = kappa * pi;
+  return v < lo ? lo : (v > hi ? hi : v);
+}
+
 __global__ void __launch_bounds__(128) allocate_kernel(StepParams p, AllocParams ap, const double* __restrict__ stats,
                                                        const int32_t* __restrict__ layer_budget, int32_t* __restrict__ M_v,
                                                        int32_t* __restrict__ M_a, int32_t* __restrict__ layer_budget_out) {
   extern __shared__ double sm_alloc[];
-  const int L = p.L;
-  double* pi = sm_alloc;            // [L]
-  double* bl = sm_alloc + L;        // [L]
-  int* B = (int*)(sm_alloc + 2 * L);  // [L]
-  int* fixed = B + L;               // [L]
+  const int L = p.L, tid = threadIdx.x, nthr = blockDim.x;
+  double* pi = sm_alloc;               // [L]   softmax over layers
+  double* bl = pi + L;                 // [L]   real-valued share
+  double* kap = bl + L;                // [2L]  breakpoints
+  double* fk = kap + 2 * L;            // [2L]  f at the breakpoints
+  int* B = (int*)(fk + 2 * L);         // [L]
+  __shared__ double sh_kmid, sh_rem, sh_pfree;
+  __shared__ long long sh_left;
+  __shared__ int sh_mode;              // 0 = solve, 1 = every layer at B_max, 2 = every layer at B_min
   if (layer_budget != nullptr) {
-    for (int l = threadIdx.x; l < L; l += blockDim.x) B[l] = layer_budget[l];
-  } else if (threadIdx.x == 0) {
+    for (int l = tid; l < L; l += nthr) B[l] = layer_budget[l];
+  } else {
     const bool clamp = ap.budget_max > 0;
     const double lo = clamp ? (double)ap.budget_min : 0.0, hi = clamp ? (double)ap.budget_max : INFINITY;
-    double mx = -INFINITY, Z = 0.0;
-    for (int l = 0; l < L; ++l) {
-      pi[l] = stats[l * 8 + 6] * (1.0 - stats[l * 8 + 7]) / ap.temperature;  // C^(l)/T, Eq.13
-      mx = fmax(mx, pi[l]);
-      fixed[l] = 0;
+    const double total = (double)ap.total_budget;
+    if (tid == 0) {                      // Eq.13-14: pi = Softmax_l(C^(l) / T), fixed summation order
+      double mx = -INFINITY, Z = 0.0;
+      for (int l = 0; l < L; ++l) {
+        pi[l] = stats[l * 8 + 6] * (1.0 - stats[l * 8 + 7]) / ap.temperature;
+        mx = fmax(mx, pi[l]);
+      }
+      for (int l = 0; l < L; ++l) Z += (pi[l] = exp(pi[l] - mx));
+      for (int l = 0; l < L; ++l) pi[l] /= Z;
+      sh_mode = (clamp && total >= hi * L) ? 1 : ((clamp && total <= lo * L) ? 2 : 0);
     }
-    for (int l = 0; l < L; ++l) Z += (pi[l] = exp(pi[l] - mx));
-    for (int l = 0; l < L; ++l) pi[l] /= Z;                                 // Eq.14 softmax over layers
-    if (clamp && (double)ap.total_budget >= hi * L) {
-      for (int l = 0; l < L; ++l) B[l] = (int)ap.budget_max;
-    } else if (clamp && (double)ap.total_budget <= lo * L) {
-      for (int l = 0; l < L; ++l) B[l] = (int)ap.budget_min;
+    __syncthreads();
+    if (sh_mode != 0) {                  // the range makes the total unreachable: the nearer bound everywhere
+      for (int l = tid; l < L; l += nthr) B[l] = (int)(sh_mode == 1 ? ap.budget_max : ap.budget_min);
     } else {
-      for (int it = 0; it <= L; ++it) {  // fix violators at the bound, re-split the rest in proportion to pi
-        double rem = (double)ap.total_budget, pfree = 0.0;
-        for (int l = 0; l < L; ++l) { if (fixed[l]) rem -= bl[l]; else pfree += pi[l]; }
-        double below = 0.0, above = 0.0;
-        for (int l = 0; l < L; ++l)
-          if (!fixed[l]) {
-            bl[l] = pfree > 0.0 ? rem * pi[l] / pfree : 0.0;
-            below += bl[l] < lo ? lo - bl[l] : 0.0;
-            above += bl[l] > hi ? bl[l] - hi : 0.0;
-          }
-        bool moved = false;
-        const bool top = above >= below;  // clamp one side per round so that the total is preserved
-        for (int l = 0; l < L; ++l)
-          if (!fixed[l] && (top ? bl[l] > hi : bl[l] < lo)) { bl[l] = top ? hi : lo; fixed[l] = 1; moved = true; }
-        if (!moved) break;
+      for (int t = tid; t < 2 * L; t += nthr) {
+        const double pl = pi[t < L ? t : t - L];
+        const double k = pl > 0.0 ? (t < L ? lo : hi) / pl : INFINITY;
+        double f = 0.0;
+        for (int l = 0; l < L; ++l) f += clip_share(k, pi[l], lo, hi);
+        kap[t] = k;
+        fk[t] = f;
       }
-      long long sum = 0;
-      for (int l = 0; l < L; ++l) { B[l] = (int)floor(bl[l]); sum += B[l]; }
-      for (long long left = ap.total_budget - sum; left > 0; --left) {  // largest remainder, ties -> lowest layer
-        int best = -1;
-        double bf = -1.0;
-        for (int l = 0; l < L; ++l) {
-          const double fl = floor(bl[l]);
-          if ((double)B[l] <= fl && (double)B[l] + 1.0 <= hi && bl[l] - fl > bf) { bf = bl[l] - fl; best = l; }
+      __syncthreads();
+      if (tid == 0) {
+        double kA = 0.0, kB = INFINITY;    // f(0) = L lo < total < L hi = f(inf)
+        for (int t = 0; t < 2 * L; ++t) {
+          if (fk[t] <= total && kap[t] > kA && kap[t] < INFINITY) kA = kap[t];
+          if (fk[t] >= total && kap[t] < kB) kB = kap[t];
         }
-        if (best < 0) break;
-        B[best] += 1;
+        const double kmid = kB < INFINITY ? 0.5 * (kA + kB) : 2.0 * kA + 1.0;
+        double rem = total, pfree = 0.0;
+        for (int l = 0; l < L; ++l) {
+          const double v = clip_share(kmid, pi[l], lo, hi);
+          if (v <= lo || v >= hi) rem -= v; else pfree += pi[l];
+        }
+        sh_kmid = kmid; sh_rem = rem; sh_pfree = pfree;
       }
+      __syncthreads();
+      for (int l = tid; l < L; l += nthr) {
+        const double v = clip_share(sh_kmid, pi[l], lo, hi);
+        bl[l] = (v <= lo || v >= hi) ? v : sh_rem * pi[l] / sh_pfree;
+        B[l] = (int)floor(bl[l]);
+      }
+      __syncthreads();
+      if (tid == 0) {
+        long long sum = 0;
+        for (int l = 0; l < L; ++l) sum += B[l];
+        sh_left = ap.total_budget - sum;
+      }
+      __syncthreads();
+      for (int l = tid; l < L; l += nthr) {
+        const double fl = floor(bl[l]), fr = bl[l] - fl;
+        bool plus = false;
+        if (fl + 1.0 <= hi) {
+          long long rank = 0;
+          for (int j = 0; j < L; ++j) {
+            const double fj = floor(bl[j]), rj = bl[j] - fj;
+            if (fj + 1.0 <= hi && (rj > fr || (rj == fr && j < l))) ++rank;
+          }
+          plus = rank < sh_left;
+        }
+        kap[l] = plus ? 1.0 : 0.0;       // applied after everyone has read bl / B
+      }
+      __syncthreads();
+      for (int l = tid; l < L; l += nthr) B[l] += (int)kap[l];
     }
   }
   __syncthreads();
-  for (int l = threadIdx.x; l < L; l += blockDim.x) {
-    const int Bl = B[l] < 0 ? 0 : B[l];
+  for (int l = tid; l < L; l += nthr) {
+    // a per-layer total above the cache capacity cannot be stored: it is clamped, not rejected (the budgets are device
+    // data, nothing on the host sees them; include/omnimem.h "Budgets")
+    const int Bl = B[l] < 0 ? 0 : (B[l] > p.cache_cap ? p.cache_cap : B[l]);
     if (layer_budget_out) layer_budget_out[l] = Bl;
     if (M_v == nullptr) continue;   // calibration: only the per-layer totals are wanted
     const int n_v = p.n_v[l], n = p.n[l];
@@ -371,7 +416,7 @@ cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const d
                             int32_t* layer_budget_out, cudaStream_t st, int* launches) {
   AllocParams ap{(double)ctx->cfg.ratio_r, (double)ctx->cfg.temperature, (long long)total_budget,
                  (long long)ctx->cfg.budget_min, (long long)ctx->cfg.budget_max};
-  const size_t smem = (size_t)p.L * (2 * sizeof(double) + 2 * sizeof(int));
+  const size_t smem = (size_t)p.L * (6 * sizeof(double) + sizeof(int));
   allocate_kernel<<<1, 128, smem, st>>>(p, ap, stats, layer_budget, M_v, M_a, layer_budget_out);
   ++*launches;
   return cudaGetLastError();
@@ -431,7 +476,9 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(StepParams p, const
   const int seg = blockIdx.x;
   const int m = seg & 1, h = (seg >> 1) % p.Hkv, l = (seg >> 1) / p.Hkv;
   const int K = seg_len(p, p.n_v[l], p.n[l], m);
-  const int M = m == 0 ? M_v[l] : M_a[l];
+  int Mv_c, Ma_c;
+  clamp_budgets(p, p.n_v[l], p.n[l], M_v[l], M_a[l], Mv_c, Ma_c);
+  const int M = m == 0 ? Mv_c : Ma_c;
   const long long lh = (long long)l * p.Hkv + h;
   const float* psi = m == 0 ? psi_v + lh * p.seg_cap_v : psi_a + lh * p.seg_cap_a;
   int32_t* out = (m == 0 ? idx_v : idx_a) + lh * p.cache_cap;
@@ -528,7 +575,7 @@ cudaError_t launch_select(const omnimem_ctx* ctx, const StepParams& p, const flo
   const int segs = p.L * p.Hkv * 2;
   const size_t smem = (size_t)(p.seg_cap_v > p.seg_cap_a ? p.seg_cap_v : p.seg_cap_a) * sizeof(uint32_t);
   ++*launches;
-  if (smem <= 200 * 1024) {
+  if (smem <= 225 * 1024) {   // up to 57600 keys (the paper's 48k budget + a 4096-row chunk) stay in shared memory
     cudaError_t e = cudaFuncSetAttribute(select_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     select_kernel<true><<<segs, kSelThreads, smem, st>>>(p, psi_v, psi_a, M_v, M_a, idx_v, idx_a);
@@ -552,7 +599,9 @@ __global__ void __launch_bounds__(256) compact_kernel(StepParams p, const uint4*
                                                       int32_t* __restrict__ dst_n) {
   constexpr int kRowsPerPass = 256 / kTPR;
   const int l = blockIdx.z, h = blockIdx.y;
-  const int Mv = M_v[l], Ma = M_a[l], total = Mv + Ma;
+  int Mv, Ma;
+  clamp_budgets(p, p.n_v[l], p.n[l], M_v[l], M_a[l], Mv, Ma);
+  const int total = Mv + Ma;
   if (blockIdx.x == 0 && h == 0 && threadIdx.x == 0) { dst_n_v[l] = Mv; dst_n[l] = total; }
   const int j0 = blockIdx.x * (kRowsPerPass * kR) + threadIdx.x / kTPR;
   if (j0 - (int)(threadIdx.x / kTPR) >= total) return;
@@ -650,7 +699,9 @@ __global__ void __launch_bounds__(256) compact_hidden_kernel(StepParams p, const
                                                              int row_vecs) {
   const int l = blockIdx.y, lane = threadIdx.x & 31;
   const int j = blockIdx.x * 8 + (threadIdx.x >> 5);
-  const int Mv = M_v[l], total = Mv + M_a[l];
+  int Mv, Ma;
+  clamp_budgets(p, p.n_v[l], p.n[l], M_v[l], M_a[l], Mv, Ma);
+  const int total = Mv + Ma;
   if (j >= total) return;
   const int m = j < Mv ? 0 : 1;
   const long long lh0 = (long long)l * p.Hkv;  // head 0 of the layer

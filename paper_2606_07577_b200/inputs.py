@@ -14,6 +14,8 @@ from __future__ import annotations
 
 import dataclasses
 import math
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass
 
 import torch
@@ -175,11 +177,13 @@ def layer_inputs(wl: Workload, layer: int, step: int = 0, with_cache: bool = Tru
     return out
 
 
-def full_inputs(wl: Workload, step: int = 0, layers=None, with_cache: bool = True, pin: bool = False) -> dict:
+def full_inputs(wl: Workload, step: int = 0, layers=None, with_cache: bool = True, pin: bool = False,
+                workers: int | None = None) -> dict:
     """Stack `layers` (default all) into [L', ...] tensors; the cache is zero-padded to cache_cap rows.
 
     Returns cacheK, cacheV [L',Hkv,cache_cap,D], chunkK, chunkV [L',Hkv,Nn,D], Q [L',Hq,Nn,D],
-    n_v, n int32 [L'] (rows valid per layer).
+    n_v, n int32 [L'] (rows valid per layer).  Layers have their own generators, so they are drawn by `workers`
+    threads (default: up to 8) with bit-identical results.
     """
     layers = list(range(wl.L)) if layers is None else list(layers)
     Lp, dt = len(layers), wl.torch_dtype
@@ -189,13 +193,22 @@ def full_inputs(wl: Workload, step: int = 0, layers=None, with_cache: bool = Tru
         out["cacheK"] = torch.zeros(Lp, wl.Hkv, wl.cache_cap, wl.D, dtype=dt)
         out["cacheV"] = torch.zeros(Lp, wl.Hkv, wl.cache_cap, wl.D, dtype=dt)
     nc = (wl.n_v + wl.n_a) if with_cache else 0
-    for i, l in enumerate(layers):
+    def fill(il):
+        i, l = il
         x = layer_inputs(wl, l, step, with_cache)
         for k in ("chunkK", "chunkV", "Q"):
             out[k][i] = x[k]
         if with_cache:
             out["cacheK"][i, :, :nc] = x["cacheK"]
             out["cacheV"][i, :, :nc] = x["cacheV"]
+
+    workers = min(8, os.cpu_count() or 1, Lp) if workers is None else workers
+    if workers > 1:
+        with ThreadPoolExecutor(max_workers=workers) as ex:
+            list(ex.map(fill, enumerate(layers)))
+    else:
+        for il in enumerate(layers):
+            fill(il)
     out["n_v"] = torch.full((Lp,), wl.n_v if with_cache else 0, dtype=torch.int32)
     out["n"] = torch.full((Lp,), nc, dtype=torch.int32)
     return out
@@ -252,8 +265,3 @@ def interleave(x: dict, modality: torch.Tensor, Nn_v: int) -> dict:
         if k in x:
             y[k] = x[k].index_select(-2, src).contiguous()
     return y
-
-
-def small(wl: Workload, **kw) -> Workload:
-    """A reduced copy of a config (same recipe and value structure) for tests the oracle finishes in seconds."""
-    return wl.replace(**kw)

@@ -118,28 +118,29 @@ def run_full_step(wl, sample_layers):
     return n_diff
 
 
+# Rule (c) would allow ~1e2 indices per segment to differ (lambda = 0.02 squeezes psi into a narrow band); what is
+# measured on every sampled layer is 0 differing indices, so that is what is asserted (SURVEY.md 8(c) "design target").
 def test_cfg2_full_size():
-    n_diff = run_full_step(I.CFG2, sample_layers=(0, 27))
-    assert n_diff <= 8, f"{n_diff} kept indices differ (all inside rule (c)'s tolerance band, but fp32-level agreement is the target)"
+    assert run_full_step(I.CFG2, sample_layers=(0, 14, 27)) == 0
 
 
 def test_cfg4_full_size():
-    n_diff = run_full_step(I.CFG4, sample_layers=(0, 18, 35))
-    assert n_diff <= 8
+    assert run_full_step(I.CFG4, sample_layers=(0, 18, 35)) == 0
 
 
 def test_cfg3_full_size():
-    n_diff = run_full_step(I.CFG3, sample_layers=(35,))
-    assert n_diff <= 8
+    assert run_full_step(I.CFG3, sample_layers=(0, 35)) == 0
 
 
 def test_cfg5_streaming_teacher_forced():
-    """CFG5 (hour-long stream, Qwen2.5-Omni-7B shape, B = 32768): the GPU runs free from an empty cache through the
-    append-only steps, the first eviction (step index 5) and into the steady state; at sampled (step, layer) pairs the
-    oracle starts from the GPU's own pre-step cache state of that layer, so each sampled step is checked on its own."""
+    """CFG5 (hour-long stream, Qwen2.5-Omni-7B shape, B = 32768), ALL 60 chunks: the GPU runs free from an empty cache
+    through the append-only steps, the first eviction (step index 5) and 54 steady-state steps; the any-size properties
+    are checked on every layer of every step, and at sampled (step, layer) pairs -- the last append-only step, the first
+    eviction, the first steady-state step, mid-stream and the last chunk -- the oracle starts from the GPU's own pre-step
+    cache state of that layer, so each sampled step is checked on its own (teacher forcing)."""
     from paper_2606_07577_b200.omnimem import Chunk, OmniMem
     wl = I.CFG5
-    n_steps, samples = 8, {4: 9, 5: 3, 7: 20}                # step index -> layer checked in full
+    n_steps, samples = wl.steps, {4: 9, 5: 3, 6: 20, 30: 14, 59: 27}     # step index -> layer checked in full
     eng = OmniMem.for_workload(wl)
     dev = eng.device
     src, dst = eng.new_cache(), eng.new_cache()
@@ -149,8 +150,13 @@ def test_cfg5_streaming_teacher_forced():
     M_a = torch.zeros_like(M_v)
     idx_v, idx_a = eng.new_indices()
     n_diff = 0
+    from concurrent.futures import ThreadPoolExecutor
+    pool = ThreadPoolExecutor(max_workers=1)                  # the next chunk is drawn on the host while this one is checked
+    nxt = pool.submit(I.full_inputs, wl, step=0, with_cache=False)
     for step in range(n_steps):
-        x = I.full_inputs(wl, step=step, with_cache=False)
+        x = nxt.result()
+        if step + 1 < n_steps:
+            nxt = pool.submit(I.full_inputs, wl, step=step + 1, with_cache=False)
         chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
         n_v, n = src.n_v.cpu().numpy(), src.n.cpu().numpy()
         assert np.all(n == min(step * wl.Nn, wl.budget)), f"step {step}: cache rows {n}"
@@ -177,6 +183,7 @@ def test_cfg5_streaming_teacher_forced():
                 assert np.array_equal(dst.k[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstK"][0, :, :nl])
                 assert np.array_equal(dst.v[l, :, :nl].cpu().view(torch.uint8).numpy(), orc["dstV"][0, :, :nl])
         src, dst = dst, src
+    pool.shutdown()
     assert int(src.n.min()) == wl.budget
-    assert n_diff <= 8
+    assert n_diff == 0
     eng.close()

@@ -322,7 +322,8 @@ def test_allocate_formula_and_edges():
 
 
 def test_layer_budgets_invariants():
-    """Eq.14 (parity unpinned beyond these, R20): softmax sums to 1, T -> inf and equal C => uniform, exact sum, clamps."""
+    """Eq.14 invariants: softmax sums to 1, T -> inf and equal C => uniform, exact sum, clamps (the clamp branch itself is
+    pinned by test_layer_budgets_clamp_branch_is_kappa_waterfilling below)."""
     L = 7
     st = np.zeros((L, 8))
     st[:, 6] = np.linspace(0.5, 0.9, L)
@@ -354,6 +355,143 @@ def test_layer_budgets_invariants():
     assert b.sum() == 256 * 9 and b.min() >= 200 and b.max() <= 320
     C9 = st9[:, 6] * (1 - st9[:, 7])
     assert np.all(np.diff(b[np.argsort(C9)]) >= 0)            # monotone in compressibility
+
+
+# ---- Eq.14 with [B_min, B_max] ("constrained within the range of [B_min, B_max]"): independent pin (R20) -------
+def kappa_waterfill(pi, lo, hi, total):
+    """The bounded proportional split that the mathematics fixes: b_l = clip(kappa * pi_l, lo, hi) with the scalar kappa
+    set by sum_l b_l = total (f(kappa) = sum clip(kappa pi) is continuous and non-decreasing, so kappa is unique wherever
+    f is strictly increasing; on a flat part every kappa gives the same b).  Plain bisection on kappa: no loop over
+    'violators', no re-splitting, nothing of the oracle's procedure."""
+    f = lambda k: np.clip(k * pi, lo, hi).sum()
+    if total >= hi * len(pi):
+        return np.full(len(pi), float(hi))
+    if total <= lo * len(pi):
+        return np.full(len(pi), float(lo))
+    k0, k1 = 0.0, 1.0
+    while f(k1) < total:
+        k1 *= 2.0
+    for _ in range(200):
+        km = 0.5 * (k0 + k1)
+        if f(km) < total:
+            k0 = km
+        else:
+            k1 = km
+    return np.clip(0.5 * (k0 + k1) * pi, lo, hi)
+
+
+def largest_remainder(b, total, hi):
+    """numpy largest-remainder integerisation: floor, then +1 to the (total - sum floor) largest fractional parts, equal
+    fractions to the lowest layer first, never above hi.  Returns (ints, gap) where gap is the distance between the
+    last fraction that got a unit and the first that did not (a near-zero gap means the choice is rounding noise)."""
+    fl = np.floor(b + 1e-9)                       # a clamped layer sits ON an integer bound; bisection leaves it 1e-13 short
+    frac = np.where(fl + 1 <= hi, b - fl, -1.0)
+    left = int(round(total - fl.sum()))
+    order = np.argsort(-frac, kind="stable")      # stable: equal fractions keep ascending layer order
+    out = fl.astype(np.int64)
+    out[order[:left]] += 1
+    gap = frac[order[left - 1]] - frac[order[left]] if 0 < left < len(b) else 1.0
+    return out, gap
+
+
+def eq14_cases(n_cases=240):
+    g = np.random.default_rng(2014)
+    for c in range(n_cases):
+        L = int(g.integers(2, 41))
+        st = np.zeros((L, 8))
+        spread = [0.05, 0.3, 0.8][c % 3]                       # narrow to wide compressibility spread
+        st[:, 6] = np.clip(0.6 + spread * g.standard_normal(L) * 0.5, 0.01, 1.0)
+        st[:, 7] = g.uniform(0.0, 0.6, L)
+        T = [0.2, 0.05, 1.0][(c // 3) % 3]
+        mean_b = int(g.integers(64, 40000))
+        kind = c % 5
+        if kind == 0:
+            lo, hi = int(0.8 * mean_b), int(1.25 * mean_b)      # both bounds bite
+        elif kind == 1:
+            lo, hi = 1, int(1.1 * mean_b)                       # upper bound only
+        elif kind == 2:
+            lo, hi = int(0.9 * mean_b), 100 * mean_b            # lower bound only
+        elif kind == 3:
+            lo, hi = int(0.5 * mean_b), int(2 * mean_b)         # mild
+        else:
+            lo, hi = int(0.97 * mean_b), int(1.03 * mean_b)     # tight: almost every layer is clamped
+        total = mean_b * L + int(g.integers(-L, L + 1))
+        if c % 40 == 7:
+            total = hi * L + 5                                  # infeasible: every layer at B_max
+        if c % 40 == 9:
+            total = max(0, lo * L - 5)                          # infeasible: every layer at B_min
+        yield L, st, T, lo, hi, total
+
+
+def test_layer_budgets_clamp_branch_is_kappa_waterfilling():
+    """R20 pin: omnimem_ref_layer_budgets with clamps == clip(kappa pi, B_min, B_max), sum = total, found by
+    bisection in numpy, then integerised by a numpy largest-remainder.  240 seeded cases: one- and two-sided clamps,
+    tight ranges, wide and narrow softmax spreads, infeasible totals."""
+    n_clamped_lo = n_clamped_hi = n_both = checked = 0
+    for L, st, T, lo, hi, total in eq14_cases():
+        p = ref.RefParams(L=L, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=T, budget_min=lo, budget_max=hi)
+        got = ref.layer_budgets(p, st, total).astype(np.int64)
+        C = st[:, 6] * (1.0 - st[:, 7])
+        e = np.exp((C - C.max()) / T)
+        pi = e / e.sum()
+        b = kappa_waterfill(pi, lo, hi, total)
+        assert got.min() >= lo and got.max() <= hi
+        if total >= hi * L or total <= lo * L:
+            assert np.all(got == (hi if total >= hi * L else lo))
+            continue
+        assert got.sum() == total
+        assert np.all(np.abs(got - b) < 1.0 + 1e-6), f"not within one unit of the kappa form: {got} vs {b}"
+        want, gap = largest_remainder(b, total, hi)
+        if gap > 1e-6:                                           # else the last unit is decided by rounding noise
+            assert np.array_equal(got, want), f"L={L} lo={lo} hi={hi} total={total}: {got} vs {want}"
+            checked += 1
+        at_lo, at_hi = (np.abs(b - lo) < 1e-9).sum(), (np.abs(b - hi) < 1e-9).sum()
+        n_clamped_lo += at_lo > 0
+        n_clamped_hi += at_hi > 0
+        n_both += (at_lo > 0) and (at_hi > 0)
+    assert checked >= 200 and n_both >= 40 and n_clamped_lo >= 80 and n_clamped_hi >= 80    # the cases do exercise the branch
+
+
+def test_layer_budgets_pin_catches_a_wrong_redistribution():
+    """The pin above discriminates: a plausible wrong rule -- clipped mass re-spread UNIFORMLY over the free layers
+    instead of in proportion to pi -- departs from the kappa form by more than a unit on most clamped cases."""
+    def uniform_respread(pi, lo, hi, total):
+        b = np.clip(pi * total, lo, hi)
+        for _ in range(100):
+            free = (b > lo) & (b < hi)
+            if not free.any() or abs(total - b.sum()) < 1e-9:
+                break
+            b[free] += (total - b.sum()) / free.sum()
+            b = np.clip(b, lo, hi)
+        return b
+    caught = tried = 0
+    for L, st, T, lo, hi, total in eq14_cases(120):
+        if total >= hi * L or total <= lo * L:
+            continue
+        C = st[:, 6] * (1.0 - st[:, 7])
+        e = np.exp((C - C.max()) / T)
+        pi = e / e.sum()
+        b = kappa_waterfill(pi, lo, hi, total)
+        if not ((np.abs(b - lo) < 1e-9).any() or (np.abs(b - hi) < 1e-9).any()):
+            continue
+        tried += 1
+        caught += np.abs(uniform_respread(pi, lo, hi, total) - b).max() > 1.0
+    assert tried >= 60 and caught >= 0.6 * tried
+
+
+def test_layer_budgets_two_layer_clamp_closed_form():
+    """Two layers, upper clamp biting: B = (total - B_max, B_max) whatever pi says; three layers with one clamped:
+    the other two split the rest in the ratio pi_0 : pi_1 = exp((C_0 - C_1)/T)."""
+    p = ref.RefParams(L=2, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=0.2, budget_min=10, budget_max=600)
+    st = np.zeros((2, 8))
+    st[:, 6] = [0.9, 0.3]
+    assert list(ref.layer_budgets(p, st, 1000)) == [600, 400]
+    p3 = ref.RefParams(L=3, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=0, Nn_a=0, temperature=0.2, budget_min=0, budget_max=500000)
+    st3 = np.zeros((3, 8))
+    st3[:, 6] = [0.5, 0.6, 0.95]                     # pi_2 dominates: unclamped it would take ~80 %
+    b = ref.layer_budgets(p3, st3, 10**6)
+    assert b[2] == 500000 and b.sum() == 10**6
+    assert abs(b[0] / b[1] - np.exp((0.5 - 0.6) / 0.2)) < 1e-4
 
 
 def test_psi_shared_heads_paper_literal():
@@ -599,3 +737,38 @@ def test_duplicate_rows_are_evicted_first():
     for h in range(wl.Hkv):
         kept = set(out["idx_v"][0, h, :out["M_v"][0]].tolist())
         assert not kept & set(range(101, 139))
+
+
+def test_oracle_under_address_and_ub_sanitizers():
+    """the oracle built with -fsanitize=address,undefined runs a whole step (blocked and interleaved
+    chunk, shared selection, Eq.14 with clamps, ragged layers incl. an empty cache) without a report.  compute-sanitizer is
+    closed on the GPU pool, so this is the sanitizer this repo can run."""
+    import subprocess
+    import sys
+    asan = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("libasan not installed")
+    code = """
+import numpy as np, torch
+from oracle import ref
+from paper_2606_07577_b200 import inputs as I
+wl = I.CFG1.replace(L=3, cache_cap=600)
+x = I.full_inputs(wl)
+x['n'][1], x['n_v'][1] = 0, 0
+x['n'][2], x['n_v'][2] = 77, 13
+mod = I.modality_pattern(wl, 5)
+for kw, scope in ((dict(), 0), (dict(chunk_modality=mod.numpy()), 1)):
+    p = ref.RefParams(L=3, Hq=wl.Hq, Hkv=wl.Hkv, D=wl.D, cache_cap=wl.cache_cap, Nn_v=wl.Nn_v, Nn_a=wl.Nn_a,
+                      sim_stride_v=16, budget_min=100, budget_max=300, **kw)
+    sc = ref.score(p, x['cacheK'], x['cacheV'], x['n_v'], x['n'], x['chunkK'], x['chunkV'], x['Q'], want_rowH=True, select_scope=scope)
+    B = ref.layer_budgets(p, sc['stats'], 3 * 200)
+    out = ref.compress_chunk(p, x['cacheK'], x['cacheV'], x['n_v'], x['n'], x['chunkK'], x['chunkV'], x['Q'], B, select_scope=scope)
+    assert out['n_out'].tolist() == np.minimum(B, x['n'].numpy() + wl.Nn).tolist()
+print('sanitized oracle ok')
+"""
+    env = dict(os.environ, OMNIMEM_REF_SANITIZE="1", LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:abort_on_error=0",
+               UBSAN_OPTIONS="print_stacktrace=1", OMP_NUM_THREADS="2")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", code], env=env, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "sanitized oracle ok" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "ERROR: AddressSanitizer" not in r.stderr and "runtime error" not in r.stderr, r.stderr[-4000:]
