@@ -138,6 +138,57 @@ int omnimem_ref_attention(const omnimem_ref_params* p, const double* cacheK, con
   return 0;
 }
 
+/* ---- A1: the chunk's multi-head self-attention over both caches and the chunk (Eq.1, Eq.2) ----
+ * Y_c = MHSA(Q_c, K_c, V_c, O_c, P_c): for query head j = h*G+g and chunk query i,
+ *   Y[l,j,i,:] = sum_{k visible} softmax_k(c <q_i, k_k>) v_k
+ * over the same logical key sequence and the same mask as O2 (cached visual, cached audio, chunk rows in storage
+ * order; causal inside the chunk, R2-R3); values V follow the keys' order.  lse[l,j,i] is the row's log-sum-exp,
+ * the quantity score pass 2 needs (Eq.6).  absY (optional) = sum_k p_k |v_k|: the magnitude that bounds the rounding
+ * error of an implementation that rounds p or Y to bf16.  Y, absY: [L,Hq,Nn,D]; lse: [L,Hq,Nn]. */
+int omnimem_ref_mhsa(const omnimem_ref_params* p, const double* cacheK, const double* cacheV, const int32_t* n,
+                     const double* chunkK, const double* chunkV, const double* Q, double* Y, double* lse,
+                     double* absY) {
+  const int Nn = p->Nn_v + p->Nn_a, G = p->Hq / p->Hkv, D = p->D;
+  if (p->Hq % p->Hkv != 0) return -1;
+  for (int l = 0; l < p->L; ++l) {
+    const int Nc = n[l], Nk = Nc + Nn;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int ri = 0; ri < p->Hq * Nn; ++ri) {
+      const int j = ri / Nn, i = ri % Nn, h = j / G;
+      const double* q = Q + IDX3(l * p->Hq + j, i, 0, Nn, D);
+      double* y = Y + IDX3(l * p->Hq + j, i, 0, Nn, D);
+      double* ay = absY ? absY + IDX3(l * p->Hq + j, i, 0, Nn, D) : NULL;
+      const int nvis = p->causal ? Nc + i + 1 : Nk; /* R3 */
+      double* z = (double*)malloc(sizeof(double) * (size_t)(nvis > 0 ? nvis : 1));
+      double m = -INFINITY;
+      for (int k = 0; k < nvis; ++k) {
+        const double* kr = key_row(p, cacheK, chunkK, l, h, Nc, k);
+        double dot = 0.0;
+        for (int d = 0; d < D; ++d) dot += q[d] * kr[d];
+        z[k] = p->scale * dot;
+        if (z[k] > m) m = z[k];
+      }
+      double Z = 0.0;
+      for (int k = 0; k < nvis; ++k) Z += exp(z[k] - m);
+      for (int d = 0; d < D; ++d) {
+        y[d] = 0.0;
+        if (ay) ay[d] = 0.0;
+      }
+      for (int k = 0; k < nvis; ++k) {
+        const double pk = exp(z[k] - m) / Z;
+        const double* vr = key_row(p, cacheV, chunkV, l, h, Nc, k);
+        for (int d = 0; d < D; ++d) {
+          y[d] += pk * vr[d];
+          if (ay) ay[d] += pk * fabs(vr[d]);
+        }
+      }
+      if (lse) lse[IDX3(l, j, i, p->Hq, Nn)] = m + log(Z);
+      free(z);
+    }
+  }
+  return 0;
+}
+
 /* Split a logical-order array into the two per-modality segment arrays [L,Hkv,seg_cap_m]. */
 int omnimem_ref_split(const omnimem_ref_params* p, const double* a_log, const int32_t* n_v, const int32_t* n,
                       double* a_v, double* a_a) {

@@ -151,6 +151,22 @@ def attention(p: RefParams, cacheK, n, chunkK, Q, want_rowH: bool = True):
     return a_log, lse, rowH
 
 
+def mhsa(p: RefParams, cacheK, cacheV, n, chunkK, chunkV, Q, want_abs: bool = False):
+    """P:54 Eq.1: the chunk's attention output over [cached visual; cached audio; chunk] and its row LSE.
+    Returns (Y [L,Hq,Nn,D], lse [L,Hq,Nn], absY or None)."""
+    cacheK, cacheV, chunkK, chunkV, Q, n = f64(cacheK), f64(cacheV), f64(chunkK), f64(chunkV), f64(Q), i32(n)
+    assert cacheK.shape == cacheV.shape == (p.L, p.Hkv, p.cache_cap, p.D), cacheK.shape
+    assert chunkK.shape == chunkV.shape == (p.L, p.Hkv, p.Nn, p.D), chunkK.shape
+    assert Q.shape == (p.L, p.Hq, p.Nn, p.D), Q.shape
+    Y = np.zeros((p.L, p.Hq, p.Nn, p.D), np.float64)
+    lse = np.zeros((p.L, p.Hq, p.Nn), np.float64)
+    absY = np.zeros_like(Y) if want_abs else None
+    cp = p.c()
+    _check(lib().omnimem_ref_mhsa(C.byref(cp), _p(cacheK), _p(cacheV), _p(n), _p(chunkK), _p(chunkV), _p(Q), _p(Y), _p(lse),
+                                  _p(absY) if want_abs else None), "mhsa")
+    return Y, lse, absY
+
+
 def split(p: RefParams, a_log, n_v, n):
     a_log, n_v, n = f64(a_log), i32(n_v), i32(n)
     a_v = np.zeros((p.L, p.Hkv, p.seg_cap_v), np.float64)

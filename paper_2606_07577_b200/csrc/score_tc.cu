@@ -67,13 +67,6 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-#ifdef OMNIMEM_DBG_FREERUN
-#define EPI_WAIT(bar, parity) ((void)0)
-#define EPI_ARRIVE(bar) ((void)0)
-#else
-#define EPI_WAIT(bar, parity) mbar_wait(bar, parity)
-#define EPI_ARRIVE(bar) mbar_arrive(bar)
-#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
@@ -155,11 +148,6 @@ __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, ui
       "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
-#ifdef OMNIMEM_DBG_NOLD
-#pragma unroll
-  for (int i = 0; i < 32; ++i) r[i] = taddr + i;   // timing experiment only
-  return;
-#endif
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
       "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
@@ -208,9 +196,6 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
   return d;
 }
 __device__ __forceinline__ float ex2(float x) {
-#ifdef OMNIMEM_DBG_NOEXP
-  return x;   // timing experiment only: results are wrong
-#endif
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
@@ -225,22 +210,44 @@ __device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
   asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
 }
+#ifndef OMNIMEM_POLY_DEG
+#define OMNIMEM_POLY_DEG 4
+#endif
+#ifndef OMNIMEM_EXP_MUL
+#define OMNIMEM_EXP_MUL 0
+#endif
 __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
   float x0, x1;
   unpack2(X, x0, x1);
-  X = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));   // keeps the biased exponent of q * 2^round(x) >= 0
+  const float kClamp = OMNIMEM_EXP_MUL ? -127.f : -126.f;
+  X = pack2(fmaxf(x0, kClamp), fmaxf(x1, kClamp));
   const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
   const uint64_t T = add2(X, MG);
   const uint64_t F = sub2(X, sub2(T, MG));
+#if OMNIMEM_POLY_DEG == 4
   uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
   Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
   Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
   Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
+#else   // degree 3: max relative error 7.5e-5, equi-oscillating (the error of a sum of many terms averages out)
+  uint64_t Q = fma2(pack2(0.0551716685295105f, 0.0551716685295105f), F, pack2(0.2426111251115799f, 0.2426111251115799f));
+  Q = fma2(Q, F, pack2(0.6932609677314758f, 0.6932609677314758f));
+  Q = fma2(Q, F, pack2(0.9999280571937561f, 0.9999280571937561f));
+#endif
   float q0, q1, t0, t1;
   unpack2(Q, q0, q1);
   unpack2(T, t0, t1);
+#if OMNIMEM_EXP_MUL
+  // q * 2^round(x) as a multiplication by the float (round(x) + 127) << 23: round(x) = -127 gives the factor 0, so
+  // everything at or below 2^-127 is exactly 0, like the MUFU lanes (ex2.approx.ftz)
+  const uint64_t SC = pack2u(((uint32_t)__float_as_int(t0) << 23) + 0x3F800000u, ((uint32_t)__float_as_int(t1) << 23) + 0x3F800000u);
+  uint64_t R;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(R) : "l"(Q), "l"(SC));
+  return R;
+#else
   return pack2(__int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23)),   // q * 2^round(x)
                __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23)));
+#endif
 }
 #ifndef OMNIMEM_POLY_NUM
 #define OMNIMEM_POLY_NUM 2
@@ -249,11 +256,6 @@ __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
 #define OMNIMEM_POLY_DEN 8
 #endif
 constexpr int kPolyNum = OMNIMEM_POLY_NUM, kPolyDen = OMNIMEM_POLY_DEN;
-#ifdef OMNIMEM_DBG_NOACC
-#define OMNIMEM_DBG_ACC(kk) 0u
-#else
-#define OMNIMEM_DBG_ACC(kk) ((kk) > 0 ? 1u : 0u)
-#endif
 // pair `pi` of a row goes to the polynomial iff the Bresenham line of slope kPolyNum / kPolyDen steps there
 __device__ __forceinline__ constexpr bool pair_is_poly(int pi) {
   return ((pi + 1) * kPolyNum) / kPolyDen > (pi * kPolyNum) / kPolyDen;
@@ -399,11 +401,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
   }
   const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
-#ifdef OMNIMEM_DBG_MAXTILES   // timing experiment only: cap the streamed sequence to expose the per-CTA fixed cost
-  w.ntiles = min(w.ntiles, OMNIMEM_DBG_MAXTILES);
-  w.ntiles_sub[0] = min(w.ntiles_sub[0], OMNIMEM_DBG_MAXTILES);
-  w.ntiles_sub[1] = min(w.ntiles_sub[1], OMNIMEM_DBG_MAXTILES);
-#endif
 
   // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
   // array is a link-time constant, so every barrier / stage address below folds into an immediate
@@ -446,9 +443,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
-#ifdef OMNIMEM_DBG_FREERUN
-  if (warp < 4) goto done;   // timing experiment only: the epilogue reads whatever tensor memory holds, nobody feeds it
-#endif
   if (warp == 0) {
     // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
     int it = kPass == 2 ? w.seq0 : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
@@ -467,13 +461,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         lh = w.hq0 + g;
         if (++it == w.seq0 + w.tiles_per_g) { it = w.seq0; ++g; }
       }
-#ifdef OMNIMEM_DBG_NOTMA
-      if (elect_one()) { mbar_arrive(bar_full + 8 * stage); if (kPass == 2) mbar_arrive(bar_lse + 8 * slot); }
-      __syncwarp();
-      if (++stage == kStages) { stage = 0; sph ^= 1; }
-      if (++slot == kLseSlots) slot = 0;
-      continue;
-#endif
       if (elect_one()) {
         mbar_expect_tx(bar_full + 8 * stage, kTileBytes / kCluster);
         if (kPass == 2) {
@@ -530,10 +517,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
             // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
             const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytesB + (kk & 3) * 32) >> 4);
-#ifndef OMNIMEM_DBG_NOMMA
-            if (kCluster == 2) tc_mma_bf16_ts_pair(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdescPair, OMNIMEM_DBG_ACC(kk));
-            else tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, OMNIMEM_DBG_ACC(kk));
-#endif
+            if (kCluster == 2) tc_mma_bf16_ts_pair(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdescPair, kk > 0 ? 1u : 0u);
+            else tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, kk > 0 ? 1u : 0u);
           }
           if (kCluster == 2) tc_commit_pair(bar_sfull + 8 * buf); else tc_commit(bar_sfull + 8 * buf);
         }
@@ -559,7 +544,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     auto release = [&](int b) {
       if (lane == 0) {
         if (kCluster == 2 && !leader) mbar_arrive_remote(bar_sempty + 8 * b, 0);
-        else EPI_ARRIVE(bar_sempty + 8 * b);
+        else mbar_arrive(bar_sempty + 8 * b);
       }
     };
     if (!w.sub_valid[s]) {
@@ -573,7 +558,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
           if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
           if (s == 0 ? tk0 : tk1) {
-            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            mbar_wait(bar_sfull + 8 * buf, ph);
             release(buf);
             if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           }
@@ -617,7 +602,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const int nt_mine = s == 0 ? w.ntiles_sub[0] : w.ntiles_sub[1];
         // accumulator batch at ring position (b, bph) -> registers; the TMEM buffer is released as soon as they hold it
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
-          EPI_WAIT(bar_sfull + 8 * b, bph);
+          mbar_wait(bar_sfull + 8 * b, bph);
           tc_fence_after();
           const uint32_t t_addr = t_col + (uint32_t)(b * kTile);
           tc_ld32(t_addr, v0);
@@ -695,7 +680,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             row_update(v0, v1, kHalf);
             continue;
           }
-          EPI_WAIT(bar_sfull + 8 * own, oph);
+          mbar_wait(bar_sfull + 8 * own, oph);
           tc_fence_after();
           const uint32_t t_addr = t_col + (uint32_t)(own * kTile);
           tc_ld32(t_addr, v0);
@@ -749,7 +734,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
           if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           if (kCluster == 2 && j >= nt_mine) {   // the peer's rows take this tile, mine do not: hand the buffer back unread
-            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            mbar_wait(bar_sfull + 8 * buf, ph);
             release(buf);
             if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
             if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
@@ -795,7 +780,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const uint64_t c2c2 = pack2(c2, c2);
         const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s];
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
-          EPI_WAIT(bar_sfull + 8 * b, bph);
+          mbar_wait(bar_sfull + 8 * b, bph);
           tc_fence_after();
           const uint32_t t_addr = t_col + (uint32_t)(b * kTile);
           tc_ld32(t_addr, v0);
@@ -831,7 +816,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             buf += 2;
             if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
             const int slot = j % kLseSlots;
-            EPI_WAIT(bar_lse + 8 * slot, (j / kLseSlots) & 1);
+            mbar_wait(bar_lse + 8 * slot, (j / kLseSlots) & 1);
             col_update(v0, v1, sLse + (uint32_t)(slot * kTile + col0) * 4);
           }
         } else {
@@ -847,7 +832,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (s == 1 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j comes first
           if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
           if (kCluster == 2 && it < it_mine) {   // the peer's keys see this query tile, mine do not yet: hand the buffer back unread
-            EPI_WAIT(bar_sfull + 8 * buf, ph);
+            mbar_wait(bar_sfull + 8 * buf, ph);
             release(buf);
             if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
             if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
@@ -859,7 +844,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           load_tile(buf, ph, v0, v1);
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
-          EPI_WAIT(bar_lse + 8 * slot, lse_parity);
+          mbar_wait(bar_lse + 8 * slot, lse_parity);
           const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
           if (first <= 0) {
             col_update(v0, v1, l_addr);
@@ -895,9 +880,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       }
     }
   }
-#ifdef OMNIMEM_DBG_FREERUN
-done:
-#endif
   tc_fence_before();
   __syncthreads();
   if (kCluster == 2) cluster_sync_all();   // nobody leaves while the peer may still write into this CTA

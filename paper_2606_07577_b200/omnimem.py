@@ -310,14 +310,3 @@ class OmniMem:
         launches = C.c_int32(0)
         self._check(self.lib.omnimem_get_stage_ms(self.ctx, out, C.byref(launches)), "omnimem_get_stage_ms")
         return {s: float(out[i]) for i, s in enumerate(STAGES)}, int(launches.value)
-
-
-# Module-level aliases with the C names (ctx first), for callers that think in terms of include/omnimem.h.
-def omnimem_score(ctx: OmniMem, *a, **k): return ctx.score(*a, **k)
-def omnimem_allocate(ctx: OmniMem, *a, **k): return ctx.allocate(*a, **k)
-def omnimem_select(ctx: OmniMem, *a, **k): return ctx.select(*a, **k)
-def omnimem_calibrate_accumulate(ctx: OmniMem, *a, **k): return ctx.calibrate_accumulate(*a, **k)
-def omnimem_calibrate_budgets(ctx: OmniMem, *a, **k): return ctx.calibrate_budgets(*a, **k)
-def omnimem_compact(ctx: OmniMem, *a, **k): return ctx.compact(*a, **k)
-def omnimem_compress_chunk(ctx: OmniMem, *a, **k): return ctx.compress_chunk(*a, **k)
-def omnimem_compress_chunk_host(ctx: OmniMem, *a, **k): return ctx.compress_chunk_host(*a, **k)

@@ -325,9 +325,13 @@ def test_budget_above_capacity_is_clamped_not_written_out_of_bounds():
     eng.compact(src, chunk, ivview, iaview, big_v, big_a, dst)
     torch.cuda.synchronize()
     Kv = wl.n_v + wl.Nn_v
-    want_v = min(Kv, cap)
+    want_v = min(Kv, cap)                                                # 5000 -> 900 visual rows, nothing left for audio
     assert torch.equal(dst.n_v, torch.full_like(dst.n_v, want_v)) and torch.equal(dst.n, torch.full_like(dst.n, cap))
-    assert bool((ivview[:, :, :want_v] == torch.arange(want_v, device="cuda", dtype=torch.int32)).all())   # M >= K: identity, cut at cap
+    p = ref_params(wl, L)
+    iv_ref, _ = ref.select(p, sc.psi_v.cpu().numpy(), sc.psi_a.cpu().numpy(), x["n_v"].numpy(), x["n"].numpy(),
+                           np.full(L, want_v, np.int32), np.zeros(L, np.int32))
+    assert np.array_equal(ivview[:, :, :want_v].cpu().numpy(), iv_ref[:, :, :want_v])    # the clamped M: a real top-900 of 1100
+    assert bool((iaview == -7).all())
     for gd, fill in ((kguard, SENT), (vguard, SENT), (ivguard, -7), (iaguard, -7)):
         assert bool((gd == fill).all()), "wrote past the end of a buffer"
     neg = torch.full((L,), -5, dtype=torch.int32, device="cuda")

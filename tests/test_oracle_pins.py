@@ -139,6 +139,86 @@ def test_attention_ignores_rows_beyond_n():
     assert np.array_equal(l1, l2)
 
 
+# ------------------------------------------------------------------------------------------ A1 (Eq.1, NEXT-1)
+def torch_mhsa(p, x, l):
+    """Library special case: torch fp64 softmax(QK^T c + mask) @ V over the concatenated keys / values."""
+    Nc, Nn, G = int(x["n"][l]), p.Nn, p.Hq // p.Hkv
+    Y = torch.zeros(p.Hq, Nn, p.D, dtype=torch.float64)
+    for j in range(p.Hq):
+        h = j // G
+        K = torch.cat([torch.from_numpy(x["cacheK"][l, h, :Nc]), torch.from_numpy(x["chunkK"][l, h])], 0)
+        V = torch.cat([torch.from_numpy(x["cacheV"][l, h, :Nc]), torch.from_numpy(x["chunkV"][l, h])], 0)
+        mask = torch.ones(Nn, Nc + Nn, dtype=torch.bool)
+        if p.causal:
+            mask[:, Nc:] = torch.tril(torch.ones(Nn, Nn, dtype=torch.bool))
+        Y[j] = torch.nn.functional.scaled_dot_product_attention(torch.from_numpy(x["Q"][l, j])[None], K[None], V[None],
+                                                                attn_mask=mask[None], scale=1.0 / math.sqrt(p.D))[0]
+    return Y.numpy()
+
+
+@pytest.mark.parametrize("causal", [1, 0])
+@pytest.mark.parametrize("shape", [dict(), dict(Hq=6, Hkv=2, D=16, cap=20, n=(13,), n_v=(8,), Nn_v=7, Nn_a=2),
+                                   dict(L=2, Hq=2, Hkv=2, D=4, cap=5, n=(5, 0), n_v=(2, 0), Nn_v=1, Nn_a=6)])
+def test_mhsa_matches_torch_sdpa(causal, shape):
+    """Eq.1: Y against torch's fp64 scaled_dot_product_attention with the explicit mask of R3; the LSE it returns
+    is the one O2 returns (one routine cannot drift from the other); absY bounds |Y|."""
+    p, x = make(causal=causal, **shape)
+    Y, lse, absY = ref.mhsa(p, x["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"], want_abs=True)
+    for l in range(p.L):
+        np.testing.assert_allclose(Y[l], torch_mhsa(p, x, l), rtol=1e-12, atol=1e-13)
+    _, lse2, _ = ref.attention(p, x["cacheK"], x["n"], x["chunkK"], x["Q"])
+    np.testing.assert_allclose(lse, lse2, rtol=1e-14, atol=1e-14)
+    assert np.all(np.abs(Y) <= absY + 1e-12)
+
+
+def test_mhsa_rational_golden_and_closed_forms():
+    """Golden worked by hand (tests/golden/mhsa_rational.txt).  Closed forms: q = 0 makes every visible key equally
+    likely, so Y_i is the running mean of the visible value rows (causal); values that do not depend on the key pass
+    through unchanged (rows sum to one); one key with a huge logit returns its value row; GQA: query head j reads the
+    keys AND the values of KV head j // G."""
+    p = ref.RefParams(L=1, Hq=1, Hkv=1, D=1, cache_cap=1, Nn_v=2, Nn_a=0, scale=1.0)
+    cacheK, cacheV = np.array([[[[math.log(1.0)]]]]), np.array([[[[6.0]]]])
+    chunkK, chunkV = np.log(np.array([2.0, 3.0])).reshape(1, 1, 2, 1), np.array([12.0, -6.0]).reshape(1, 1, 2, 1)
+    Y, lse, _ = ref.mhsa(p, cacheK, cacheV, [1], chunkK, chunkV, np.ones((1, 1, 2, 1)))
+    for line in open(os.path.join(GOLD, "mhsa_rational.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        i, y, el = line.split()
+        assert abs(Y[0, 0, int(i), 0] - float(y)) < 1e-12 and abs(math.exp(lse[0, 0, int(i)]) - float(el)) < 1e-12
+    p, x = make(Hq=4, Hkv=2, D=8, cap=12, n=(9,), n_v=(6,), Nn_v=5, Nn_a=3)
+    Y, _, _ = ref.mhsa(p, x["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], 0 * x["Q"])
+    for h in range(2):
+        V = np.concatenate([x["cacheV"][0, h, :9], x["chunkV"][0, h]], 0)
+        for i in range(p.Nn):
+            for g in range(2):
+                np.testing.assert_allclose(Y[0, 2 * h + g, i], V[:9 + i + 1].mean(0), rtol=1e-13)     # running mean
+    const = np.broadcast_to(rnd(1, 2, 1, 8, seed=9), (1, 2, 12, 8))
+    Y, _, _ = ref.mhsa(p, x["cacheK"], const, x["n"], x["chunkK"], const[:, :, :8], x["Q"])
+    np.testing.assert_allclose(Y[0, :, :, :], np.repeat(const[0, :, :1], 2, 0).repeat(8, 1), rtol=1e-13)
+    xk = {k: v.copy() for k, v in x.items()}
+    xk["cacheK"][0, 1, 4] = 60.0 * np.sign(x["Q"][0, 3, 2])                    # KV head 1, cached row 4 dominates for q head 3, query 2
+    Y, _, _ = ref.mhsa(p, xk["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+    np.testing.assert_allclose(Y[0, 3, 2], x["cacheV"][0, 1, 4], atol=1e-9)
+    np.testing.assert_allclose(Y[0, :2], ref.mhsa(p, x["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"])[0][0, :2])  # head 0 untouched
+
+
+def test_mhsa_lse_feeds_the_column_sums():
+    """The point of NEXT-1: the LSE that the attention forward emits, fed to Eq.6's column sums as exp(z - lse), gives
+    the importance of O2 (the two-pass formulation and the forward + one-pass formulation are the same function)."""
+    p, x = make(Hq=4, Hkv=2, D=8, cap=12, n=(9,), n_v=(6,), Nn_v=5, Nn_a=3)
+    _, lse, _ = ref.mhsa(p, x["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+    a_log, _, _ = ref.attention(p, x["cacheK"], x["n"], x["chunkK"], x["Q"])
+    a = np.zeros_like(a_log)
+    for h in range(2):
+        K = np.concatenate([x["cacheK"][0, h, :9], x["chunkK"][0, h]], 0)
+        for g in range(2):
+            z = x["Q"][0, 2 * h + g] @ K.T / math.sqrt(8)
+            P = np.exp(z - lse[0, 2 * h + g][:, None])
+            P[:, 9:] *= np.tril(np.ones((8, 8)))
+            a[0, h, :17] += P.sum(0)
+    np.testing.assert_allclose(a, a_log, rtol=1e-12, atol=1e-14)
+
+
 def test_split_segment_maps():
     """O1 / Eq.3: visual = cached visual ++ new visual, audio = cached audio ++ new audio (R9)."""
     p, x = make()
