@@ -139,6 +139,22 @@ OMNIMEM_API int32_t omnimem_seg_cap(const omnimem_ctx* ctx, int32_t modality);
 OMNIMEM_API const char* omnimem_strerror(int status);              /* static string                                     */
 OMNIMEM_API const char* omnimem_last_cuda_error(const omnimem_ctx* ctx); /* cudaGetErrorString of the last CUDA failure  */
 
+/* ---- the step before the path: the chunk's attention forward (Eq.1, Eq.2) ---- */
+/* Y_c = MHSA(Q_c, K_c, V_c, O_c, P_c): for every layer l, query head j and chunk query i
+ *     y[l, j, i, :] = sum_k softmax_k(c <q_i, k_k>) v_k      over the logical key order of "Conventions"
+ * (cached visual, cached audio, chunk rows; ONE joint softmax, R2; causal inside the chunk, R3; query head j reads
+ * KV head j / G, R5), and lse_out[l, j, i] = log sum_k exp(c <q_i, k_k>) (natural log) -- exactly the array
+ * omnimem_chunk.lse takes, so that omnimem_compress_chunk on the same chunk skips score pass 1: the forward a model
+ * runs anyway (Eq.1) makes Eq.6 a single pass over Q K^T.
+ * y: DEVICE [L, Hq, Nn, D] of the context dtype (bf16: fp32 accumulation, P rounded to bf16 before P V, Y rounded once);
+ * lse_out: DEVICE float [L, Hq, Nn].  Both required.  chunk->lse, ->h and ->modality are ignored (the mask follows the
+ * storage order of the chunk rows, which is the temporal order in both chunk layouts).  bf16 with D = 128 runs on
+ * tcgen05 (tensor memory accumulators for S and O, TMA-fed K / V ring); fp32 and D = 64 on a SIMT kernel.
+ * Rows n[l] .. cache_cap of the cache buffers are never read into a result.  Nn = 0: nothing is written.
+ * Errors: INVALID_ARG, CAPACITY (Nn_v > max_chunk_v, Nn_a > max_chunk_a), WORKSPACE_TOO_SMALL, CUDA_ERROR. */
+OMNIMEM_API int omnimem_attend(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, void* y, float* lse_out,
+                   void* ws, size_t ws_bytes, void* stream);
+
 /* ---- stage 1-3a: importance, redundancy, psi, AVBA statistics (Eq.6-10, Eq.13) ------------------------------- */
 /* src, chunk, out: HOST structs holding DEVICE pointers.  Launches: [LSE pass unless chunk->lse] -> column-sum pass
  * -> cosine pass -> finalize (psi, partial statistics) -> statistics.  Errors: INVALID_ARG, CAPACITY (Nn_v > max_chunk_v,
@@ -224,7 +240,8 @@ enum {
   OMNIMEM_STAGE_ALLOCATE = 4,
   OMNIMEM_STAGE_SELECT = 5,
   OMNIMEM_STAGE_COMPACT = 6,
-  OMNIMEM_N_STAGES = 7
+  OMNIMEM_STAGE_ATTEND = 7,   /* omnimem_attend (not part of the fused step) */
+  OMNIMEM_N_STAGES = 8
 };
 OMNIMEM_API int omnimem_set_profiling(omnimem_ctx* ctx, int32_t enabled);
 /* HOST out[OMNIMEM_N_STAGES]: milliseconds of each stage in the most recent call (0 for stages that did not run);

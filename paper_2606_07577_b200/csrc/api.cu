@@ -390,6 +390,25 @@ int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chun
   return run_score(ctx, p, b, (cudaStream_t)stream);
 }
 
+int omnimem_attend(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, void* y, float* lse_out, void* ws,
+                   size_t ws_bytes, void* stream) {
+  if (!ctx || !y || !lse_out || !ws) return OMNIMEM_INVALID_ARG;
+  int rc = check_cache(src);
+  if (rc) return rc;
+  rc = check_chunk(ctx, chunk, true);
+  if (rc) return rc;
+  if (ws_bytes < ws_layout(ctx).total) return OMNIMEM_WORKSPACE_TOO_SMALL;
+  begin_call(ctx);
+  cudaStream_t st = (cudaStream_t)stream;
+  StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);
+  StepBuffers b{};
+  b.cacheK = src->k; b.cacheV = src->v; b.chunkK = chunk->k; b.chunkV = chunk->v; b.Q = chunk->q;
+  StageTimer t(ctx, st, OMNIMEM_STAGE_ATTEND);
+  cudaError_t e = ctx->use_tc ? launch_attend_tc(ctx, p, b, y, lse_out, st, &ctx->launches)
+                              : launch_attend_simt(ctx, p, b, y, lse_out, st, &ctx->launches);
+  return e == cudaSuccess ? OMNIMEM_OK : fail_cuda(ctx, e);
+}
+
 int omnimem_allocate(omnimem_ctx* ctx, const double* stats, const int32_t* n_v, const int32_t* n, int32_t Nn_v,
                      int32_t Nn_a, const int32_t* layer_budget, int64_t total_budget, int32_t* M_v, int32_t* M_a,
                      int32_t* layer_budget_out, void* stream) {

@@ -1,0 +1,369 @@
+// The chunk's attention forward (Eq.1, Eq.2) for bf16, head_dim 128, on tcgen05 / TMEM / TMA (sm_100a):
+//     Y_c = MHSA(Q_c, [K_v ; K_a ; K_c], [V_v ; V_a ; V_c]),   and the row log-sum-exp of its softmax.
+// It is the step BEFORE the compression path: the LSE it writes is what Eq.6's column sums
+// need, so a caller that runs this forward passes `lse` to omnimem_compress_chunk and score pass 1 disappears.
+//
+// One CTA = 256 queries of one query head = two 128-row sub-tiles that take turns on the tensor pipe:
+//   S_s = Q_s K_j^T   (SS mode: Q from shared memory, staged once; K tiles stream through a 4-slot ring shared with V)
+//   softmax threads (one per query row): P = 2^(c2 S - m) in fp32, row sum l in fp32, P rounded to bf16 and written
+//   back into tensor memory ON TOP of S_s (columns [0, 64) of its 128)
+//   O_s += P_s V_j    (TS mode: P from tensor memory, V tile MN-major from shared memory)
+// Issue order on the tensor pipe: O_0(j), S_0(j+1), O_1(j), S_1(j+1): while one sub-tile's softmax runs, the other's
+// two products execute.  Tensor memory: S_0, S_1 at columns [0, 256), O_0, O_1 at [256, 512).
+// The running reference m is LAZY, as in score pass 1: a tile's exponentials are taken against m as it stands; only if
+// that could overflow (tile sum not below 2^100) the thread takes the exact path: tile maximum, new reference, and a
+// rescale of its O row in tensor memory (possible because nothing of this sub-tile is in flight at that point).
+// Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-11 = softmax / epilogue (sub-tile x lane quarter).
+#include <cuda.h>
+#include <math.h>
+
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace omnimem {
+
+namespace {
+
+constexpr int kT = 128;               // rows per tile (queries per sub-tile, keys per streamed tile) and head_dim
+constexpr int kTileB = kT * 128 * 2;  // 32 KB: two 64-element K-blocks of 16 KB
+constexpr int kSlots = 4;             // ring of K / V tiles: K_j, V_j, K_{j+1}, V_{j+1}
+constexpr int kThr = 384;             // 4 control warps + 8 softmax warps
+constexpr int kOffQ = 0;                          // [2 sub][32 KB]
+constexpr int kOffKV = 2 * kTileB;                // [kSlots][32 KB]
+constexpr int kOffBar = kOffKV + kSlots * kTileB;
+constexpr size_t kSmem = 1024 + kOffBar + 256;
+constexpr uint32_t kColS = 0, kColO = 256;        // tensor-memory columns
+
+// D = f32, A = B = bf16, N = 128, M = 128; bit 16: B is MN-major (the V tile: rows = keys, head_dim contiguous)
+constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kT >> 3) << 17) | ((uint32_t)(kT >> 4) << 24);
+constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
+
+struct AttendArgs {
+  StepParams p;
+  __nv_bfloat16* y;   // [L, Hq, Nn, 128]
+  float* lse_nat;     // [L, Hq, Nn]
+};
+
+__device__ __forceinline__ void tc_ld32x(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tc_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+               :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+                  "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {   // element 2c in the low half: the A-operand word
+  uint32_t d;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
+
+__global__ void __launch_bounds__(kThr, 1)
+attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapKc,
+                 const __grid_constant__ CUtensorMap mapKn, const __grid_constant__ CUtensorMap mapVc,
+                 const __grid_constant__ CUtensorMap mapVn, const AttendArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const StepParams& p = a.p;
+  const int l = blockIdx.z, jh = blockIdx.y, h = jh / p.G;
+  const int n = uniform(p.n[l]);
+  const int row0 = blockIdx.x * 2 * kT;                         // first query of this CTA
+  const int nct = (n + kT - 1) / kT, nnt = (p.Nn + kT - 1) / kT;  // cache tiles, chunk tiles
+  int nt[2];
+  for (int s = 0; s < 2; ++s) {
+    const int r0 = row0 + s * kT;
+    nt[s] = r0 < p.Nn ? nct + (p.causal ? min(nnt, r0 / kT + 1) : nnt) : 0;   // R3: chunk key t visible iff t <= i
+  }
+  const int ntiles = max(nt[0], nt[1]);
+  if (ntiles == 0) return;
+
+  const uint32_t s_raw = smem_u32(smem_raw);
+  const uint32_t sBase = (s_raw + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sBase - s_raw);
+  const uint32_t sQ = sBase + kOffQ, sKV = sBase + kOffKV, bars = sBase + kOffBar;
+  const uint32_t bar_q = bars, bar_full = bars + 8, bar_empty = bar_full + 8 * kSlots;
+  const uint32_t bar_s = bar_empty + 8 * kSlots, bar_p = bar_s + 16, bar_o = bar_p + 16;
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBar + 8 + 16 * kSlots + 48);
+  const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    mbar_init(bar_q, 1);
+    for (int i = 0; i < kSlots; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_p + 8 * s, 4); mbar_init(bar_o + 8 * s, 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
+  const int lhq = l * p.Hq + jh, lhk = l * p.Hkv + h;
+
+  if (warp == 0) {
+    // ===================== TMA producer: Q once, then K_0, V_0, K_1, V_1, ... through the ring =====================
+    if (elect_one()) {
+      mbar_expect_tx(bar_q, (nt[1] > 0 ? 2 : 1) * kTileB);
+      for (int s = 0; s < 2; ++s)
+        if (nt[s] > 0)
+          for (int kb = 0; kb < 2; ++kb) tma_load_3d(sQ + s * kTileB + kb * (kTileB / 2), &mapQ, kb * 64, row0 + s * kT, lhq, bar_q);
+    }
+    __syncwarp();
+    int slot = 0, ph = 1;
+    for (int j = 0; j < ntiles; ++j) {
+      const bool cache = j < nct;
+      const int r0 = (cache ? j : j - nct) * kT;
+      for (int t = 0; t < 2; ++t) {   // t = 0: K tile, t = 1: V tile
+        mbar_wait(bar_empty + 8 * slot, ph);
+        if (elect_one()) {
+          mbar_expect_tx(bar_full + 8 * slot, kTileB);
+          const CUtensorMap* m = t == 0 ? (cache ? &mapKc : &mapKn) : (cache ? &mapVc : &mapVn);
+          for (int kb = 0; kb < 2; ++kb) tma_load_3d(sKV + slot * kTileB + kb * (kTileB / 2), m, kb * 64, r0, lhk, bar_full + 8 * slot);
+        }
+        __syncwarp();
+        if (++slot == kSlots) { slot = 0; ph ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    int slot = 0, ph = 0;             // ring position of the next tile to consume (K_0, V_0, K_1, ...)
+    auto advance = [&]() { if (++slot == kSlots) { slot = 0; ph ^= 1; } };
+    auto issue_s = [&](int s, int kslot) {   // S_s = Q_s K^T
+      if (elect_one()) {
+        const uint64_t a_desc = umma_desc_sw128(sQ + s * kTileB), b_desc = umma_desc_sw128(sKV + kslot * kTileB);
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+          const uint64_t koff = (uint64_t)(((kk >> 2) * (kTileB / 2) + (kk & 3) * 32) >> 4);
+          tc_mma_bf16(tmem_base + kColS + s * kT, a_desc + koff, b_desc + koff, kIdescQK, kk > 0 ? 1u : 0u);
+        }
+        tc_commit(bar_s + 8 * s);
+      }
+      __syncwarp();
+    };
+    auto issue_o = [&](int s, int vslot, int j) {   // O_s += P_s V
+      mbar_wait(bar_p + 8 * s, j & 1);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t b_desc = umma_desc_sw128_mn(sKV + vslot * kTileB, kTileB / 2);
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)   // 16 keys per step: 8 TMEM columns of P, 16 rows (2048 B) of the V tile
+          tc_mma_bf16_ts(tmem_base + kColO + s * kT, tmem_base + kColS + s * kT + kk * 8, b_desc + (uint64_t)((kk * 2048) >> 4),
+                         kIdescPV, (j > 0 || kk > 0) ? 1u : 0u);
+        tc_commit(bar_o + 8 * s);
+      }
+      __syncwarp();
+    };
+    mbar_wait(bar_q, 0);
+    mbar_wait(bar_full + 8 * slot, ph);   // K_0
+    tc_fence_after();
+    for (int s = 0; s < 2; ++s) if (nt[s] > 0) issue_s(s, slot);
+    if (elect_one()) tc_commit(bar_empty + 8 * slot);
+    __syncwarp();
+    advance();
+    for (int j = 0; j < ntiles; ++j) {
+      const int vslot = slot, vph = ph;
+      advance();
+      const int kslot = slot;
+      mbar_wait(bar_full + 8 * vslot, vph);   // V_j
+      if (j == nct - 1 && (n & (kT - 1)) != 0) {
+        // the last cache tile is ragged: rows >= n of the V tile are stale cache rows.  Their P columns are zero, but
+        // 0 * (Inf or NaN bits) would poison O: zero those rows in shared memory (a row is one 128-byte line per K-block)
+        const int first = n - j * kT;
+        for (int idx = lane; idx < (kT - first) * 16; idx += 32) {
+          const int r = first + (idx >> 4), c = idx & 15;
+          const uint32_t addr = sKV + vslot * kTileB + (c >> 3) * (kTileB / 2) + r * 128 + (c & 7) * 16;
+          asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0) : "memory");
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+      }
+      tc_fence_after();
+      if (j < nt[0]) issue_o(0, vslot, j);
+      if (j + 1 < ntiles) { mbar_wait(bar_full + 8 * kslot, ph); tc_fence_after(); }   // K_{j+1}
+      if (j + 1 < nt[0]) issue_s(0, kslot);
+      if (j < nt[1]) issue_o(1, vslot, j);
+      if (elect_one()) tc_commit(bar_empty + 8 * vslot);
+      __syncwarp();
+      if (j + 1 < nt[1]) issue_s(1, kslot);
+      if (j + 1 < ntiles) {
+        if (elect_one()) tc_commit(bar_empty + 8 * kslot);
+        __syncwarp();
+        advance();
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== softmax / epilogue: thread = one query row of sub-tile s =====================
+    const int s = (warp - 4) >> 2, q4 = warp & 3;
+    const int r = q4 * 32 + lane, i = row0 + s * kT + r;
+    if (nt[s] > 0) {
+      const float c2 = p.scale_log2e;
+      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+      const uint32_t tS = t_lane + kColS + s * kT, tO = t_lane + kColO + s * kT;
+      float m_ref = -INFINITY, lsum = 0.f;
+      for (int j = 0; j < nt[s]; ++j) {
+        int limit;                               // visible key columns of this tile for this row
+        if (j < nct) limit = n - j * kT;
+        else {
+          const int t0 = (j - nct) * kT;
+          limit = p.Nn - t0;
+          if (p.causal) limit = min(limit, i - t0 + 1);
+        }
+        mbar_wait(bar_s + 8 * s, j & 1);
+        tc_fence_after();
+        uint32_t pk[64];                         // the tile's P row, bf16 pairs
+        float tsum;
+        // exponentials of the tile against reference `mref`; fills pk, returns the fp32 row sum
+        auto exp_tile = [&](float mref) {
+          float z[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            uint32_t v[32];
+            tc_ld32x(tS + c * 32, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; e += 2) {
+              float p0 = ex2(fmaf(__uint_as_float(v[e]), c2, -mref)), p1 = ex2(fmaf(__uint_as_float(v[e + 1]), c2, -mref));
+              if (limit < kT) { p0 = c * 32 + e < limit ? p0 : 0.f; p1 = c * 32 + e + 1 < limit ? p1 : 0.f; }
+              z[(e >> 1) & 3] += p0 + p1;
+              pk[c * 16 + (e >> 1)] = pack_bf16(p0, p1);
+            }
+          }
+          return (z[0] + z[1]) + (z[2] + z[3]);
+        };
+        bool ok = false;
+        if (j > 0) {                             // lazy reference: exact unless something overflows
+          tsum = exp_tile(m_ref);
+          ok = tsum < 1.2676506e30f && lsum < 1.2676506e30f;   // 2^100; false for inf and NaN
+        }
+        if (!__all_sync(0xffffffffu, ok)) {      // first tile, or the row's maximum jumped: exact path (warp-uniform)
+          float mx = -INFINITY;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            uint32_t v[32];
+            tc_ld32x(tS + c * 32, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; ++e) mx = fmaxf(mx, c * 32 + e < limit ? __uint_as_float(v[e]) : -INFINITY);
+          }
+          const float m_new = fmaxf(m_ref, mx * c2);
+          if (j > 0) {
+            // everything issued for this sub-tile has completed (S_s(j) is there, the tensor pipe runs in order) and
+            // O_s(j) waits for this thread: the O row can be rescaled in place
+            const float sc = ex2(m_ref - m_new);
+            lsum *= sc;
+            mbar_wait(bar_o + 8 * s, (j - 1) & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint32_t v[32];
+              tc_ld32x(tO + c * 32, v);
+              tc_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * sc);
+              tc_st32(tO + c * 32, v);
+            }
+          }
+          m_ref = m_new;
+          tsum = exp_tile(m_ref);
+        }
+        lsum += tsum;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tc_st16(tS + c * 16, pk + c * 16);   // P over the first 64 columns of S
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_p + 8 * s);
+      }
+      // epilogue: Y = O / l (bf16), lse = ln 2 (m + log2 l)
+      mbar_wait(bar_o + 8 * s, (nt[s] - 1) & 1);
+      tc_fence_after();
+      const float inv = 1.f / lsum;
+      const bool valid = i < p.Nn;
+      uint4* yrow = reinterpret_cast<uint4*>(a.y + ((long long)lhq * p.Nn + (valid ? i : 0)) * kT);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint32_t v[32];
+        tc_ld32x(tO + c * 32, v);
+        tc_wait_ld();
+        if (valid) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            uint4 o;
+            o.x = pack_bf16(__uint_as_float(v[8 * u]) * inv, __uint_as_float(v[8 * u + 1]) * inv);
+            o.y = pack_bf16(__uint_as_float(v[8 * u + 2]) * inv, __uint_as_float(v[8 * u + 3]) * inv);
+            o.z = pack_bf16(__uint_as_float(v[8 * u + 4]) * inv, __uint_as_float(v[8 * u + 5]) * inv);
+            o.w = pack_bf16(__uint_as_float(v[8 * u + 6]) * inv, __uint_as_float(v[8 * u + 7]) * inv);
+            yrow[c * 4 + u] = o;
+          }
+        }
+      }
+      if (valid) a.lse_nat[(long long)lhq * p.Nn + i] = (m_ref + log2f(lsum)) * 0.6931471805599453f;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// [outer, rows, 128] bf16 row-major -> 3-D map, box = 64 x 128 x 1, 128-byte swizzle, zero fill out of bounds
+cudaError_t make_map(EncodeTiledFn enc, CUtensorMap* m, const void* base, uint64_t rows, uint64_t outer) {
+  if (rows == 0 || outer == 0 || base == nullptr) { memset(m, 0, sizeof(*m)); return cudaSuccess; }
+  const cuuint64_t dims[3] = {128, rows, outer};
+  const cuuint64_t strides[2] = {256, rows * 256};
+  const cuuint32_t box[3] = {64, (cuuint32_t)kT, 1};
+  const cuuint32_t es[3] = {1, 1, 1};
+  const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+cudaError_t launch_attend_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, void* y, float* lse_nat,
+                             cudaStream_t st, int* launches) {
+  if (p.Nn == 0) return cudaSuccess;
+  omnimem_ctx* c = const_cast<omnimem_ctx*>(ctx);
+  if (!c->encode_tiled) {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (q != cudaDriverEntryPointSuccess || !f) return cudaErrorNotSupported;
+    c->encode_tiled = f;
+  }
+  EncodeTiledFn enc = (EncodeTiledFn)c->encode_tiled;
+  CUtensorMap mq, mkc, mkn, mvc, mvn;
+  cudaError_t e;
+  if ((e = make_map(enc, &mq, b.Q, p.Nn, (uint64_t)p.L * p.Hq)) != cudaSuccess) return e;
+  if ((e = make_map(enc, &mkc, b.cacheK, p.cache_cap, (uint64_t)p.L * p.Hkv)) != cudaSuccess) return e;
+  if ((e = make_map(enc, &mkn, b.chunkK, p.Nn, (uint64_t)p.L * p.Hkv)) != cudaSuccess) return e;
+  if ((e = make_map(enc, &mvc, b.cacheV, p.cache_cap, (uint64_t)p.L * p.Hkv)) != cudaSuccess) return e;
+  if ((e = make_map(enc, &mvn, b.chunkV, p.Nn, (uint64_t)p.L * p.Hkv)) != cudaSuccess) return e;
+  AttendArgs a{};
+  a.p = p;
+  a.y = (__nv_bfloat16*)y;
+  a.lse_nat = lse_nat;
+  e = cudaFuncSetAttribute(attend_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+  if (e != cudaSuccess) return e;
+  const dim3 grid((p.Nn + 2 * kT - 1) / (2 * kT), p.Hq, p.L);
+  ++*launches;
+  attend_tc_kernel<<<grid, kThr, kSmem, st>>>(mq, mkc, mkn, mvc, mvn, a);
+  return cudaGetLastError();
+}
+
+}  // namespace omnimem

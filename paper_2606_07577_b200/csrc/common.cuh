@@ -119,6 +119,10 @@ cudaError_t launch_lse_simt(const omnimem_ctx* ctx, const StepParams& p, const S
 cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_attend_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, void* y, float* lse_nat,
+                             cudaStream_t st, int* launches);
+cudaError_t launch_attend_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, void* y, float* lse_nat,
+                               cudaStream_t st, int* launches);
 cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,

@@ -144,6 +144,55 @@ __global__ void __launch_bounds__(128) colsum_simt_kernel(StepParams p, const T*
   }
 }
 
+// ---- Eq.1: Y[l,j,i,:] = sum_k exp(c <q_i, k_k> - lse[l,j,i]) v_k, given the row LSE of pass 1 ----
+// One block per query row: 128 keys at a time, thread t takes key t's weight, then thread d accumulates output column d
+// over the 128 weights (coalesced value reads).  fp32 throughout; serves fp32 inputs and head_dim != 128.
+__device__ __forceinline__ void store_out(float* p, float v) { *p = v; }
+__device__ __forceinline__ void store_out(__nv_bfloat16* p, float v) { *p = __float2bfloat16_rn(v); }
+
+template <typename T>
+__global__ void __launch_bounds__(128) attend_simt_kernel(StepParams p, const T* __restrict__ cacheK,
+                                                          const T* __restrict__ cacheV, const T* __restrict__ chunkK,
+                                                          const T* __restrict__ chunkV, const T* __restrict__ Q,
+                                                          const float* __restrict__ lse, T* __restrict__ Y) {
+  extern __shared__ float sm_att[];
+  const int i = blockIdx.x, j = blockIdx.y, l = blockIdx.z, t = threadIdx.x;
+  const int h = j / p.G, D = p.D;
+  float* sq = sm_att;         // [D]
+  float* sp = sm_att + D;     // [128]
+  const long long row = ((long long)l * p.Hq + j) * p.Nn + i;
+  for (int d = t; d < D; d += 128) sq[d] = to_float(Q[row * D + d]);
+  __syncthreads();
+  const int Nc = p.n[l];
+  const int nvis = p.causal ? Nc + i + 1 : Nc + p.Nn;
+  const long long lh = (long long)l * p.Hkv + h;
+  const T* kc = cacheK + lh * p.cache_cap * D;
+  const T* vc = cacheV + lh * p.cache_cap * D;
+  const T* kn = chunkK + lh * p.Nn * D;
+  const T* vn = chunkV + lh * p.Nn * D;
+  const float row_lse = lse[row];
+  float acc = 0.f;
+  for (int k0 = 0; k0 < nvis; k0 += 128) {
+    const int k = k0 + t;
+    float w = 0.f;
+    if (k < nvis) {
+      const T* kr = k < Nc ? kc + (long long)k * D : kn + (long long)(k - Nc) * D;
+      w = expf(p.scale * dot_row<T>(sq, kr, D) - row_lse);
+    }
+    sp[t] = w;
+    __syncthreads();
+    const int cnt = min(128, nvis - k0);
+    for (int d = t; d < D; d += 128)
+      for (int u = 0; u < cnt; ++u) {
+        const int kk = k0 + u;
+        const T* vr = kk < Nc ? vc + (long long)kk * D : vn + (long long)(kk - Nc) * D;
+        acc = fmaf(sp[u], to_float(vr[d]), acc);
+      }
+    __syncthreads();
+  }
+  for (int d = t; d < D; d += 128) store_out(Y + row * D + d, acc);
+}
+
 template <typename T>
 static cudaError_t lse_simt_t(const StepParams& p, const StepBuffers& b, cudaStream_t st) {
   const long long rows = (long long)p.L * p.Hq * p.Nn;
@@ -164,6 +213,28 @@ cudaError_t launch_lse_simt(const omnimem_ctx* ctx, const StepParams& p, const S
   if ((long long)p.L * p.Hq * p.Nn == 0) return cudaSuccess;
   ++*launches;
   return ctx->cfg.dtype == OMNIMEM_FP32 ? lse_simt_t<float>(p, b, st) : lse_simt_t<__nv_bfloat16>(p, b, st);
+}
+
+// pass 1 (LSE, natural log, into lse_nat) then the weighted value sum
+cudaError_t launch_attend_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, void* y, float* lse_nat,
+                               cudaStream_t st, int* launches) {
+  if ((long long)p.L * p.Hq * p.Nn == 0) return cudaSuccess;
+  StepBuffers b2 = b;
+  b2.lse = lse_nat;
+  b2.row_entropy = nullptr;
+  cudaError_t e = launch_lse_simt(ctx, p, b2, st, launches);
+  if (e != cudaSuccess) return e;
+  const dim3 grid((unsigned)p.Nn, (unsigned)p.Hq, (unsigned)p.L);
+  const size_t smem = (size_t)(p.D + 128) * sizeof(float);
+  ++*launches;
+  if (ctx->cfg.dtype == OMNIMEM_FP32)
+    attend_simt_kernel<float><<<grid, 128, smem, st>>>(p, (const float*)b.cacheK, (const float*)b.cacheV, (const float*)b.chunkK,
+                                                       (const float*)b.chunkV, (const float*)b.Q, lse_nat, (float*)y);
+  else
+    attend_simt_kernel<__nv_bfloat16><<<grid, 128, smem, st>>>(p, (const __nv_bfloat16*)b.cacheK, (const __nv_bfloat16*)b.cacheV,
+                                                               (const __nv_bfloat16*)b.chunkK, (const __nv_bfloat16*)b.chunkV,
+                                                               (const __nv_bfloat16*)b.Q, lse_nat, (__nv_bfloat16*)y);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,

@@ -18,6 +18,7 @@
 #include <math.h>
 
 #include "common.cuh"
+#include "tc_ptx.cuh"
 
 namespace omnimem {
 
@@ -56,151 +57,6 @@ constexpr int kKBlockBytesB = kRowsB * 128;  // one 64-element K-block of them
 #endif
 constexpr bool kLazyMax = OMNIMEM_LAZY_MAX != 0;   // pass 1: running reference instead of a per-tile maximum (see the loop)
 
-// ---- PTX wrappers -------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");  // suspend-time hint: sleep, do not spin
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
-          "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
-}
-// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t bar, uint32_t rank) {
-  uint32_t remote;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
-  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
-}
-// wait that also acquires what other CTAs of the cluster released (remote arrives)
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAITC_LOOP:\n\t"
-      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra WAITC_DONE;\n\t"
-      "bra WAITC_LOOP;\n\t"
-      "WAITC_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
-}
-__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {   // both CTAs' barriers at this offset
-  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
-               "h"((uint16_t)3) : "memory");
-}
-__device__ __forceinline__ void tc_mma_bf16_ts_pair(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
-      "r"(acc) : "memory");
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
-               "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ float4 lds128(uint32_t addr) {
-  float4 v;
-  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-  return v;
-}
-// one lane of a fully converged warp (the rest of the warp keeps executing the same uniform control flow)
-__device__ __forceinline__ bool elect_one() {
-  uint32_t pred;
-  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
-  return pred != 0;
-}
-__device__ __forceinline__ int uniform(int x) { return __shfl_sync(0xffffffffu, x, 0); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc),
-      "r"(acc) : "memory");
-}
-__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&r)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
-        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
-        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-      : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tc_st32(uint32_t taddr, const uint32_t (&r)[32]) {
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
-               :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
-}
-__device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// D[tmem] (+)= A[tmem] * B[smem]^T : the stationary operand is read from tensor memory, only B from shared memory
-__device__ __forceinline__ void tc_mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
-      "r"(acc) : "memory");
-}
-__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// packed fp32x2 arithmetic (sm_100): one issue slot for two lanes' worth of FMA / ADD
-__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
-  uint64_t r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ uint64_t pack2u(uint32_t lo, uint32_t hi) {
-  uint64_t r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
-  return r;
-}
-__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
-  uint64_t d;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-  return d;
-}
-__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
-  uint64_t d;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-__device__ __forceinline__ float ex2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
 // 2^x on the FMA/ALU pipes (Cody-Waite split + degree-4 minimax polynomial on [-0.5, 0.5], max relative error
 // 2.7e-6, mean error 4e-8; coefficients fitted for this file), two lanes per instruction
 // (fp32x2).  The MUFU ex2 pipe (16/clk/SM) is the limiter of both scoring passes (ncu: xu pipe 89 %), so
@@ -211,25 +67,23 @@ __device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
   return d;
 }
 #ifndef OMNIMEM_POLY_DEG
-#define OMNIMEM_POLY_DEG 4
-#endif
-#ifndef OMNIMEM_EXP_MUL
-#define OMNIMEM_EXP_MUL 0
+#define OMNIMEM_POLY_DEG 3
 #endif
 __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
   float x0, x1;
   unpack2(X, x0, x1);
-  const float kClamp = OMNIMEM_EXP_MUL ? -127.f : -126.f;
-  X = pack2(fmaxf(x0, kClamp), fmaxf(x1, kClamp));
+  // below -126.5 the result q * 2^-126 (q < 1) is a denormal; the sums that consume it are flush-to-zero adds (add2z),
+  // so everything below 2^-126 contributes exactly 0, as in the MUFU lanes (ex2.approx.ftz)
+  X = pack2(fmaxf(x0, -126.5f), fmaxf(x1, -126.5f));
   const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
   const uint64_t T = add2(X, MG);
   const uint64_t F = sub2(X, sub2(T, MG));
-#if OMNIMEM_POLY_DEG == 4
+#if OMNIMEM_POLY_DEG == 4    // max relative error 2.7e-6
   uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
   Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
   Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
   Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
-#else   // degree 3: max relative error 7.5e-5, equi-oscillating (the error of a sum of many terms averages out)
+#else                        // degree 3: max relative error 7.5e-5, equi-oscillating in f (it averages out over a sum)
   uint64_t Q = fma2(pack2(0.0551716685295105f, 0.0551716685295105f), F, pack2(0.2426111251115799f, 0.2426111251115799f));
   Q = fma2(Q, F, pack2(0.6932609677314758f, 0.6932609677314758f));
   Q = fma2(Q, F, pack2(0.9999280571937561f, 0.9999280571937561f));
@@ -237,17 +91,8 @@ __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
   float q0, q1, t0, t1;
   unpack2(Q, q0, q1);
   unpack2(T, t0, t1);
-#if OMNIMEM_EXP_MUL
-  // q * 2^round(x) as a multiplication by the float (round(x) + 127) << 23: round(x) = -127 gives the factor 0, so
-  // everything at or below 2^-127 is exactly 0, like the MUFU lanes (ex2.approx.ftz)
-  const uint64_t SC = pack2u(((uint32_t)__float_as_int(t0) << 23) + 0x3F800000u, ((uint32_t)__float_as_int(t1) << 23) + 0x3F800000u);
-  uint64_t R;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(R) : "l"(Q), "l"(SC));
-  return R;
-#else
   return pack2(__int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23)),   // q * 2^round(x)
                __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23)));
-#endif
 }
 #ifndef OMNIMEM_POLY_NUM
 #define OMNIMEM_POLY_NUM 2
@@ -268,15 +113,6 @@ __device__ __forceinline__ uint64_t ex2_pair(uint64_t X, int pi) {
   return pack2(ex2(x0), ex2(x1));
 }
 
-// UMMA shared-memory descriptor, K-major, 128-byte swizzle: 8-row groups are 1024 B apart (SBO), LBO unused,
-// descriptor version 1 (sm_100), layout type 2 (SWIZZLE_128B).
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
-  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)(1024u >> 4) << 32;
-  d |= (uint64_t)1 << 46;
-  d |= (uint64_t)2 << 61;
-  return d;
-}
 // Instruction descriptor: D = f32 (bit 4), A = B = bf16 (bits 7, 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
 constexpr uint32_t kIdescPair = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(2 * kTile >> 4) << 24);  // M = 256
 constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
@@ -639,8 +475,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           for (int e = 0; e < kHalf; e += 4) {
             const uint64_t A01 = fma2(pack2(x[e], x[e + 1]), c2c2, nm), A23 = fma2(pack2(x[e + 2], x[e + 3]), c2c2, nm);
             const uint64_t P01 = ex2_pair(A01, e / 2), P23 = ex2_pair(A23, e / 2 + 1);
-            z01 = add2(z01, P01);
-            z23 = add2(z23, P23);
+            z01 = add2z(z01, P01);
+            z23 = add2z(z23, P23);
             if (kEntropy) {  // sum p z2 over visible columns (masked ones have p = 0 but z2 = -inf)
               float a0, a1, a2, a3, p0, p1, p2, p3;
               unpack2(A01, a0, a1);
@@ -699,13 +535,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const uint64_t c2c2 = pack2(c2, c2), nm = pack2(-m_run, -m_run);
 #pragma unroll
           for (int e = 0; e < 32; e += 4) {
-            z01 = add2(z01, ex2_pair(fma2(pack2u(v0[e], v0[e + 1]), c2c2, nm), e / 2));
-            z23 = add2(z23, ex2_pair(fma2(pack2u(v0[e + 2], v0[e + 3]), c2c2, nm), e / 2 + 1));
+            z01 = add2z(z01, ex2_pair(fma2(pack2u(v0[e], v0[e + 1]), c2c2, nm), e / 2));
+            z23 = add2z(z23, ex2_pair(fma2(pack2u(v0[e + 2], v0[e + 3]), c2c2, nm), e / 2 + 1));
           }
 #pragma unroll
           for (int e = 0; e < 32; e += 4) {
-            z01 = add2(z01, ex2_pair(fma2(pack2u(v1[e], v1[e + 1]), c2c2, nm), 16 + e / 2));
-            z23 = add2(z23, ex2_pair(fma2(pack2u(v1[e + 2], v1[e + 3]), c2c2, nm), 16 + e / 2 + 1));
+            z01 = add2z(z01, ex2_pair(fma2(pack2u(v1[e], v1[e + 1]), c2c2, nm), 16 + e / 2));
+            z23 = add2z(z23, ex2_pair(fma2(pack2u(v1[e + 2], v1[e + 3]), c2c2, nm), 16 + e / 2 + 1));
           }
           float z0, z1, z2, z3;
           unpack2(z01, z0, z1);
@@ -799,10 +635,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             const uint64_t x1 = fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w));
             const uint64_t x2 = fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y));
             const uint64_t x3 = fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w));
-            acc01 = add2(acc01, ex2_pair(x0, 4 * e4));
-            acc23 = add2(acc23, ex2_pair(x1, 4 * e4 + 1));
-            acc01 = add2(acc01, ex2_pair(x2, 4 * e4 + 2));
-            acc23 = add2(acc23, ex2_pair(x3, 4 * e4 + 3));
+            acc01 = add2z(acc01, ex2_pair(x0, 4 * e4));
+            acc23 = add2z(acc23, ex2_pair(x1, 4 * e4 + 1));
+            acc01 = add2z(acc01, ex2_pair(x2, 4 * e4 + 2));
+            acc23 = add2z(acc23, ex2_pair(x3, 4 * e4 + 3));
           }
         };
         if (w.sub_valid[0] && w.sub_valid[1] && !(p.causal && w.a_chunk)) {

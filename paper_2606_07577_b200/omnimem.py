@@ -17,12 +17,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libomnimem.so")
 
 OMNIMEM_FP32, OMNIMEM_BF16 = 0, 1
-STAGES = ("lse", "colsum", "cosine", "finalize", "allocate", "select", "compact")
+STAGES = ("lse", "colsum", "cosine", "finalize", "allocate", "select", "compact", "attend")
 STAT_NAMES = ("Hn_v", "Hn_a", "sbar_v", "sbar_a", "C_v", "C_a", "Hn_all", "sbar_all")
 EXPORTS = ("omnimem_create", "omnimem_destroy", "omnimem_workspace_bytes", "omnimem_seg_cap", "omnimem_strerror",
            "omnimem_last_cuda_error", "omnimem_score", "omnimem_allocate", "omnimem_select", "omnimem_compact",
            "omnimem_compress_chunk", "omnimem_compress_chunk_host", "omnimem_set_profiling", "omnimem_get_stage_ms",
-           "omnimem_calibrate_accumulate", "omnimem_calibrate_budgets")
+           "omnimem_calibrate_accumulate", "omnimem_calibrate_budgets", "omnimem_attend")
 
 
 class OmniMemError(RuntimeError):
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
         lib.omnimem_last_cuda_error.restype = C.c_char_p
         lib.omnimem_score.argtypes = [vp, C.POINTER(omnimem_cache), C.POINTER(omnimem_chunk), C.POINTER(omnimem_scores),
                                       vp, C.c_size_t, vp]
+        lib.omnimem_attend.argtypes = [vp, C.POINTER(omnimem_cache), C.POINTER(omnimem_chunk), vp, vp, vp, C.c_size_t, vp]
         lib.omnimem_allocate.argtypes = [vp, vp, vp, vp, i32, i32, vp, i64, vp, vp, vp, vp]
         lib.omnimem_calibrate_accumulate.argtypes = [vp, vp, vp, vp]
         lib.omnimem_calibrate_budgets.argtypes = [vp, vp, i64, vp, vp, vp]
@@ -234,6 +235,19 @@ class OmniMem:
         self._check(self.lib.omnimem_score(self.ctx, C.byref(cs), C.byref(cc), C.byref(co), _ptr(self.ws), self.ws_bytes,
                                            _stream()), "omnimem_score")
         return out
+
+    def attend(self, src: Cache, chunk: Chunk, y: Optional[torch.Tensor] = None, lse: Optional[torch.Tensor] = None):
+        """P:54 Eq.1: the chunk's attention output y [L,Hq,Nn,D] (context dtype) and its row LSE [L,Hq,Nn] (fp32, natural
+        log: the array Chunk.lse takes)."""
+        Nn = chunk.Nn_v + chunk.Nn_a
+        if y is None:
+            y = torch.empty(self.L, self.Hq, Nn, self.D, dtype=self.torch_dtype, device=self.device)
+        if lse is None:
+            lse = torch.empty(self.L, self.Hq, Nn, dtype=torch.float32, device=self.device)
+        cs, cc = src.c(), chunk.c()
+        self._check(self.lib.omnimem_attend(self.ctx, C.byref(cs), C.byref(cc), _ptr(y), _ptr(lse), _ptr(self.ws), self.ws_bytes,
+                                            _stream()), "omnimem_attend")
+        return y, lse
 
     def allocate(self, stats: torch.Tensor, n_v: torch.Tensor, n: torch.Tensor, Nn_v: int, Nn_a: int,
                  layer_budget: Optional[torch.Tensor] = None, total_budget: int = 0):

@@ -1,0 +1,174 @@
+"""GPU parity of omnimem_attend (Eq.1) against the fp64 oracle's omnimem_ref_mhsa.
+
+Tolerances: LSE at rule (a) (absolute tol: an LSE error is a relative error of every exp(z - lse)).
+Y: the bf16 kernel rounds every weight p to bf16 before P V (bf16 keeps 8 significant bits: relative error <= 2^-8 just
+above a power of two, 2^-9 just below) and rounds Y once to bf16 (<= 2^-8 |Y|), so the rigorous bound is
+|Y_gpu - Y_ref| <= 2^-8 sum_k p_k |v_k| + 2^-8 |Y| <= 2^-7 * sum_k p_k |v_k| (the oracle returns that magnitude, absY);
+it is attained when one key takes the whole row (p ~ 1, Y ~ v).  fp32 inputs: 1e-5 of the same magnitude.
+Then the point of the row: attend -> compress_chunk(lse = ...) must keep what the two-pass step keeps.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ref
+from paper_2606_07577_b200 import inputs as I
+from tests.test_gpu_parity import SMALL2, SMALL3, SMALL4, dev_objs, engine_for
+from tests.util import TOL, compare_scores, ref_params, scores_to_numpy
+
+pytestmark = pytest.mark.gpu
+
+Y_TOL = {"fp32": 1e-5, "bf16": 2.0 ** -7}
+
+
+def compare_attend(wl, y_gpu, lse_gpu, Y_ref, lse_ref, absY, what=""):
+    tol = TOL[wl.dtype]
+    err_l = np.abs(lse_gpu.astype(np.float64) - lse_ref)
+    assert err_l.max() <= tol * np.maximum(1.0, np.abs(lse_ref)).max(), f"{what} lse: max err {err_l.max():.3e}"
+    assert np.all(err_l <= tol * np.maximum(1.0, np.abs(lse_ref))), f"{what} lse: max err {err_l.max():.3e}"
+    err = np.abs(y_gpu.astype(np.float64) - Y_ref)
+    bound = Y_TOL[wl.dtype] * absY + 1e-30
+    bad = err > bound
+    if bad.any():
+        i = np.unravel_index(np.argmax(err / bound), err.shape)
+        raise AssertionError(f"{what} Y: {int(bad.sum())}/{bad.size} outside the bound; worst at {i}: got {y_gpu[i]!r} exp "
+                             f"{Y_ref[i]!r} bound {bound[i]:.3e}")
+    return float((err / bound).max())
+
+
+def check_attend(wl, x=None, eng_kw=None, ref_kw=None, also_compress=True):
+    eng_kw, ref_kw = dict(eng_kw or {}), dict(ref_kw or {})
+    x = x if x is not None else I.full_inputs(wl)
+    L = x["Q"].shape[0]
+    wl = wl.replace(L=L)
+    p = ref_params(wl, L, **ref_kw)
+    Y_ref, lse_ref, absY = ref.mhsa(p, x["cacheK"], x["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"], want_abs=True)
+    eng = engine_for(wl, **eng_kw)
+    src, chunk = dev_objs(x, wl)
+    y, lse = eng.attend(src, chunk)
+    torch.cuda.synchronize()
+    worst = compare_attend(wl, y.float().cpu().numpy(), lse.cpu().numpy(), Y_ref, lse_ref, absY, wl.name)
+    if also_compress and wl.Nn:
+        from paper_2606_07577_b200.omnimem import Chunk
+        B = torch.full((L,), wl.budget, dtype=torch.int32, device="cuda")
+        out = []
+        for ch in (chunk, Chunk(chunk.k, chunk.v, chunk.q, wl.Nn_v, wl.Nn_a, lse=lse)):     # two-pass, then forward + one pass
+            dst = eng.new_cache()
+            iv, ia = eng.new_indices()
+            sc = eng.new_scores(wl.Nn)
+            M_v = torch.zeros(L, dtype=torch.int32, device="cuda")
+            M_a = torch.zeros_like(M_v)
+            eng.set_profiling(True)
+            eng.compress_chunk(src, ch, B, dst, out=sc, idx_v=iv, idx_a=ia, M_v=M_v, M_a=M_a)
+            torch.cuda.synchronize()
+            ms, _ = eng.stage_ms()
+            out.append((dst, iv, ia, M_v, M_a, sc, ms))
+        assert out[0][6]["lse"] > 0.0 and out[1][6]["lse"] == 0.0                           # pass 1 really was skipped
+        orc = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+        compare_scores(wl, x["n_v"].numpy(), x["n"].numpy(), scores_to_numpy(out[1][5]), orc, TOL[wl.dtype])
+        assert torch.equal(out[0][3], out[1][3]) and torch.equal(out[0][4], out[1][4])
+        same = 0
+        for l in range(L):
+            mv, ma = int(out[0][3][l]), int(out[0][4][l])
+            same += int((out[0][1][l, :, :mv] != out[1][1][l, :, :mv]).sum()) + int((out[0][2][l, :, :ma] != out[1][2][l, :, :ma]).sum())
+        assert same == 0, f"{same} kept indices differ between the two-pass step and forward + one pass"
+    eng.close()
+    return worst
+
+
+def test_attend_cfg1_fp32():
+    check_attend(I.CFG1)
+    check_attend(I.CFG1, eng_kw=dict(causal=0), ref_kw=dict(causal=0))
+
+
+@pytest.mark.parametrize("wl", [SMALL2, SMALL3, SMALL4], ids=lambda w: w.name)
+def test_attend_bf16_tcgen05_small(wl):
+    check_attend(wl)
+    check_attend(wl, eng_kw=dict(causal=0), ref_kw=dict(causal=0))
+
+
+def test_attend_bf16_simt_paths():
+    check_attend(SMALL2, eng_kw=dict(score_path=1))
+    check_attend(SMALL2.replace(D=64))
+
+
+def test_attend_edge_shapes():
+    check_attend(SMALL2.replace(n_v=0, n_a=0))                                                  # empty cache: first chunk of a stream
+    check_attend(SMALL2.replace(Nn_v=1, Nn_a=0))                                                # one-token chunk
+    check_attend(SMALL2.replace(n_v=128, n_a=128, Nn_v=128, Nn_a=128, budget=256, cache_cap=256))   # tile-aligned everywhere
+    check_attend(SMALL3.replace(n_v=1000, n_a=24, Nn_v=256, Nn_a=0, cache_cap=1100, budget=1100))   # one full CTA of queries
+    check_attend(SMALL3.replace(n_v=1, n_a=0, Nn_v=257, Nn_a=0, cache_cap=300, budget=258))         # a second CTA with one row
+    check_attend(SMALL3.replace(n_v=700, n_a=100, Nn_v=600, Nn_a=170, cache_cap=1700, budget=1000, Hq=14, Hkv=2))  # G = 7
+
+
+def test_attend_ignores_rows_beyond_n():
+    """Rows n .. cache_cap of the cache buffers may hold anything (stale rows, NaN bit patterns): masked key columns are
+    selected away and the value rows of the ragged last cache tile are zeroed in shared memory before P V."""
+    wl = SMALL2.replace(cache_cap=1100)
+    x = I.full_inputs(wl)
+    nc = wl.n_v + wl.n_a
+    x["cacheK"][:, :, nc:] = float("nan")
+    x["cacheV"][:, :, nc:] = float("nan")
+    x["cacheV"][:, :, nc + 1] = float("inf")
+    L = wl.L
+    p = ref_params(wl, L)
+    clean = {k: (v.clone() if torch.is_tensor(v) else v) for k, v in x.items()}
+    clean["cacheK"][:, :, nc:] = 0
+    clean["cacheV"][:, :, nc:] = 0
+    Y_ref, lse_ref, absY = ref.mhsa(p, clean["cacheK"], clean["cacheV"], x["n"], x["chunkK"], x["chunkV"], x["Q"], want_abs=True)
+    eng = engine_for(wl)
+    src, chunk = dev_objs(x, wl)
+    y, lse = eng.attend(src, chunk)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(y.float()).all()) and bool(torch.isfinite(lse).all())
+    compare_attend(wl, y.float().cpu().numpy(), lse.cpu().numpy(), Y_ref, lse_ref, absY)
+    eng.close()
+
+
+@pytest.mark.parametrize("mult", [12.0, 40.0])
+def test_attend_wide_logits_rebase_the_reference(mult):
+    """Keys with 64 x the norm in the first cache tile, the last cache tile and the chunk, softmax scale x 12 / x 40: the
+    lazy reference overflows in the middle of a row, the thread re-bases and rescales its O row in tensor memory."""
+    for wl in (SMALL2, SMALL3):
+        x = I.full_inputs(wl)
+        nc = wl.n_v + wl.n_a
+        x["cacheK"][:, :, 5] *= 64.0
+        x["cacheK"][:, :, nc - 3] *= 64.0
+        x["chunkK"][:, :, wl.Nn // 2] *= 64.0
+        c = mult / float(np.sqrt(wl.D))
+        check_attend(wl, x=x, eng_kw=dict(softmax_scale=c), ref_kw=dict(scale=c), also_compress=False)
+
+
+def oracle_one_kv_head(wl, x, l, h):
+    """The oracle's Eq.1 on the G query heads of KV head h of layer slot l (query heads are independent given their KV head)."""
+    G = wl.G
+    p = ref_params(wl.replace(Hq=G, Hkv=1), 1)
+    sl = lambda t, a, b: t[l:l + 1, a:b]
+    return ref.mhsa(p, sl(x["cacheK"], h, h + 1), sl(x["cacheV"], h, h + 1), x["n"][l:l + 1], sl(x["chunkK"], h, h + 1),
+                    sl(x["chunkV"], h, h + 1), sl(x["Q"], h * G, (h + 1) * G), want_abs=True)
+
+
+@pytest.mark.parametrize("wl,samples", [(I.CFG2, ((0, 0), (14, 3), (27, 1))), (I.CFG4, ((0, 7), (35, 2))), (I.CFG3, ((35, 5),))],
+                         ids=["cfg2", "cfg4", "cfg3"])
+def test_attend_full_size(wl, samples):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (one omnimem_attend over all layers): sampled
+    (layer, KV head) units in full against the oracle; every row of every layer: finite, and the LSE equal (to fp32
+    rounding) to the one score pass 1 computes."""
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
+    x = I.full_inputs(wl)
+    eng = OmniMem.for_workload(wl)
+    dev = eng.device
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+    y, lse = eng.attend(src, chunk)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(lse).all()) and bool(torch.isfinite(y.float()).all())
+    sc = eng.score(src, chunk, want_lse=True)
+    torch.cuda.synchronize()
+    assert float((sc.lse - lse).abs().max()) < 1e-4
+    G = wl.G
+    for l, h in samples:
+        Y_ref, lse_ref, absY = oracle_one_kv_head(wl, x, l, h)
+        compare_attend(wl, y[l:l + 1, h * G:(h + 1) * G].float().cpu().numpy(), lse[l:l + 1, h * G:(h + 1) * G].cpu().numpy(),
+                       Y_ref, lse_ref, absY, f"{wl.name} layer {l} kv head {h}")
+    eng.close()
