@@ -2,12 +2,15 @@
 """bench.py -- ms per chunk compression step (all layers) and KV tok/s of the OmniMem hot path on B200.
 
 A "step" is one `omnimem_compress_chunk` call: all five stages (score, AVBA budgets, select, compact) over every
-layer of one synthetic chunk.  Default workload = BASELINE.json configs[1] (Qwen2.5-Omni-7B-shaped, bf16).
+layer of one synthetic chunk.  BASELINE.json's `metric` names no config, so the line of record is the LARGEST
+single-GPU config, configs[2] (8B-shaped, 253 TFLOP per step); the same run also times configs[1] (the
+Qwen2.5-Omni-7B-shaped step, object "cfg2", same keys) and the 60-chunk stream of configs[4] (object "stream":
+p50 / p99 per chunk, total ingest tok/s), so that the driver records all three.  `--config N` runs one config only.
 `value` = KV tokens processed per second = Nk / t_step (Nk = cached + new rows per layer), whole job over N GPUs.
 Multi-GPU: the path does not shard in this repo (replicas only) -> N independent replicas,
 weak scaling, no data-path collective.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0|1..5] [--impl ours|reference]
 """
 from __future__ import annotations
 
@@ -177,7 +180,8 @@ def job_value(world: int, units_per_rank: float, seconds: float) -> float:
 
 
 # ------------------------------------------------------------------------------------------------ our arm
-def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
+def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int, cpu_baseline: bool = True):
+    """One config, device-resident and end to end; returns the JSON object (rank 0) or None."""
     import torch.distributed as dist
     from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
     dev = torch.device(f"cuda:{local_rank}")
@@ -238,6 +242,28 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     t_one_pass = ev2.elapsed_time(ev3) / 1e3
     del sc
 
+    # ---- NEXT-1 proper: the attention forward (Eq.1, omnimem_attend) writes Y and the LSE; the compression step then
+    # takes that LSE.  Timed: the forward alone, and forward + one-pass compression back to back.
+    y_out = torch.empty(wl.L, wl.Hq, wl.Nn, wl.D, dtype=wl.torch_dtype, device=dev)
+    lse_out = torch.empty(wl.L, wl.Hq, wl.Nn, dtype=torch.float32, device=dev)
+    chunk_fwd = Chunk(chunk.k, chunk.v, chunk.q, wl.Nn_v, wl.Nn_a, lse=lse_out)
+    for _ in range(2):
+        eng.attend(src, chunk, y_out, lse_out)
+        eng.compress_chunk(src, chunk_fwd, B, dst)
+    barrier()
+    ev8, ev9, ev10 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    ev8.record()
+    for _ in range(args.steps):
+        eng.attend(src, chunk, y_out, lse_out)
+    ev9.record()
+    for _ in range(args.steps):
+        eng.attend(src, chunk, y_out, lse_out)
+        eng.compress_chunk(src, chunk_fwd, B, dst)
+    ev10.record()
+    barrier()
+    t_fwd, t_fwd_step = ev8.elapsed_time(ev9) / 1e3, ev9.elapsed_time(ev10) / 1e3
+    del y_out, lse_out
+
     # ---- the same step replayed from a CUDA graph (the call is stream-ordered and never synchronises the host, so it
     # captures as is); matters for small, launch-bound shapes such as config 1
     t_graph = None
@@ -271,17 +297,21 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
     barrier()
     t_e2e = ev4.elapsed_time(ev5) / 1e3
 
-    t_total, t_e2e, t_one_pass = max_over_ranks([t_total, t_e2e, t_one_pass], dev, world)
+    t_total, t_e2e, t_one_pass, t_fwd, t_fwd_step = max_over_ranks([t_total, t_e2e, t_one_pass, t_fwd, t_fwd_step], dev, world)
     if t_graph is not None:
         t_graph = max_over_ranks([t_graph], dev, world)[0]
+    eng.close()
     if rank != 0:
-        return
+        return None
     t_step = t_total / args.steps
     stage_ms = {k: v / args.steps for k, v in stage_sum.items()}
     dom = "colsum" if stage_ms.get("colsum", 0) >= stage_ms.get("lse", 0) else "lse"
     t_dom = stage_ms[dom] / 1e3
     achieved = work["f_pass"] / t_dom / 1e12 if t_dom > 0 else 0.0
-    t_roof = max(2 * work["f_pass"] / (peaks["tf_sust"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
+    # P_TC = the measured BURST bf16 peak ("the stricter one"); the sustained figure is printed beside it
+    t_roof = max(2 * work["f_pass"] / (peaks["tf_burst"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
+    t_roof_sust = max(2 * work["f_pass"] / (peaks["tf_sust"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
+    traffic, traffic_src = ncu_traffic(wl.name, 2 if dom == "colsum" else 1)
     out = {
         "metric": "kv_tokens_per_s", "value": job_value(world, work["Nk"], t_step), "unit": "KV tok/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
@@ -295,23 +325,38 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
         "gpu_launches": launches,
         "stage_ms": stage_ms,
         "roofline": {"bound": "tensor", "kernel": f"score_tc_kernel<{2 if dom == 'colsum' else 1}> ({dom})",
-                     "achieved": achieved, "peak": peaks["tf_sust"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_sust"],
-                     "peak_source": f"{peaks['src']} bf16 sustained (kernel timed inside the step)",
-                     "frac_of_burst": achieved / peaks["tf_burst"], "traffic": NCU_TRAFFIC_BYTES.get(dom) if wl.name == I.CFG2.name else None,
+                     "achieved": achieved, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_burst"],
+                     "peak_source": f"{peaks['src']} bf16 burst (SURVEY.md 8(d): the stricter peak)",
+                     "peak_burst": peaks["tf_burst"], "peak_sustained": peaks["tf_sust"],
+                     "frac_of_sustained": achieved / peaks["tf_sust"], "frac_of_burst": achieved / peaks["tf_burst"],
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "algorithmic_flops_per_launch": work["f_pass"], "exps_per_launch": work["exps_pass"]},
         "step_roofline": {"t_roof_ms": t_roof * 1e3, "frac_two_pass": t_roof / t_step,
+                          "frac_two_pass_of_sustained": t_roof_sust / t_step,
                           "frac_one_pass_normalised": t_roof / 2 / t_step, "bytes": work["bytes"]["total"],
-                          "flops_two_pass": 2 * work["f_pass"]},
+                          "flops_two_pass": 2 * work["f_pass"], "target_60pct_ms": t_roof / 0.6 * 1e3},
     }
     t_one_pass /= args.steps
     out["supplied_lse"] = {"ms_per_step": t_one_pass * 1e3, "value": job_value(world, work["Nk"], t_one_pass), "unit": "KV tok/s",
                            "note": "row LSE supplied by the caller (chunk.lse): scoring pass 1 skipped; context, not the headline"}
+    t_fwd /= args.steps
+    t_fwd_step /= args.steps
+    f_fwd = 2 * work["f_pass"]                               # Q K^T and P V: 4 D flops per visible (q, k) pair
+    out["next1"] = {"forward_ms": t_fwd * 1e3, "forward_plus_compress_ms": t_fwd_step * 1e3,
+                    "two_pass_compress_ms": t_step * 1e3, "forward_plus_two_pass_ms": (t_fwd + t_step) * 1e3,
+                    "saved_ms_per_step": (t_fwd + t_step - t_fwd_step) * 1e3,
+                    "roofline": {"bound": "tensor", "kernel": "attend_tc_kernel", "achieved": f_fwd / t_fwd / 1e12, "unit": "TFLOP/s",
+                                 "peak": peaks["tf_burst"], "frac": f_fwd / t_fwd / 1e12 / peaks["tf_burst"],
+                                 "frac_of_sustained": f_fwd / t_fwd / 1e12 / peaks["tf_sust"], "algorithmic_flops_per_launch": f_fwd,
+                                 "traffic": None},
+                    "note": "omnimem_attend (Eq.1: Y and the row LSE) then omnimem_compress_chunk(lse=...): a model that runs this "
+                            "forward anyway pays forward_plus_compress instead of forward + two-pass"}
     out["derived"] = {"ingest_tok_per_s": world * wl.Nn / t_step, "layer_entries_per_s": world * wl.L * work["Nk"] / t_step,
                       "note": "SURVEY.md 8(d): chunk tokens ingested per second; (layer, KV entry) pairs scored and compacted per second"}
     if t_graph is not None:
         out["cuda_graph"] = {"ms_per_step": t_graph / args.steps * 1e3,
                              "note": "one omnimem_compress_chunk captured once and replayed (no profiling events)"}
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and cpu_baseline:
         from oracle import ref
         secs = oracle_sample_seconds(wl, 0, [0, 1][: wl.Hkv])
         nunits = min(2, wl.Hkv)
@@ -320,11 +365,11 @@ def run_ours(args, wl: I.Workload, rank: int, local_rank: int, world: int):
                                "ms_per_step": t_cpu * 1e3,
                                "sample": f"layer 0, KV heads 0-{nunits - 1} of {wl.Hkv} (all five stages, {secs:.1f} s), "
                                          f"scaled x{wl.L * wl.Hkv // nunits}"}
-    print(json.dumps(out), flush=True)
+    return out
 
 
 # ------------------------------------------------------------------------------------------------ streaming (cfg5)
-def run_stream(args, wl: I.Workload, local_rank: int):
+def measure_stream(args, wl: I.Workload, local_rank: int):
     """BASELINE.json configs[4]: `chunks` consecutive chunks from an empty cache, free-running on the device state
     (ping-pong caches, no host sync inside a step).  Per-chunk CUDA-event times -> p50 / p99 over all chunks and over
     the steady-state ones (cache full), total ingest tok/s = chunks * Nn / sum(t)."""
@@ -335,7 +380,10 @@ def run_stream(args, wl: I.Workload, local_rank: int):
     src, dst = eng.new_cache(), eng.new_cache()
     B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
     n_chunks = args.chunks or wl.steps
+    from concurrent.futures import ThreadPoolExecutor
+    pool = ThreadPoolExecutor(max_workers=1)                  # the next chunk is drawn on the host while this one runs
     x = I.full_inputs(wl, step=0, with_cache=False)
+    nxt = pool.submit(I.full_inputs, wl, step=1, with_cache=False) if n_chunks > 1 else None
     chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
     scratch = eng.new_cache()
     for _ in range(max(args.warmup, 3)):                      # warm-up on a scratch destination: the stream state is untouched
@@ -346,7 +394,8 @@ def run_stream(args, wl: I.Workload, local_rank: int):
     with ClockSampler(local_rank) as clk:
         for step in range(n_chunks):
             if step:
-                x = I.full_inputs(wl, step=step, with_cache=False)
+                x = nxt.result()
+                nxt = pool.submit(I.full_inputs, wl, step=step + 1, with_cache=False) if step + 1 < n_chunks else None
                 chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
             rows.append(int(src.n[0]) + wl.Nn)
             ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -360,7 +409,9 @@ def run_stream(args, wl: I.Workload, local_rank: int):
     steady = t[np.array(rows) >= wl.budget + wl.Nn] if any(r >= wl.budget + wl.Nn for r in rows) else t
     total_s = t.sum() / 1e3
     pct = lambda a, q: float(np.percentile(a, q))
-    print(json.dumps({
+    pool.shutdown()
+    eng.close()
+    return {
         "metric": "kv_tokens_per_s", "value": float(np.mean(rows)) / (t.mean() / 1e3), "unit": "KV tok/s", "n_gpus": 1,
         "steps": n_chunks, "warmup": max(args.warmup, 3), "ms_per_step": float(t.mean()), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype, "data": "synthetic",
@@ -371,11 +422,30 @@ def run_stream(args, wl: I.Workload, local_rank: int):
                    "steady_p99_ms": pct(steady, 99), "steady_chunks": int(len(steady)), "total_s": total_s,
                    "ingest_tok_per_s": n_chunks * wl.Nn / total_s, "ms_per_chunk": [round(v, 3) for v in times],
                    "rows_scored": rows},
-    }), flush=True)
+    }
 
 
-# per-launch DRAM bytes of the scoring kernels from the committed ncu --set full capture (profiles/); None = not captured
-NCU_TRAFFIC_BYTES = {"colsum": 1.7913e9, "lse": 1.7789e9}   # profiles/r01c_score_tc_full_cfg2.csv (CFG2 only)
+NCU_CAPTURES = {"cfg2_qwen25omni7b": "profiles/r02_score_tc_full_cfg2.csv"}   # committed `ncu --set full` summaries
+
+
+def ncu_traffic(workload: str, pass_no: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of score_tc_kernel<pass_no> from the committed ncu capture
+    of this workload (profiles/), read at run time.  Returns (bytes or None, source)."""
+    rel = NCU_CAPTURES.get(workload)
+    path = os.path.join(ROOT, rel) if rel else None
+    if not path or not os.path.exists(path):
+        return None, "no ncu --set full capture committed for this workload"
+    import csv
+    rows = list(csv.reader(open(path)))
+    col = next((i for i, c in enumerate(rows[0]) if f"score_tc_kernel<{pass_no}" in c), None)
+    if col is None:
+        return None, f"{rel}: kernel column not found"
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot = 0.0
+    for r in rows:
+        if r and r[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            tot += float(r[col]) * unit[r[1]]
+    return (tot or None), rel
 
 
 def main():
@@ -383,26 +453,41 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[i-1]; 2 = the config the metric is quoted on")
+    ap.add_argument("--config", type=int, default=0,
+                    help="BASELINE.json configs[i-1]; 0 (default) = the line of record: config 3 (largest) + objects cfg2 and stream (config 5)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunks", type=int, default=0, help="config 5 only: chunks in the stream (default: the config's 60)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    wl = I.CONFIGS[args.config]
+    wl = I.CONFIGS[args.config or 3]
     rank, local_rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":
         run_reference(args, wl, rank, world)
         return
     if wl.steps > 1 and world == 1:
-        run_stream(args, wl, local_rank)
+        print(json.dumps(measure_stream(args, wl, local_rank)), flush=True)
         return
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     try:
-        run_ours(args, wl, rank, local_rank, world)
+        out = measure_config(args, wl, rank, local_rank, world)
+        if args.config == 0:
+            # the other two workloads BASELINE.json singles out, in the same line so that the driver records them
+            torch.cuda.empty_cache()
+            cfg2 = measure_config(args, I.CFG2, rank, local_rank, world, cpu_baseline=False)
+            if rank == 0:
+                out["cfg2"] = cfg2
+            if world == 1:
+                torch.cuda.empty_cache()
+                st = measure_stream(args, I.CFG5, local_rank)
+                out["stream"] = {"workload": I.CFG5.name, "chunks": st["steps"], "ms_per_step_mean": st["ms_per_step"],
+                                 "kv_tok_per_s": st["value"], "clocks": st["clocks"],
+                                 **{k: v for k, v in st["stream"].items() if k not in ("ms_per_chunk", "rows_scored")}}
+        if rank == 0:
+            print(json.dumps(out), flush=True)
     finally:
         if world > 1:
             import torch.distributed as dist

@@ -12,7 +12,7 @@ using namespace omnimem;
 namespace {
 
 struct WsLayout {
-  size_t lse, cosn, partials, a_v, a_a, s_v, s_a, psi_v, psi_a, stats, M_v, M_a, idx_v, idx_a, total;
+  size_t lse, cosn, partials, a_v, a_a, la_v, la_a, s_v, s_a, psi_v, psi_a, stats, M_v, M_a, idx_v, idx_a, total;
 };
 
 size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
@@ -29,6 +29,8 @@ WsLayout ws_layout(const omnimem_ctx* c) {
   w.partials = take(L * 2 * (size_t)c->fin_blocks * 3 * sizeof(double));
   w.a_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
   w.a_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
+  w.la_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
+  w.la_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
   w.s_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
   w.s_a = take(L * Hkv * (size_t)c->seg_cap_a * sizeof(float));
   w.psi_v = take(L * Hkv * (size_t)c->seg_cap_v * sizeof(float));
@@ -111,6 +113,7 @@ int run_score(omnimem_ctx* c, const StepParams& p, StepBuffers& b, cudaStream_t 
   {
     StageTimer t(c, st, OMNIMEM_STAGE_COLSUM);
     e = c->use_tc ? launch_colsum_tc(c, p, b, st, &c->launches) : launch_colsum_simt(c, p, b, st, &c->launches);
+    if (e == cudaSuccess) e = launch_colsum_rescue(c, p, b, st, &c->launches);   // keys below fp32's range (R31)
     if (e != cudaSuccess) return fail_cuda(c, e);
   }
   {
@@ -141,6 +144,8 @@ void fill_buffers(const omnimem_ctx* c, const omnimem_cache* src, const omnimem_
   b.s_a = out ? out->s_a : (float*)(ws + w.s_a);
   b.psi_v = out ? out->psi_v : (float*)(ws + w.psi_v);
   b.psi_a = out ? out->psi_a : (float*)(ws + w.psi_a);
+  b.la_v = (float*)(ws + w.la_v);
+  b.la_a = (float*)(ws + w.la_a);
   b.cosn = (float*)(ws + w.cosn);
   b.partials = (double*)(ws + w.partials);
   b.stats = out ? out->stats : (double*)(ws + w.stats);
@@ -216,8 +221,8 @@ int compress_layers(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_ch
   w2.lse += lz * Hq * lse_stride * sizeof(float);
   w2.cosn += lz * Hkv * ((size_t)ctx->seg_cap_v + ctx->seg_cap_a) * sizeof(float);
   w2.partials += lz * 2 * (size_t)ctx->fin_blocks * 3 * sizeof(double);
-  w2.a_v += segv_b; w2.s_v += segv_b; w2.psi_v += segv_b;
-  w2.a_a += sega_b; w2.s_a += sega_b; w2.psi_a += sega_b;
+  w2.a_v += segv_b; w2.la_v += segv_b; w2.s_v += segv_b; w2.psi_v += segv_b;
+  w2.a_a += sega_b; w2.la_a += sega_b; w2.s_a += sega_b; w2.psi_a += sega_b;
   w2.stats += lz * 8 * sizeof(double);
   w2.M_v += lz * sizeof(int32_t); w2.M_a += lz * sizeof(int32_t);
   w2.idx_v += idx_b; w2.idx_a += idx_b;

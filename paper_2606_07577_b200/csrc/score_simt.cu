@@ -193,6 +193,85 @@ __global__ void __launch_bounds__(128) attend_simt_kernel(StepParams p, const T*
   for (int d = t; d < D; d += 128) store_out(Y + row * D + d, acc);
 }
 
+// ---- Eq.6 below fp32's range (R31) ---------------------------------------------------------------------
+// Both column-sum kernels add fp32 weights: a weight below 2^-126 is flushed, so a key that NO query attends to comes
+// out as 0 (or as a sum that lost most of its terms) although Eq.8 raises it to lambda = 0.02, which maps 1e-80 to 0.025:
+// the ranking among unattended keys lives in that range.  Keys whose fp32 sum is below 2^-100 (at most G Nq lost
+// terms of < 2^-126 each cannot move a larger sum by 1e-3) are therefore recomputed here in the log domain,
+//     la = log2 sum_{g,i visible} 2^(c2 <q_i, k> - lse2_i)      (per-lane running maximum, merged across the warp),
+// and finalize takes psi = 2^(lambda la) (1 - s) for them.  Weights below 2^-1074 are dropped: fp64, the oracle's type,
+// ends there, and psi jumps from 3e-7 to 0 at that point in the oracle as well.  One warp looks at 32 consecutive key
+// slots and works through the flagged ones; with ordinary logits nothing is flagged and the kernel is one load per key.
+constexpr float kTinyImportance = 7.888609052210118e-31f;   // 2^-100
+
+template <typename T>
+__global__ void __launch_bounds__(128) colsum_rescue_kernel(StepParams p, const T* __restrict__ cacheK,
+                                                            const T* __restrict__ chunkK, const T* __restrict__ Q,
+                                                            const float* __restrict__ lse_arr, int lse_stride, float lse_coef,
+                                                            float* __restrict__ a_v, float* __restrict__ a_a,
+                                                            float* __restrict__ la_v, float* __restrict__ la_a) {
+  extern __shared__ float sk[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int slots = p.cache_cap + p.Nn;               // logical key slots per (l,h): cache rows by capacity, then chunk rows
+  const int groups = (slots + 31) / 32;
+  const long long item = (long long)blockIdx.x * 4 + warp;
+  if (item >= (long long)p.L * p.Hkv * groups) return;
+  const int grp = (int)(item % groups);
+  const int h = (int)((item / groups) % p.Hkv);
+  const int l = (int)(item / ((long long)groups * p.Hkv));
+  if (layer_skips_scoring(p, l)) return;
+  const int D = p.D, n_v = p.n_v[l], n = p.n[l];
+  const long long lh = (long long)l * p.Hkv + h;
+  auto locate = [&](int kk, int& m, int& t, int& t_chunk) -> bool {   // slot -> (modality, segment index); false = no key there
+    t_chunk = -1;
+    if (kk >= slots) return false;
+    if (kk < p.cache_cap) {
+      if (kk >= n) return false;
+      cache_row_to_seg(n_v, kk, m, t);
+    } else {
+      t_chunk = kk - p.cache_cap;
+      chunk_row_to_seg(p, n_v, n, t_chunk, m, t);
+    }
+    return true;
+  };
+  int m, t, t_chunk;
+  const bool valid = locate(grp * 32 + lane, m, t, t_chunk);
+  float av = 1.f;
+  if (valid) av = (m == 0 ? a_v + lh * p.seg_cap_v : a_a + lh * p.seg_cap_a)[t];
+  unsigned todo = __ballot_sync(0xffffffffu, valid && !(av >= kTinyImportance));
+  float* myk = sk + warp * D;
+  const int rows = p.G * p.Nn;
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1;
+    locate(grp * 32 + src, m, t, t_chunk);
+    const T* kr = t_chunk < 0 ? cacheK + (lh * p.cache_cap + (grp * 32 + src)) * D : chunkK + (lh * p.Nn + t_chunk) * D;
+    __syncwarp();
+    for (int d = lane; d < D; d += 32) myk[d] = to_float(kr[d]);
+    __syncwarp();
+    float mx = -INFINITY, z = 0.f;
+    for (int rr = lane; rr < rows; rr += 32) {
+      const int g = rr / p.Nn, i = rr % p.Nn;
+      if (p.causal && t_chunk > i) continue;
+      const long long qh = (long long)l * p.Hq + h * p.G + g;
+      const float x = fmaf(p.scale_log2e, dot_row<T>(myk, Q + (qh * p.Nn + i) * D, D), lse_coef * lse_arr[qh * lse_stride + i]);
+      if (x < -1074.f) continue;   // below the smallest fp64 number: such a weight is 0 in the oracle's arithmetic too
+      if (x > mx) { z = z * exp2f(mx - x) + 1.f; mx = x; } else z += exp2f(x - mx);
+    }
+    float M = mx;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    z = mx == -INFINITY ? 0.f : z * exp2f(mx - M);
+#pragma unroll
+    for (int o = 16; o; o >>= 1) z += __shfl_xor_sync(0xffffffffu, z, o);
+    if (lane == 0) {
+      const float la = z > 0.f ? M + log2f(z) : -INFINITY;
+      (m == 0 ? la_v + lh * p.seg_cap_v : la_a + lh * p.seg_cap_a)[t] = la;
+      (m == 0 ? a_v + lh * p.seg_cap_v : a_a + lh * p.seg_cap_a)[t] = exp2f(la);   // what fp32 can hold of it (usually 0)
+    }
+  }
+}
+
 template <typename T>
 static cudaError_t lse_simt_t(const StepParams& p, const StepBuffers& b, cudaStream_t st) {
   const long long rows = (long long)p.L * p.Hq * p.Nn;
@@ -251,6 +330,32 @@ cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, cons
     colsum_simt_kernel<__nv_bfloat16><<<grid, 128, smem, st>>>(p, (const __nv_bfloat16*)b.cacheK,
                                                                (const __nv_bfloat16*)b.chunkK,
                                                                (const __nv_bfloat16*)b.Q, b.lse, b.a_v, b.a_a);
+  return cudaGetLastError();
+}
+
+}  // namespace omnimem
+
+namespace omnimem {
+
+// tcgen05 path: lse_arr = the internal NEGATED log2-domain LSE (row stride padded to 128); SIMT path: the natural-log LSE.
+cudaError_t launch_colsum_rescue(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
+                                 int* launches) {
+  if (p.Nn == 0) return cudaSuccess;     // no queries: a = 0 everywhere by definition, psi = 0^lambda (1 - s)
+  const int groups = (p.cache_cap + p.Nn + 31) / 32;
+  const long long items = (long long)p.L * p.Hkv * groups;
+  const unsigned grid = (unsigned)((items + 3) / 4);
+  const size_t smem = 4 * p.D * sizeof(float);
+  const float* lse_arr = ctx->use_tc ? b.lse2 : b.lse;
+  const int stride = ctx->use_tc ? (p.Nn + 127) / 128 * 128 : p.Nn;
+  const float coef = ctx->use_tc ? 1.f : -1.4426950408889634f;
+  ++*launches;
+  if (ctx->cfg.dtype == OMNIMEM_FP32)
+    colsum_rescue_kernel<float><<<grid, 128, smem, st>>>(p, (const float*)b.cacheK, (const float*)b.chunkK, (const float*)b.Q,
+                                                         lse_arr, stride, coef, b.a_v, b.a_a, b.la_v, b.la_a);
+  else
+    colsum_rescue_kernel<__nv_bfloat16><<<grid, 128, smem, st>>>(p, (const __nv_bfloat16*)b.cacheK, (const __nv_bfloat16*)b.chunkK,
+                                                                 (const __nv_bfloat16*)b.Q, lse_arr, stride, coef, b.a_v, b.a_a,
+                                                                 b.la_v, b.la_a);
   return cudaGetLastError();
 }
 

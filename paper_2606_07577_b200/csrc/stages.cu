@@ -177,8 +177,16 @@ cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const Ste
 // Finalize: s_t (Eq.7 mean over existing neighbours, clamp, R10/R12), psi = a^lambda (1-s) (Eq.8), and per-block
 // partial sums of A_t = sum_h a, A_t ln A_t and s for the AVBA statistics (Eq.9-10, 13; H = ln S - sum A ln A / S).
 // ------------------------------------------------------------------------------------------------------------
+// a^lambda with the log-domain value for the keys below fp32's range (R31; colsum_rescue_kernel wrote la for exactly the
+// keys with a < 2^-100); C pow semantics at the ends: x^0 = 1, 0^lambda = 0 (R13)
+__device__ __forceinline__ float pow_importance(float a, float la, float lambda) {
+  if (a >= 7.888609052210118e-31f) return powf(a, lambda);
+  return lambda == 0.f ? 1.f : exp2f(lambda * la);
+}
+
 __global__ void __launch_bounds__(256) finalize_kernel(StepParams p, const float* __restrict__ a_v,
-                                                       const float* __restrict__ a_a, const float* __restrict__ cosn,
+                                                       const float* __restrict__ a_a, const float* __restrict__ la_v,
+                                                       const float* __restrict__ la_a, const float* __restrict__ cosn,
                                                        float* __restrict__ s_v, float* __restrict__ s_a,
                                                        float* __restrict__ psi_v, float* __restrict__ psi_a,
                                                        double* __restrict__ partials, int nblk) {
@@ -191,7 +199,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams p, const float
   const bool skip = layer_skips_scoring(p, l);
   double v0 = 0.0, v1 = 0.0, v2 = 0.0;
   if (t < Km && !skip) {
-    float A = 0.f, ssum = 0.f;
+    float A = 0.f, ssum = 0.f, la_max = -INFINITY;
     for (int h = 0; h < p.Hkv; ++h) {
       const long long lh = (long long)l * p.Hkv + h;
       const float* cs = cosn + lh * items + (m == 0 ? 0 : p.seg_cap_v);
@@ -202,13 +210,21 @@ __global__ void __launch_bounds__(256) finalize_kernel(StepParams p, const float
       float s = cnt == 2 ? 0.5f * sum : sum;  // cnt == 0 -> 0 (R10)
       s = fminf(1.f, fmaxf(-1.f, s));
       const float a = (m == 0 ? a_v : a_a)[lh * cap + t];
+      const float la = a >= 7.888609052210118e-31f ? 0.f : (p.Nn > 0 ? (m == 0 ? la_v : la_a)[lh * cap + t] : -INFINITY);
       (m == 0 ? s_v : s_a)[lh * cap + t] = s;
-      if (!p.shared_heads) (m == 0 ? psi_v : psi_a)[lh * cap + t] = powf(a, p.lambda) * (1.f - s);
+      if (!p.shared_heads) (m == 0 ? psi_v : psi_a)[lh * cap + t] = pow_importance(a, la, p.lambda) * (1.f - s);
+      else if (a < 7.888609052210118e-31f) la_max = fmaxf(la_max, la);
       A += a;
       ssum += s;
     }
     if (p.shared_heads) {  // R29: one score per token and layer, written to every head's row (identical index sets)
-      const float psi = powf(A, p.lambda) * (1.f - ssum / (float)p.Hkv);
+      float LA = la_max;   // log2 of the sum over heads, needed only when even the sum is below fp32's range
+      if (A < 7.888609052210118e-31f && la_max > -INFINITY) {
+        float zs = 0.f;
+        for (int h = 0; h < p.Hkv; ++h) zs += exp2f((m == 0 ? la_v : la_a)[((long long)l * p.Hkv + h) * cap + t] - la_max);
+        LA = la_max + log2f(zs);
+      }
+      const float psi = pow_importance(A, LA, p.lambda) * (1.f - ssum / (float)p.Hkv);
       for (int h = 0; h < p.Hkv; ++h) (m == 0 ? psi_v : psi_a)[((long long)l * p.Hkv + h) * cap + t] = psi;
     }
     v0 = (double)A;
@@ -276,7 +292,7 @@ cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const S
                             int* launches) {
   const int nblk = ctx->fin_blocks;
   dim3 grid(nblk, 2, p.L);
-  finalize_kernel<<<grid, 256, 0, st>>>(p, b.a_v, b.a_a, b.cosn, b.s_v, b.s_a, b.psi_v, b.psi_a, b.partials, nblk);
+  finalize_kernel<<<grid, 256, 0, st>>>(p, b.a_v, b.a_a, b.la_v, b.la_a, b.cosn, b.s_v, b.s_a, b.psi_v, b.psi_a, b.partials, nblk);
   stats_kernel<<<p.L, 32, 0, st>>>(p, b.partials, nblk, b.stats);
   *launches += 2;
   return cudaGetLastError();

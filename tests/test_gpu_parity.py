@@ -372,19 +372,51 @@ def test_select_at_the_papers_largest_budgets(cap):
 def test_wide_logit_range(mult):
     """Logits far wider than the Gaussian test inputs give: the softmax scale is multiplied by 12 / 40 and three keys get
     64 x the norm -- one in the FIRST cache tile, one in the LAST cache tile and one in the chunk -- so that in pass 1 the
-    running reference is re-based in the middle of a row with Z != 0 (the lazy-maximum vote fails mid-row), many
-    probabilities underflow (the polynomial's exponent clamp, ex2.approx.ftz) and rows are dominated by one key.
-    Rules (a)-(c) unchanged."""
-    for wl in (SMALL2, SMALL3):
+    running reference is re-based in the middle of a row with Z != 0 (the lazy-maximum vote fails mid-row), most
+    probabilities underflow (the polynomial's exponent clamp, ex2.approx.ftz, flush-to-zero sums), 7 of 8 rows are taken
+    by one key, and at x 40 more than half of the keys have an importance below 1e-30 (down to 1e-107 in the mixture
+    input): those are recomputed in the log domain (R31).  Rules (a)-(c) unchanged, causal and not."""
+    for wl in (SMALL2, SMALL3, SMALL4):
         x = I.full_inputs(wl)
         nc = wl.n_v + wl.n_a
-        for l in range(wl.L):
-            for h in range(wl.Hkv):
-                x["cacheK"][l, h, 5] *= 64.0
-                x["cacheK"][l, h, nc - 3] *= 64.0
-                x["chunkK"][l, h, wl.Nn // 2] *= 64.0
+        x["cacheK"][:, :, 5] *= 64.0
+        x["cacheK"][:, :, nc - 3] *= 64.0
+        x["chunkK"][:, :, wl.Nn // 2] *= 64.0
         c = mult / float(np.sqrt(wl.D))
         check_step(wl, x=x, eng_kw=dict(softmax_scale=c), ref_kw=dict(scale=c))
+        check_step(wl, x=x, eng_kw=dict(softmax_scale=c, causal=0), ref_kw=dict(scale=c, causal=0))
+    # (fp32 inputs are left out: logits of +-100 computed in fp32 carry an absolute error of ~1e-5, i.e. the whole 1e-5
+    # tolerance of rule (a), before anything else is counted)
+    check_step(SMALL2, eng_kw=dict(softmax_scale=c, score_path=1), ref_kw=dict(scale=c))        # bf16 SIMT path
+    check_step(SMALL3.replace(Hq=8, Hkv=4), eng_kw=dict(softmax_scale=c), ref_kw=dict(scale=c), select_scope=1)   # log-sum over heads
+
+
+def test_importance_below_fp32_range_is_recovered():
+    """DESIGN.md R31: two cached keys point AGAINST every query (logit between -318 and -106 for all of them): every one of
+    their softmax weights is below 2^-126, the fp32 column sum is exactly 0, and the true importance is about 1e-55.
+    Eq.8 maps that to psi ~ 0.08 (1 - s), so it must not be lost: the key is recomputed in the log domain, psi matches the
+    oracle at rule (a), and the published fp32 `a` holds what fp32 can (0)."""
+    wl = SMALL3
+    x = I.full_inputs(wl)
+    e = torch.ones(wl.D) / float(np.sqrt(wl.D))                                  # a fixed unit direction
+    x["Q"] = (x["Q"].float() + 12.0 * e).to(x["Q"].dtype)                        # <q, e> = 12 + N(0, u^2) in [6, 18], u <= 2
+    dead = (-200.0 * e).to(x["cacheK"].dtype)                                    # c <q, dead> in [-318, -106] for every query
+    x["cacheK"][:, :, 7] = dead
+    x["cacheK"][:, :, 600] = dead
+    L = wl.L
+    p = ref_params(wl, L)
+    orc = ref.score(p, x["cacheK"], x["cacheV"], x["n_v"], x["n"], x["chunkK"], x["chunkV"], x["Q"])
+    assert orc["a_v"][:, :, 7].max() < 2.0 ** -140 and orc["a_v"][:, :, 7].min() > 0.0      # the oracle: tiny but positive
+    assert orc["psi_v"][:, :, 7].min() > 1e-3
+    eng = engine_for(wl)
+    src, chunk = dev_objs(x, wl)
+    sc = eng.score(src, chunk)
+    torch.cuda.synchronize()
+    for t in (7, 600):
+        assert bool((sc.a_v[:, :, t] == 0).all())
+    compare_scores(wl, x["n_v"].numpy(), x["n"].numpy(), scores_to_numpy(sc), orc, TOL[wl.dtype])
+    eng.close()
+    check_step(wl, x=x)
 
 
 # ---------------------------------------------------------------------------------------------- streaming (cfg5 shape logic at cfg1 size)
