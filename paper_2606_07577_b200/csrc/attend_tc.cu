@@ -17,6 +17,8 @@
 #include <cuda.h>
 #include <math.h>
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "tc_ptx.cuh"
 
@@ -33,6 +35,10 @@ constexpr int kOffKV = 2 * kTileB;                // [kSlots][32 KB]
 constexpr int kOffBar = kOffKV + kSlots * kTileB;
 constexpr size_t kSmem = 1024 + kOffBar + 256;
 constexpr uint32_t kColS = 0, kColO = 256;        // tensor-memory columns
+#ifndef OMNIMEM_ATT_POLY_NUM
+#define OMNIMEM_ATT_POLY_NUM 2
+#endif
+constexpr int kPolyNum = OMNIMEM_ATT_POLY_NUM, kPolyDen = 8;   // exponential pairs on the FMA-pipe polynomial, of every 8
 
 // D = f32, A = B = bf16, N = 128, M = 128; bit 16: B is MN-major (the V tile: rows = keys, head_dim contiguous)
 constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kT >> 3) << 17) | ((uint32_t)(kT >> 4) << 24);
@@ -218,29 +224,58 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
         mbar_wait(bar_s + 8 * s, j & 1);
         tc_fence_after();
         uint32_t pk[64];                         // the tile's P row, bf16 pairs
-        float tsum;
-        // exponentials of the tile against reference `mref`; fills pk, returns the fp32 row sum
-        auto exp_tile = [&](float mref) {
-          float z[4] = {0.f, 0.f, 0.f, 0.f};
+        float tsum, pmax;
+        // exponentials of the tile against reference `mref`; fills pk, returns the fp32 row sum.  The 128 columns come in
+        // four tcgen05.ld of 32: the next one is in flight while the current one is computed (wait::ld waits for all
+        // outstanding loads, hence: wait, issue the next, compute).  Scale and sums are packed fp32x2; kPolyNum of every
+        // kPolyDen pairs take the FMA-pipe polynomial (tc_ptx.cuh) instead of the MUFU.
+        auto exp_tile = [&](float mref, auto masked_tag) {
+          constexpr bool kMasked = decltype(masked_tag)::value;
+          uint64_t zA = 0ull, zB = 0ull;
+          const uint64_t c2c2 = pack2(c2, c2), nm = pack2(-mref, -mref);
+          pmax = -INFINITY;   // largest raw score of a polynomial lane: unlike the MUFU, the polynomial does not overflow to inf
+          uint32_t va[32], vb[32];
+          tc_ld32x(tS, va);
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
-            uint32_t v[32];
-            tc_ld32x(tS + c * 32, v);
             tc_wait_ld();
+            uint32_t (&cur)[32] = (c & 1) ? vb : va;
+            if (c < 3) tc_ld32x(tS + (c + 1) * 32, (c & 1) ? va : vb);
 #pragma unroll
-            for (int e = 0; e < 32; e += 2) {
-              float p0 = ex2(fmaf(__uint_as_float(v[e]), c2, -mref)), p1 = ex2(fmaf(__uint_as_float(v[e + 1]), c2, -mref));
-              if (limit < kT) { p0 = c * 32 + e < limit ? p0 : 0.f; p1 = c * 32 + e + 1 < limit ? p1 : 0.f; }
-              z[(e >> 1) & 3] += p0 + p1;
-              pk[c * 16 + (e >> 1)] = pack_bf16(p0, p1);
+            for (int e = 0; e < 32; e += 4) {
+              if (pair_is_poly_t<kPolyNum, kPolyDen>(c * 16 + e / 2)) pmax = fmaxf(pmax, fmaxf(__uint_as_float(cur[e]), __uint_as_float(cur[e + 1])));
+              if (pair_is_poly_t<kPolyNum, kPolyDen>(c * 16 + e / 2 + 1)) pmax = fmaxf(pmax, fmaxf(__uint_as_float(cur[e + 2]), __uint_as_float(cur[e + 3])));
+              uint64_t P01 = ex2_pair_t<kPolyNum, kPolyDen>(fma2(pack2u(cur[e], cur[e + 1]), c2c2, nm), c * 16 + e / 2);
+              uint64_t P23 = ex2_pair_t<kPolyNum, kPolyDen>(fma2(pack2u(cur[e + 2], cur[e + 3]), c2c2, nm), c * 16 + e / 2 + 1);
+              float p0, p1, p2, p3;
+              unpack2(P01, p0, p1);
+              unpack2(P23, p2, p3);
+              if (kMasked) {
+                const int col = c * 32 + e;
+                p0 = col < limit ? p0 : 0.f; p1 = col + 1 < limit ? p1 : 0.f;
+                p2 = col + 2 < limit ? p2 : 0.f; p3 = col + 3 < limit ? p3 : 0.f;
+                P01 = pack2(p0, p1);
+                P23 = pack2(p2, p3);
+              }
+              zA = add2z(zA, P01);
+              zB = add2z(zB, P23);
+              pk[c * 16 + e / 2] = pack_bf16(p0, p1);
+              pk[c * 16 + e / 2 + 1] = pack_bf16(p2, p3);
             }
           }
-          return (z[0] + z[1]) + (z[2] + z[3]);
+          float z0, z1, z2, z3;
+          unpack2(zA, z0, z1);
+          unpack2(zB, z2, z3);
+          return (z0 + z1) + (z2 + z3);
+        };
+        auto exp_tile_any = [&](float mref) {   // the unmasked body for whole tiles (warp-uniform choice)
+          return __all_sync(0xffffffffu, limit >= kT) ? exp_tile(mref, std::false_type{}) : exp_tile(mref, std::true_type{});
         };
         bool ok = false;
         if (j > 0) {                             // lazy reference: exact unless something overflows
-          tsum = exp_tile(m_ref);
-          ok = tsum < 1.2676506e30f && lsum < 1.2676506e30f;   // 2^100; false for inf and NaN
+          tsum = exp_tile_any(m_ref);
+          ok = tsum < 1.2676506e30f && lsum < 1.2676506e30f &&   // 2^100; false for inf and NaN
+               fmaf(pmax, c2, -m_ref) < 100.f;
         }
         if (!__all_sync(0xffffffffu, ok)) {      // first tile, or the row's maximum jumped: exact path (warp-uniform)
           float mx = -INFINITY;
@@ -271,7 +306,7 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
             }
           }
           m_ref = m_new;
-          tsum = exp_tile(m_ref);
+          tsum = exp_tile_any(m_ref);
         }
         lsum += tsum;
 #pragma unroll

@@ -12,7 +12,8 @@
 // (sub-tile x column half) drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns,
 // frees the TMEM buffer as soon as its registers hold the data, and merges with its partner thread once, at the end.
 // The epilogue is bound by the MUFU ex2 pipe and by instruction dispatch: 2 of every 8
-// exponential pairs run as a packed fp32x2 polynomial on the FMA pipe, and the tile loops carry as little else as possible.
+// exponential pairs run as a packed fp32x2 degree-3 polynomial on the FMA pipe, and the tile loops carry as little else as
+// possible.
 // Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-19 = epilogue.
 #include <cuda.h>
 #include <math.h>
@@ -39,82 +40,25 @@ constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 
 constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
-// OMNIMEM_CLUSTER == 2: the two CTAs of a cluster (one TPC) take neighbouring stationary blocks, stream ONE tile
-// sequence (the union of what both need) and run it as tcgen05.mma.cta_group::2: M = 256 (128 stationary rows of
-// each CTA, out of its own tensor memory), N = 128 with each CTA holding HALF of every streamed tile (64 rows, 16 KB)
-// in its shared memory.  That halves the L2 -> SM traffic, the shared-memory writes and the tensor-pipe reads of the
-// streamed operand.  Only the leader CTA (rank 0) issues MMAs; completion is multicast to both CTAs' barriers; the
-// peer's "my half has landed", "stationary rows staged" and "accumulator read" signals reach the leader's barriers
-// by remote mbarrier arrives.
-#ifndef OMNIMEM_CLUSTER
-#define OMNIMEM_CLUSTER 1
-#endif
-constexpr int kCluster = OMNIMEM_CLUSTER;   // 1 or 2
-constexpr int kRowsB = 128 / kCluster;       // rows of a streamed tile in this CTA's shared memory
-constexpr int kKBlockBytesB = kRowsB * 128;  // one 64-element K-block of them
+constexpr int kKBlockBytes = kTile * 128;   // one 64-element K-block of a streamed tile (16 KB)
 #ifndef OMNIMEM_LAZY_MAX
 #define OMNIMEM_LAZY_MAX 1
 #endif
 constexpr bool kLazyMax = OMNIMEM_LAZY_MAX != 0;   // pass 1: running reference instead of a per-tile maximum (see the loop)
 
-// 2^x on the FMA/ALU pipes (Cody-Waite split + degree-4 minimax polynomial on [-0.5, 0.5], max relative error
-// 2.7e-6, mean error 4e-8; coefficients fitted for this file), two lanes per instruction
-// (fp32x2).  The MUFU ex2 pipe (16/clk/SM) is the limiter of both scoring passes (ncu: xu pipe 89 %), so
-// kPolyNum of every kPolyDen exponential PAIRS of a row are evaluated here instead of on the MUFU.
-__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
-  uint64_t d;
-  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-#ifndef OMNIMEM_POLY_DEG
-#define OMNIMEM_POLY_DEG 3
-#endif
-__device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
-  float x0, x1;
-  unpack2(X, x0, x1);
-  // below -126.5 the result q * 2^-126 (q < 1) is a denormal; the sums that consume it are flush-to-zero adds (add2z),
-  // so everything below 2^-126 contributes exactly 0, as in the MUFU lanes (ex2.approx.ftz)
-  X = pack2(fmaxf(x0, -126.5f), fmaxf(x1, -126.5f));
-  const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
-  const uint64_t T = add2(X, MG);
-  const uint64_t F = sub2(X, sub2(T, MG));
-#if OMNIMEM_POLY_DEG == 4    // max relative error 2.7e-6
-  uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
-  Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
-  Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
-  Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
-#else                        // degree 3: max relative error 7.5e-5, equi-oscillating in f (it averages out over a sum)
-  uint64_t Q = fma2(pack2(0.0551716685295105f, 0.0551716685295105f), F, pack2(0.2426111251115799f, 0.2426111251115799f));
-  Q = fma2(Q, F, pack2(0.6932609677314758f, 0.6932609677314758f));
-  Q = fma2(Q, F, pack2(0.9999280571937561f, 0.9999280571937561f));
-#endif
-  float q0, q1, t0, t1;
-  unpack2(Q, q0, q1);
-  unpack2(T, t0, t1);
-  return pack2(__int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23)),   // q * 2^round(x)
-               __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23)));
-}
 #ifndef OMNIMEM_POLY_NUM
 #define OMNIMEM_POLY_NUM 2
 #endif
 #ifndef OMNIMEM_POLY_DEN
 #define OMNIMEM_POLY_DEN 8
 #endif
+// share of the exponential PAIRS of a row that run as the fp32x2 polynomial on the FMA pipe instead of on the MUFU
+// (tc_ptx.cuh; measured optimum of both scoring passes under the 1000 W cap: 2 of 8, degree 3)
 constexpr int kPolyNum = OMNIMEM_POLY_NUM, kPolyDen = OMNIMEM_POLY_DEN;
-// pair `pi` of a row goes to the polynomial iff the Bresenham line of slope kPolyNum / kPolyDen steps there
-__device__ __forceinline__ constexpr bool pair_is_poly(int pi) {
-  return ((pi + 1) * kPolyNum) / kPolyDen > (pi * kPolyNum) / kPolyDen;
-}
-// 2^x of a packed pair: MUFU for both lanes, or the FMA-pipe polynomial
-__device__ __forceinline__ uint64_t ex2_pair(uint64_t X, int pi) {
-  if (pair_is_poly(pi)) return ex2_poly2(X);
-  float x0, x1;
-  unpack2(X, x0, x1);
-  return pack2(ex2(x0), ex2(x1));
-}
+__device__ __forceinline__ constexpr bool pair_is_poly(int pi) { return pair_is_poly_t<kPolyNum, kPolyDen>(pi); }
+__device__ __forceinline__ uint64_t ex2_pair(uint64_t X, int pi) { return ex2_pair_t<kPolyNum, kPolyDen>(X, pi); }
 
 // Instruction descriptor: D = f32 (bit 4), A = B = bf16 (bits 7, 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.
-constexpr uint32_t kIdescPair = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(2 * kTile >> 4) << 24);  // M = 256
 constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kTile >> 3) << 17) | ((uint32_t)(kTile >> 4) << 24);
 
 struct TcArgs {
@@ -140,8 +84,9 @@ struct Work {
   int n_cache_tiles, ntiles_sub[2], h;
   // pass 2
   int it0[2], tiles_per_g, hq0;
-  int seq0;              // first query tile of the streamed sequence (== it0[0] unless a cluster peer starts earlier)
-  // pair level (== the CTA's own values without a cluster): which batches exist for sub-tile s
+  int seq0;              // first query tile of the streamed sequence (== it0[0])
+  // which accumulator batches exist for sub-tile s (copies of ntiles_sub / it0 / sub_valid made after the kernel's early
+  // exit: see the note there)
   int ntp[2], it0p[2];
   bool validp[2];
 };
@@ -207,36 +152,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const StepParams& p = a.p;
   Work w;
   const bool mine = make_work<kPass>(a, w, (int)blockIdx.x);
-  // Pair level (kCluster == 2): the two CTAs stream one sequence, the union of what they need, and every MMA covers
-  // sub-tile s of BOTH.  ntp[s] (pass 1) / it0p[s], validp[s] (pass 2) say which batches exist; a CTA whose own sub-tile
-  // does not take a batch still has to release the accumulator ("ghost" consumption in the epilogue).
-  int peer_stage_warps = 0;
-  if (kCluster == 2) {
-    Work wp;
-    const bool peer = make_work<kPass>(a, wp, (int)blockIdx.x ^ 1);
-    if (!mine && !peer) return;           // uniform across the cluster
-    for (int s = 0; s < 2; ++s) {
-      if (kPass == 1) {
-        w.ntp[s] = max(w.sub_valid[s] ? w.ntiles_sub[s] : 0, wp.sub_valid[s] ? wp.ntiles_sub[s] : 0);
-      } else {
-        w.it0p[s] = min(w.sub_valid[s] ? w.it0[s] : 1 << 30, wp.sub_valid[s] ? wp.it0[s] : 1 << 30);
-      }
-      w.validp[s] = w.sub_valid[s] || wp.sub_valid[s];
-      peer_stage_warps += wp.sub_valid[s] ? 8 : 0;
-    }
-    if (kPass == 1) {
-      w.ntiles = max(w.ntp[0], w.ntp[1]);
-    } else {
-      w.seq0 = min(w.it0p[0], w.it0p[1]);
-      w.tiles_per_g = (p.Nn + kTile - 1) / kTile - w.seq0;
-      w.ntiles = p.G * w.tiles_per_g;
-    }
-  } else {
-    if (!mine) return;                    // uniform across the CTA
-    // (set AFTER the early exit: written before it, ptxas stopped using the uniform datapath in the tile loops)
-    for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
-  }
-  const uint32_t cta_rank = kCluster == 2 ? cluster_ctarank() : 0u;
+  if (!mine) return;                    // uniform across the CTA
+  // (set AFTER the early exit: written before it, ptxas stopped using the uniform datapath in the tile loops)
+  for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
 
   // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
   // array is a link-time constant, so every barrier / stage address below folds into an immediate
@@ -249,33 +167,25 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages, bar_a = bar_empty + 8 * kStages;
   const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
   const uint32_t bar_lse = bar_sempty + 8 * kAccBufs;                           // [kLseSlots]
-  const uint32_t bar_pfull = bar_lse + 8 * kLseSlots;                           // [kStages] leader only: the peer's half of a stage has landed
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots + 8 * kStages);
-  const bool leader = cta_rank == 0;
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots);
   const int my_stage_warps = (w.sub_valid[0] ? 8 : 0) + (w.sub_valid[1] ? 8 : 0);
 
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); mbar_init(bar_pfull + 8 * s, 1); }
-    // one arrival per epilogue warp that stages stationary rows (the leader also collects the peer's, remotely)
-    mbar_init(bar_a, max(1, my_stage_warps + (kCluster == 2 ? peer_stage_warps : 0)));
-    // an accumulator buffer is free when the 8 warps of its sub-tile's group have read it -- in BOTH CTAs for a pair
-    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8 * kCluster); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+    // one arrival per epilogue warp that stages stationary rows
+    mbar_init(bar_a, max(1, my_stage_warps));
+    // an accumulator buffer is free when the 8 warps of its sub-tile's group have read it
+    for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
-    if (kCluster == 2) {
-      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-    } else {
-      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
-  if (kCluster == 2) cluster_sync_all();   // the peer's barriers exist before anything is multicast into them
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
@@ -298,7 +208,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         if (++it == w.seq0 + w.tiles_per_g) { it = w.seq0; ++g; }
       }
       if (elect_one()) {
-        mbar_expect_tx(bar_full + 8 * stage, kTileBytes / kCluster);
+        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
         if (kPass == 2) {
           // lse2 of these 128 queries: its own ring + barrier.  Slot j % 16 was last read for tile j - 16; this load is
           // issued only after the MMAs of tile j - kStages completed, which needed the accumulator of a batch at most 3
@@ -307,43 +217,25 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
           bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
         }
-        // pair: this CTA's 64 rows of the tile (the peer loads the other 64 into ITS shared memory)
         for (int kb = 0; kb < 2; ++kb)
-          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytesB, mB, kb * kKBlock, row0 + (int)cta_rank * kRowsB, lh,
-                      bar_full + 8 * stage);
+          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
       }
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
       if (++slot == kLseSlots) slot = 0;
     }
-    if (kCluster == 2) {
-      // drain: the leader's last commits have reached this CTA's barriers before anybody leaves
-      for (int j = max(0, w.ntiles - kStages); j < w.ntiles; ++j) mbar_wait(bar_empty + 8 * (j % kStages), (j / kStages) & 1);
-    }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (kCluster == 2 && !leader) {
-      // peer of a pair: no MMAs of its own; it tells the leader when its half of a stage has landed
-      int stage = 0, sph = 0;
-      for (int j = 0; j < w.ntiles; ++j) {
-        mbar_wait(bar_full + 8 * stage, sph);
-        if (elect_one()) mbar_arrive_remote(bar_pfull + 8 * stage, 0);
-        __syncwarp();
-        if (++stage == kStages) { stage = 0; sph ^= 1; }
-      }
-    } else {
-    if (kCluster == 2) { if (my_stage_warps + peer_stage_warps > 0) mbar_wait_cluster(bar_a, 0); }
-    else if (mine) mbar_wait(bar_a, 0);  // stationary rows are in TMEM
+    mbar_wait(bar_a, 0);  // stationary rows are in TMEM
     tc_fence_after();
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
     int it = kPass == 2 ? w.seq0 : 0, stage = 0, sph = 0;
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_full + 8 * stage, sph);
-      if (kCluster == 2) mbar_wait_cluster(bar_pfull + 8 * stage, sph);
       tc_fence_after();
       for (int s = 0; s < 2; ++s) {
         if (!(kPass == 1 ? j < w.ntp[s] : (w.validp[s] && it >= w.it0p[s]))) continue;
-        if (kCluster == 2) mbar_wait_cluster(bar_sempty + 8 * buf, ph ^ 1); else mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
+        mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
         const uint32_t a_tmem = tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2));
@@ -352,20 +244,18 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
             // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
-            const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytesB + (kk & 3) * 32) >> 4);
-            if (kCluster == 2) tc_mma_bf16_ts_pair(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdescPair, kk > 0 ? 1u : 0u);
-            else tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, kk > 0 ? 1u : 0u);
+            const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
+            tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, kk > 0 ? 1u : 0u);
           }
-          if (kCluster == 2) tc_commit_pair(bar_sfull + 8 * buf); else tc_commit(bar_sfull + 8 * buf);
+          tc_commit(bar_sfull + 8 * buf);
         }
         __syncwarp();
         if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
       }
-      if (elect_one()) { if (kCluster == 2) tc_commit_pair(bar_empty + 8 * stage); else tc_commit(bar_empty + 8 * stage); }
+      if (elect_one()) tc_commit(bar_empty + 8 * stage);
       __syncwarp();
       if (++stage == kStages) { stage = 0; sph ^= 1; }
       if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
-    }
     }
   } else if (warp >= 4) {
     // ===================== epilogue groups =====================
@@ -376,32 +266,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     const int r = q4 * 32 + lane;        // row of the sub-tile == TMEM lane
     const int col0 = half * kHalf;
     const float c2 = p.scale_log2e;
-    // "this warp has read accumulator buffer b": the leader of a pair collects its peer's arrivals remotely
+    // "this warp has read accumulator buffer b"
     auto release = [&](int b) {
-      if (lane == 0) {
-        if (kCluster == 2 && !leader) mbar_arrive_remote(bar_sempty + 8 * b, 0);
-        else mbar_arrive(bar_sempty + 8 * b);
-      }
+      if (lane == 0) mbar_arrive(bar_sempty + 8 * b);
     };
-    if (!w.sub_valid[s]) {
-      // pair only: this CTA has no rows in sub-tile s but its peer does; every MMA still writes this CTA's accumulator
-      // buffer, which has to be handed back in ring order
-      if (kCluster == 2 && (s == 0 ? w.validp[0] : w.validp[1])) {
-        int buf = 0, ph = 0, it = kPass == 2 ? w.seq0 : 0;
-        for (int j = 0; j < w.ntiles; ++j) {
-          const bool tk0 = kPass == 1 ? j < w.ntp[0] : (w.validp[0] && it >= w.it0p[0]);
-          const bool tk1 = kPass == 1 ? j < w.ntp[1] : (w.validp[1] && it >= w.it0p[1]);
-          if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
-          if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
-          if (s == 0 ? tk0 : tk1) {
-            mbar_wait(bar_sfull + 8 * buf, ph);
-            release(buf);
-            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-          }
-          if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
-        }
-      }
-    } else {
+    if (w.sub_valid[s]) {
       const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
       {
         // Stage this thread's share of the stationary operand: row r of the sub-tile, bf16 elements [64 half, 64 half + 64)
@@ -427,7 +296,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) { if (kCluster == 2 && !leader) mbar_arrive_remote(bar_a, 0); else mbar_arrive(bar_a); }
+        if (lane == 0) mbar_arrive(bar_a);
       }
       const uint32_t t_col = t_lane + (uint32_t)col0;
       int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile
@@ -435,7 +304,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
         const int n = p.n[w.l];
         float m_run = -1e30f, Z = 0.f, W = 0.f;
-        const int nt_mine = s == 0 ? w.ntiles_sub[0] : w.ntiles_sub[1];
         // accumulator batch at ring position (b, bph) -> registers; the TMEM buffer is released as soon as they hold it
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
           mbar_wait(bar_sfull + 8 * b, bph);
@@ -569,13 +437,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const bool tk0 = s == 0 ? tk_mine : tk_other, tk1 = s == 0 ? tk_other : tk_mine;
           if (s == 1 && tk0) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j
           if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
-          if (kCluster == 2 && j >= nt_mine) {   // the peer's rows take this tile, mine do not: hand the buffer back unread
-            mbar_wait(bar_sfull + 8 * buf, ph);
-            release(buf);
-            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-            if (s == 0 && tk1) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
-            continue;
-          }
           // number of visible key columns of this tile for this row, relative to this thread's first column
           int limit;
           if (j < w.n_cache_tiles) limit = n - j * kTile;
@@ -614,7 +475,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
         uint64_t acc01 = 0ull, acc23 = 0ull;   // packed fp32x2 partial sums of the unmasked tiles
         const uint64_t c2c2 = pack2(c2, c2);
-        const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g, it_mine = w.it0[s];
+        const int it_first = w.seq0, it_end = w.seq0 + w.tiles_per_g;
         auto load_tile = [&](int b, int bph, uint32_t (&v0)[32], uint32_t (&v1)[32]) {
           mbar_wait(bar_sfull + 8 * b, bph);
           tc_fence_after();
@@ -667,13 +528,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           const bool other = s == 0 ? tk1 : tk0;
           if (s == 1 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 0's batch of tile j comes first
           if (!(s == 0 ? tk0 : tk1)) { if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } } continue; }
-          if (kCluster == 2 && it < it_mine) {   // the peer's keys see this query tile, mine do not yet: hand the buffer back unread
-            mbar_wait(bar_sfull + 8 * buf, ph);
-            release(buf);
-            if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
-            if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
-            continue;
-          }
           // causal (R3): chunk key krow is visible to query i iff i >= krow; first visible column (thread-relative):
           const int first = ((p.causal && w.a_chunk) ? krow - it * kTile : 0) - col0;
           uint32_t v0[32], v1[32];
@@ -718,11 +572,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   }
   tc_fence_before();
   __syncthreads();
-  if (kCluster == 2) cluster_sync_all();   // nobody leaves while the peer may still write into this CTA
   if (warp == 2) {
     tc_fence_after();
-    if (kCluster == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
-    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
   }
 }
 
@@ -758,7 +610,7 @@ static cudaError_t make_map(EncodeTiledFn enc, CUtensorMap* m, const void* base,
   if (rows == 0 || outer == 0 || base == nullptr) { memset(m, 0, sizeof(*m)); return cudaSuccess; }
   const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, outer};
   const cuuint64_t strides[2] = {(cuuint64_t)kHeadDim * 2, rows * kHeadDim * 2};
-  const cuuint32_t box[3] = {(cuuint32_t)kKBlock, (cuuint32_t)kRowsB, 1};   // a CTA of a pair loads half of the tile's rows
+  const cuuint32_t box[3] = {(cuuint32_t)kKBlock, (cuuint32_t)kTile, 1};
   const cuuint32_t es[3] = {1, 1, 1};
   const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -793,30 +645,13 @@ static TcArgs make_args(const StepParams& p, const StepBuffers& b) {
   return a;
 }
 
-// One launch of a scoring kernel: 211 KB of dynamic shared memory, and a (2,1,1) cluster when kCluster == 2 (grid.x is
-// rounded up to even; the extra CTA has no rows of its own and only serves its peer, or exits with it).
+// One launch of a scoring kernel: 211 KB of dynamic shared memory, one CTA per SM.
 typedef void (*ScoreKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const TcArgs);
 static cudaError_t launch_score(ScoreKernel k, dim3 grid, cudaStream_t st, const Maps& m, const TcArgs& a) {
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
-  if (kCluster == 1) {
-    k<<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
-    return cudaGetLastError();
-  }
-  grid.x = (grid.x + kCluster - 1) / kCluster * kCluster;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = grid;
-  cfg.blockDim = dim3(kThreads);
-  cfg.dynamicSmemBytes = kSmemBytes;
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = kCluster;
-  attr[0].val.clusterDim.y = 1;
-  attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, k, m.q, m.kc, m.kn, a);
+  k<<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {

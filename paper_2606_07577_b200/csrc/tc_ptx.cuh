@@ -31,41 +31,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::
           "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
-// arrive on the barrier at the same shared-memory offset in CTA `rank` of the cluster
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t bar, uint32_t rank) {
-  uint32_t remote;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
-  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
-}
-// wait that also acquires what other CTAs of the cluster released (remote arrives)
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAITC_LOOP:\n\t"
-      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra WAITC_DONE;\n\t"
-      "bra WAITC_LOOP;\n\t"
-      "WAITC_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
-}
-__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {   // both CTAs' barriers at this offset
-  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
-               "h"((uint16_t)3) : "memory");
-}
-__device__ __forceinline__ void tc_mma_bf16_ts_pair(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
-      "r"(acc) : "memory");
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
                "r"(bytes), "r"(bar) : "memory");
@@ -165,6 +130,59 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   d |= (uint64_t)2 << 61;
   return d;
 }
+// ---- 2^x on the FMA / ALU pipes ------------------------------------------------------------------------------------
+// Cody-Waite split + minimax polynomial on [-0.5, 0.5], two lanes per instruction (fp32x2).  The MUFU ex2 pipe
+// (16 / clk / SM) limits every softmax epilogue here (ncu: xu pipe 82-89 %), so a share of the exponential PAIRS of a row
+// is evaluated with this instead.  Degree 3: max relative error 7.5e-5, equi-oscillating in the fractional part (the error
+// of a sum of many terms averages out); degree 4: 2.7e-6.  Coefficients fitted for this repository (Lawson iteration on
+// the relative error).
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+#ifndef OMNIMEM_POLY_DEG
+#define OMNIMEM_POLY_DEG 3
+#endif
+__device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
+  float x0, x1;
+  unpack2(X, x0, x1);
+  // below -126.5 the result q * 2^-126 (q < 1) is a denormal; the sums that consume it are flush-to-zero adds (add2z),
+  // so everything below 2^-126 contributes exactly 0, as in the MUFU lanes (ex2.approx.ftz)
+  X = pack2(fmaxf(x0, -126.5f), fmaxf(x1, -126.5f));
+  const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
+  const uint64_t T = add2(X, MG);
+  const uint64_t F = sub2(X, sub2(T, MG));
+#if OMNIMEM_POLY_DEG == 4
+  uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
+  Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
+  Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
+  Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
+#else
+  uint64_t Q = fma2(pack2(0.0551716685295105f, 0.0551716685295105f), F, pack2(0.2426111251115799f, 0.2426111251115799f));
+  Q = fma2(Q, F, pack2(0.6932609677314758f, 0.6932609677314758f));
+  Q = fma2(Q, F, pack2(0.9999280571937561f, 0.9999280571937561f));
+#endif
+  float q0, q1, t0, t1;
+  unpack2(Q, q0, q1);
+  unpack2(T, t0, t1);
+  return pack2(__int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23)),   // q * 2^round(x)
+               __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23)));
+}
+// pair `pi` of a row goes to the polynomial iff the Bresenham line of slope kNum / kDen steps there
+template <int kNum, int kDen>
+__device__ __forceinline__ constexpr bool pair_is_poly_t(int pi) {
+  return ((pi + 1) * kNum) / kDen > (pi * kNum) / kDen;
+}
+// 2^x of a packed pair: MUFU for both lanes, or the FMA-pipe polynomial
+template <int kNum, int kDen>
+__device__ __forceinline__ uint64_t ex2_pair_t(uint64_t X, int pi) {
+  if (pair_is_poly_t<kNum, kDen>(pi)) return ex2_poly2(X);
+  float x0, x1;
+  unpack2(X, x0, x1);
+  return pack2(ex2(x0), ex2(x1));
+}
+
 // The same for an MN-major operand (rows of the shared-memory tile are K indices, 64 MN elements = 128 bytes contiguous
 // per row, 128-byte swizzle): 8-row groups along K are 1024 B apart (SBO), the next 64 MN elements `lbo_bytes` away (LBO).
 __device__ __forceinline__ uint64_t umma_desc_sw128_mn(uint32_t saddr, uint32_t lbo_bytes) {
