@@ -152,8 +152,11 @@ def oracle_one_kv_head(wl, x, l, h):
                          ids=["cfg2", "cfg4", "cfg3"])
 def test_attend_full_size(wl, samples):
     """BASELINE.json's full sizes in the launch configuration bench.py times (one omnimem_attend over all layers): sampled
-    (layer, KV head) units in full against the oracle; every row of every layer: finite, and the LSE equal (to fp32
-    rounding) to the one score pass 1 computes."""
+    (layer, KV head) units in full against the oracle; every row of every layer: finite, and the LSE equal to the one
+    score pass 1 computes up to the two kernels' exponential error: each puts a different quarter of a row's terms on the
+    degree-3 polynomial (relative error <= 7.5e-5, tc_ptx.cuh), so a row whose mass sits on one key (config 4's x4
+    outliers) can differ by 2 x 7.5e-5 in ln Z, plus fp32 rounding of an LSE of ~15 (1.488e-4 is what config 4 shows).
+    Rule (a) against the oracle (2e-3) is checked below on the sampled units."""
     from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
     x = I.full_inputs(wl)
     eng = OmniMem.for_workload(wl)
@@ -165,7 +168,7 @@ def test_attend_full_size(wl, samples):
     assert bool(torch.isfinite(lse).all()) and bool(torch.isfinite(y.float()).all())
     sc = eng.score(src, chunk, want_lse=True)
     torch.cuda.synchronize()
-    assert float((sc.lse - lse).abs().max()) < 1e-4
+    assert float((sc.lse - lse).abs().max()) < 2 * 7.5e-5 + 1e-5
     G = wl.G
     for l, h in samples:
         Y_ref, lse_ref, absY = oracle_one_kv_head(wl, x, l, h)
