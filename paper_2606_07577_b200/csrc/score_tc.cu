@@ -164,17 +164,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const uint32_t sLse = sB + kOffLse;                    // [kLseSlots][128] float (pass 2)
   float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 sub][128]
   const uint32_t bars = sB + kOffBars;
-  const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages, bar_a = bar_empty + 8 * kStages;
-  const uint32_t bar_sfull = bar_a + 8, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
+  const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages;
+  const uint32_t bar_sfull = bar_empty + 8 * kStages, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
   const uint32_t bar_lse = bar_sempty + 8 * kAccBufs;                           // [kLseSlots]
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 8 + 16 * kAccBufs + 8 * kLseSlots);
-  const int my_stage_warps = (w.sub_valid[0] ? 8 : 0) + (w.sub_valid[1] ? 8 : 0);
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 16 * kAccBufs + 8 * kLseSlots);
 
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
-    // one arrival per epilogue warp that stages stationary rows
-    mbar_init(bar_a, max(1, my_stage_warps));
     // an accumulator buffer is free when the 8 warps of its sub-tile's group have read it
     for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
@@ -192,6 +189,21 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   if (warp == 0) {
     // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
     int it = kPass == 2 ? w.seq0 : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
+    // the stationary sub-tiles go through the same ring: the MMA warp copies them on into tensor memory (tcgen05.cp).
+    // Rows past the end of the tensor are zero-filled by the TMA unit; rows n .. cache_cap of a cache tile are stale, which
+    // only reaches the (unpublished) results of those rows' own threads.
+    for (int s = 0; s < 2; ++s) {
+      if (!w.sub_valid[s]) continue;
+      mbar_wait(bar_empty + 8 * stage, sph);
+      if (elect_one()) {
+        const CUtensorMap* mA = kPass == 1 ? &mapQ : (w.a_chunk ? &mapKn : &mapKc);
+        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
+        for (int kb = 0; kb < 2; ++kb)
+          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mA, kb * kKBlock, w.rowA0 + s * kTile, w.lhA, bar_full + 8 * stage);
+      }
+      __syncwarp();
+      if (++stage == kStages) { stage = 0; sph ^= 1; }
+    }
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_empty + 8 * stage, sph);
       const CUtensorMap* mB;
@@ -226,10 +238,26 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    mbar_wait(bar_a, 0);  // stationary rows are in TMEM
-    tc_fence_after();
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
     int it = kPass == 2 ? w.seq0 : 0, stage = 0, sph = 0;
+    // stationary sub-tiles: shared memory -> tensor memory columns kTmemA + 64 s (lane = row, word c = elements 2c, 2c+1:
+    // the A-operand layout of a TS-mode tcgen05.mma), 8 columns per K16 step.  The copies run in issue order with the MMAs.
+    for (int s = 0; s < 2; ++s) {
+      if (!w.validp[s]) continue;
+      mbar_wait(bar_full + 8 * stage, sph);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t a_desc = umma_desc_sw128(sB + stage * kTileBytes);
+#pragma unroll
+        for (int kk = 0; kk < kHeadDim / 16; ++kk) {
+          const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
+          tc_cp_128x256b(tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2) + kk * 8), a_desc + koff);
+        }
+        tc_commit(bar_empty + 8 * stage);
+      }
+      __syncwarp();
+      if (++stage == kStages) { stage = 0; sph ^= 1; }
+    }
     for (int j = 0; j < w.ntiles; ++j) {
       mbar_wait(bar_full + 8 * stage, sph);
       tc_fence_after();
@@ -272,32 +300,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     };
     if (w.sub_valid[s]) {
       const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
-      {
-        // Stage this thread's share of the stationary operand: row r of the sub-tile, bf16 elements [64 half, 64 half + 64)
-        // = 32 words, straight from global memory into TMEM columns kTmemA + 64 s + 32 half (lane = row, word c = elements
-        // 2c, 2c+1: the A-operand layout of tcgen05.mma).  Rows past the end are zero.
-        const int row = w.rowA0 + s * kTile + r;
-        const __nv_bfloat16* base = kPass == 1 ? a.q : (w.a_chunk ? a.kn : a.kc);
-        const int rows_total = (kPass == 1 || w.a_chunk) ? p.Nn : p.cache_cap;
-        const int rows_valid = (kPass == 1 || w.a_chunk) ? p.Nn : p.n[w.l];
-        uint32_t av[32];
-        if (row < rows_valid) {
-          const uint4* src = reinterpret_cast<const uint4*>(base + ((long long)w.lhA * rows_total + row) * kHeadDim) + half * 8;
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const uint4 t4 = __ldg(src + u);
-            av[4 * u] = t4.x; av[4 * u + 1] = t4.y; av[4 * u + 2] = t4.z; av[4 * u + 3] = t4.w;
-          }
-        } else {
-#pragma unroll
-          for (int u = 0; u < 32; ++u) av[u] = 0u;
-        }
-        tc_st32(t_lane + (uint32_t)(kTmemA + s * (kHeadDim / 2) + half * 32), av);
-        tc_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_a);
-      }
       const uint32_t t_col = t_lane + (uint32_t)col0;
       int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile
       if (kPass == 1) {

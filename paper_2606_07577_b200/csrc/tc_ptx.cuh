@@ -85,6 +85,12 @@ __device__ __forceinline__ void tc_mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem,
       "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc),
       "r"(acc) : "memory");
 }
+// shared memory -> tensor memory, 128 lanes x 256 bits (8 columns): one K16 step of a K-major 128-row bf16 operand, read
+// through the same shared-memory descriptor a tcgen05.mma would take.  Asynchronous; executes in issue order with the
+// tcgen05.mma of the same thread, and tcgen05.commit covers it.
+__device__ __forceinline__ void tc_cp_128x256b(uint32_t taddr, uint64_t s_desc) {
+  asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(s_desc) : "memory");
+}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // packed fp32x2 arithmetic (sm_100): one issue slot for two lanes' worth of FMA / ADD
 __device__ __forceinline__ uint64_t pack2(float lo, float hi) {
