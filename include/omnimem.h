@@ -89,6 +89,9 @@ typedef struct {
                                               I carries no head index (R29): psi = (sum_h a)^lambda (1 - mean_h s)         */
   int32_t d_model;                         /* width of the retained hidden states (cache.h, chunk.h); 0 = none;
                                               d_model * element size must be a multiple of 16 bytes                  */
+  int32_t score_ctas;                      /* tcgen05 scoring kernels: number of persistent CTAs that share the work
+                                              items of a launch; 0 = one per SM (default).  A smaller number leaves SMs
+                                              to concurrent work; results do not depend on it                        */
 } omnimem_config;
 
 typedef struct {     /* one pooled KV cache */

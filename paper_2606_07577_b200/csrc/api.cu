@@ -283,7 +283,7 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
   if (g.n_layers <= 0 || g.n_q_heads <= 0 || g.n_kv_heads <= 0 || g.cache_cap <= 0 || g.max_chunk_v < 0 ||
       g.max_chunk_a < 0 || g.n_q_heads % g.n_kv_heads != 0 || g.sim_stride_v < 1 || g.sim_stride_a < 1 ||
       g.softmax_scale < 0.f || g.lambda < 0.f || g.ratio_r <= 0.f || g.temperature <= 0.f || g.budget_min < 0 ||
-      g.budget_max < g.budget_min || g.sim_source < 0 || g.sim_source > 2 || (g.select_scope != 0 && g.select_scope != 1) || g.d_model < 0 ||
+      g.budget_max < g.budget_min || g.sim_source < 0 || g.sim_source > 2 || (g.select_scope != 0 && g.select_scope != 1) || g.d_model < 0 || g.score_ctas < 0 ||
       (g.sim_source == 2 && (g.d_model == 0 || g.select_scope != 1 || (g.d_model * (g.dtype == OMNIMEM_FP32 ? 4 : 2)) % 16 != 0)) || g.n_kv_heads > 65535)
     return OMNIMEM_INVALID_ARG;
   if (g.dtype != OMNIMEM_FP32 && g.dtype != OMNIMEM_BF16) return OMNIMEM_UNSUPPORTED;
@@ -318,8 +318,11 @@ int omnimem_create(const omnimem_config* cfg, omnimem_ctx** out) {
   }
   for (int s = 0; s < OMNIMEM_N_STAGES; ++s) c->ev_used[s] = false;
   c->chunk_maps = nullptr;
+  c->sched = nullptr;
   c->copy_stream = nullptr;
   for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) c->ev_copy[i] = nullptr;
+  e = cudaMalloc((void**)&c->sched, 4 * sizeof(int32_t));
+  if (e != cudaSuccess) { omnimem_destroy(c); return OMNIMEM_CUDA_ERROR; }
   if (g.max_chunk_v + g.max_chunk_a > 0) {
     e = cudaMalloc((void**)&c->chunk_maps, 2 * sizeof(int32_t) * ((size_t)g.max_chunk_v + g.max_chunk_a));
     if (e != cudaSuccess) { omnimem_destroy(c); return OMNIMEM_CUDA_ERROR; }
@@ -339,6 +342,7 @@ int omnimem_destroy(omnimem_ctx* ctx) {
   for (int i = 0; i <= OMNIMEM_HOST_GROUPS; ++i) if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   if (ctx->chunk_maps) cudaFree(ctx->chunk_maps);
+  if (ctx->sched) cudaFree(ctx->sched);
   delete ctx;
   return OMNIMEM_OK;
 }

@@ -108,6 +108,7 @@ struct omnimem_ctx {
   bool ev_used[OMNIMEM_N_STAGES];
   int launches;
   void* encode_tiled;  // cuTensorMapEncodeTiled entry point
+  int32_t* sched;        // device [4]: work-item counters of the persistent scoring kernels (zeroed before each launch)
   int32_t* chunk_maps;   // device [2 * (max_chunk_v + max_chunk_a)]: row_of_seg, seg_of_row of an interleaved chunk
   cudaStream_t copy_stream;                        // omnimem_compress_chunk_host: host -> device copies of the next layer group
   cudaEvent_t ev_copy[OMNIMEM_HOST_GROUPS + 1];    // [g] group g is on the device; [last] `stream` reached the call

@@ -5,16 +5,21 @@
 //                        accumulator, keeps an online max / sum and writes lse2 = log2 sum_k 2^(c2 s_k).
 //   pass 2 (kPass == 2)  S^T = K Q^T, M = 128 keys per sub-tile: each thread owns one KEY row, the sum over
 //                        queries is thread-local: a_k = sum_{g,i} 2^(c2 s - lse2_i).  No atomics, no shuffles.
-// One CTA holds two stationary 128-row sub-tiles, staged once by the epilogue threads from global memory into tensor
-// memory (tcgen05.st: the A operand of a TS-mode tcgen05.mma, 64 TMEM columns each), and streams 128-row tiles of the
-// other operand (B, six 32 KB stages) by TMA; one elected thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile and
-// sub-tile) into a ring of three 128-column TMEM accumulators shared by both sub-tiles; four 4-warp epilogue groups
-// (sub-tile x column half) drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns,
-// frees the TMEM buffer as soon as its registers hold the data, and merges with its partner thread once, at the end.
-// The epilogue is bound by the MUFU ex2 pipe and by instruction dispatch: 2 of every 8
-// exponential pairs run as a packed fp32x2 degree-3 polynomial on the FMA pipe, and the tile loops carry as little else as
-// possible.
-// Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-19 = epilogue.
+// Both kernels are PERSISTENT: one CTA per SM (cfg.score_ctas overrides the count) draws work items (256 stationary rows
+// of one head and layer x their whole streamed sequence) from a device counter; the TMA stage ring, the accumulator ring,
+// the lse ring and all their barrier phases run on across items, and the producer warp prefetches the next item's tiles
+// while the epilogue finishes the current one.
+// An item = two stationary 128-row sub-tiles.  They arrive through the same TMA ring as the streamed tiles and are copied
+// into tensor memory by the MMA warp (tcgen05.cp 128x256b, 64 TMEM columns each: the A operand of a TS-mode tcgen05.mma,
+// in issue order between the previous item's last MMAs and this item's first).  The other operand streams as 128-row
+// tiles (B, six 32 KB stages); one elected thread issues tcgen05.mma (M=128,N=128,K=16 x 8 per tile and sub-tile) into a
+// ring of three 128-column TMEM accumulators shared by both sub-tiles; four 4-warp epilogue groups (sub-tile x column
+// half) drain them with tcgen05.ld 32x32b: a thread owns one row and 64 of the tile's 128 columns, frees the TMEM buffer
+// as soon as its registers hold the data, and merges with its partner thread once per item.
+// The epilogue is bound by the MUFU ex2 pipe, by instruction dispatch and -- over a whole step -- by the board's power
+// cap: 2 of every 8 exponential pairs run as a packed fp32x2 degree-3 polynomial on the FMA pipe,
+// and the tile loops carry as little else as possible.
+// Warp roles: 0 = TMA producer + item scheduler, 1 = MMA issuer, 2 = TMEM allocator, 4-19 = epilogue.
 #include <cuda.h>
 #include <math.h>
 
@@ -36,8 +41,9 @@ constexpr int kTmemA = kAccBufs * kTile;  // stationary operand: 64 columns per 
 constexpr int kLseSlots = 16;       // pass 2: ring of 128-float lse2 tiles (512 B each); see the reuse argument at the producer
 constexpr int kHalf = kTile / 2;    // columns of a tile owned by one epilogue thread
 constexpr int kOffLse = kStages * kTileBytes;
-constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 sub][128 rows] float4
-constexpr int kOffBars = kOffMerge + 2 * kTile * 16;
+constexpr int kOffMerge = kOffLse + kLseSlots * kTile * 4;       // [2 item parities][2 sub][128 rows] float4
+constexpr int kOffBars = kOffMerge + 2 * 2 * kTile * 16;
+constexpr int kQueue = 2;           // work items announced ahead by the producer warp
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
 constexpr int kKBlockBytes = kTile * 128;   // one 64-element K-block of a streamed tile (16 KB)
@@ -70,7 +76,9 @@ struct TcArgs {
   float* a_v;          // pass 2 outputs
   float* a_a;
   int n_cache_pairs;   // pass 2: ceil(cache_cap / 256)
-  const __nv_bfloat16 *q, *kc, *kn;  // raw operands (stationary rows are staged into TMEM by the epilogue threads)
+  // persistent CTAs: work item = (x, y, z) of the nx * ny * nz item grid, x fastest; handed out through *counter
+  int nx, ny, n_items;
+  int* counter;        // zeroed by the launcher
 };
 
 // What one CTA works on, computed identically by every role.
@@ -89,17 +97,23 @@ struct Work {
   // exit: see the note there)
   int ntp[2], it0p[2];
   bool validp[2];
+  int nbatch;            // accumulator batches of the item (both sub-tiles)
 };
 
 template <int kPass>
-__device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int bx) {   // bx: x index of the CTA described
+__device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int item) {   // item: index in the (x, y, z) item grid
   const StepParams& p = a.p;
-  w.l = blockIdx.z;
+  int bx = item % a.nx;
+  const int yz = item / a.nx, by = yz % a.ny;
+  w.l = yz / a.ny;
+  w.nbatch = 0;
   // values loaded from memory are made provably warp-uniform (shfl) so that the control warps stay on the uniform datapath
   const int n = uniform(p.n[w.l]);
   if (p.skip_budget != nullptr && n + p.Nn <= uniform(p.skip_budget[w.l])) return false;
+  bool mine;
   if (kPass == 1) {
-    const int j = blockIdx.y;  // query head
+    bx = a.nx - 1 - bx;        // the longest items (most visible chunk tiles) of a head first
+    const int j = by;          // query head
     w.h = j / p.G;
     w.lhA = w.l * p.Hq + j;
     w.rowA0 = bx * 2 * kTile;
@@ -113,10 +127,12 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int bx) {   
       const int nc = p.causal ? min(nct, r0 / kTile + 1) : nct;  // R3: chunk key t visible iff t <= i
       w.ntiles_sub[s] = w.sub_valid[s] ? w.n_cache_tiles + nc : 0;
       w.ntiles = max(w.ntiles, w.ntiles_sub[s]);
+      w.it0[s] = 0;
     }
-    return w.sub_valid[0];
+    w.nbatch = w.ntiles_sub[0] + w.ntiles_sub[1];
+    mine = w.sub_valid[0];
   } else {
-    const int h = blockIdx.y;  // KV head
+    const int h = by;  // KV head
     w.h = h;
     w.lhA = w.l * p.Hkv + h;
     w.hq0 = w.l * p.Hq + h * p.G;
@@ -135,13 +151,75 @@ __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int bx) {   
       const int r0 = w.rowA0 + s * kTile;
       w.sub_valid[s] = r0 < valid_rows;
       w.it0[s] = (p.causal && w.a_chunk) ? r0 / kTile : 0;  // first query tile that can see this key sub-tile
+      w.ntiles_sub[s] = 0;
     }
     w.seq0 = w.it0[0];
     w.tiles_per_g = nqt - w.seq0;
     w.ntiles = w.sub_valid[0] ? p.G * w.tiles_per_g : 0;
     if (w.ntiles <= 0) { w.ntiles = 0; w.sub_valid[0] = w.sub_valid[1] = false; }
-    return w.sub_valid[0];
+    for (int s = 0; s < 2; ++s)
+      if (w.sub_valid[s]) w.nbatch += p.G * (nqt - max(w.it0[s], w.seq0));
+    mine = w.sub_valid[0];
   }
+  for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
+  return mine;
+}
+
+// Steady state of pass 2 (cached keys, or no causal mask): both sub-tiles take every streamed tile and nothing is masked;
+// the accumulator ring advances by two batches per tile.  The ring position comes in through shuffles so that ptxas keeps
+// the loop's ring and barrier bookkeeping on the uniform datapath (254 instructions per tile and thread in the
+// one-item-per-CTA kernel of round 1, 292 when the persistent kernel carried the positions in vector registers).
+struct SteadyState { int buf, ph; uint64_t acc01, acc23; };
+__device__ __forceinline__ SteadyState colsum_steady(int ntiles, int s, int half, int jt, uint32_t t_col, float c2, int buf, int ph,
+                                                  uint64_t acc01, uint64_t acc23) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t sB = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sLse = sB + kOffLse, bars = sB + kOffBars;
+  const uint32_t bar_sfull = bars + 16 * kStages, bar_sempty = bar_sfull + 8 * kAccBufs, bar_lse = bar_sempty + 8 * kAccBufs;
+  const int lane = threadIdx.x & 31;
+  ntiles = uniform(ntiles); s = uniform(s); half = uniform(half); jt = uniform(jt); buf = uniform(buf); ph = uniform(ph);
+  const uint64_t c2c2 = pack2(c2, c2);
+  // position in the lse ring, kept as loop-carried addresses (one uniform register each for the tile's 512 bytes and for
+  // its barrier; computed from the tile index, ptxas split the address in two and copied one part into a vector register
+  // for each of the 16 loads)
+  const int slot0 = jt & (kLseSlots - 1);
+  uint32_t l_addr = sLse + (uint32_t)(slot0 * kTile + half * kHalf) * 4, l_bar = bar_lse + 8 * slot0;
+  const uint32_t l_bar_end = bar_lse + 8 * kLseSlots;
+  int l_par = (jt / kLseSlots) & 1;
+  for (int j = 0; j < ntiles; ++j) {
+    int own = buf + s, oph = ph;
+    if (own >= kAccBufs) { own -= kAccBufs; oph ^= 1; }
+    uint32_t v0[32], v1[32];
+    mbar_wait(bar_sfull + 8 * own, oph);
+    tc_fence_after();
+    const uint32_t t_addr = t_col + (uint32_t)(own * kTile);
+    tc_ld32(t_addr, v0);
+    tc_ld32(t_addr + 32, v1);
+    tc_wait_ld();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_sempty + 8 * own);
+    buf += 2;
+    if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
+    mbar_wait(l_bar, l_par);
+    const uint32_t l_cur = l_addr;
+    l_addr += kTile * 4;
+    l_bar += 8;
+    if (l_bar == l_bar_end) { l_bar = bar_lse; l_addr -= kLseSlots * kTile * 4; l_par ^= 1; }
+#pragma unroll
+    for (int e4 = 0; e4 < 8; ++e4) {
+      const float4 la = lds128(l_cur + e4 * 16), lb = lds128(l_cur + 128 + e4 * 16);
+      const uint64_t x0 = fma2(pack2u(v0[4 * e4], v0[4 * e4 + 1]), c2c2, pack2(la.x, la.y));
+      const uint64_t x1 = fma2(pack2u(v0[4 * e4 + 2], v0[4 * e4 + 3]), c2c2, pack2(la.z, la.w));
+      const uint64_t x2 = fma2(pack2u(v1[4 * e4], v1[4 * e4 + 1]), c2c2, pack2(lb.x, lb.y));
+      const uint64_t x3 = fma2(pack2u(v1[4 * e4 + 2], v1[4 * e4 + 3]), c2c2, pack2(lb.z, lb.w));
+      acc01 = add2z(acc01, ex2_pair(x0, 4 * e4));
+      acc23 = add2z(acc23, ex2_pair(x1, 4 * e4 + 1));
+      acc01 = add2z(acc01, ex2_pair(x2, 4 * e4 + 2));
+      acc23 = add2z(acc23, ex2_pair(x3, 4 * e4 + 3));
+    }
+  }
+  return SteadyState{buf, ph, acc01, acc23};
 }
 
 template <int kPass, bool kEntropy>
@@ -150,11 +228,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
                 const __grid_constant__ CUtensorMap mapKn, const TcArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const StepParams& p = a.p;
-  Work w;
-  const bool mine = make_work<kPass>(a, w, (int)blockIdx.x);
-  if (!mine) return;                    // uniform across the CTA
-  // (set AFTER the early exit: written before it, ptxas stopped using the uniform datapath in the tile loops)
-  for (int s = 0; s < 2; ++s) { w.ntp[s] = w.ntiles_sub[s]; w.it0p[s] = w.it0[s]; w.validp[s] = w.sub_valid[s]; }
 
   // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
   // array is a link-time constant, so every barrier / stage address below folds into an immediate
@@ -162,12 +235,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   const uint32_t sB = (s_raw + 1023u) & ~1023u;          // [kStages][2 kb][16 KB]
   uint8_t* smem = smem_raw + (sB - s_raw);
   const uint32_t sLse = sB + kOffLse;                    // [kLseSlots][128] float (pass 2)
-  float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 sub][128]
+  float4* sMerge = reinterpret_cast<float4*>(smem + kOffMerge);  // [2 item parities][2 sub][128]
   const uint32_t bars = sB + kOffBars;
   const uint32_t bar_full = bars, bar_empty = bar_full + 8 * kStages;
   const uint32_t bar_sfull = bar_empty + 8 * kStages, bar_sempty = bar_sfull + 8 * kAccBufs;  // [accumulator buffer]
   const uint32_t bar_lse = bar_sempty + 8 * kAccBufs;                           // [kLseSlots]
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 16 * kAccBufs + 8 * kLseSlots);
+  const uint32_t bar_qfull = bar_lse + 8 * kLseSlots, bar_qempty = bar_qfull + 8 * kQueue;   // [kQueue] item queue
+  const uint32_t sQueue = bar_qempty + 8 * kQueue;                              // [kQueue] int
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBars + 16 * kStages + 16 * kAccBufs + 8 * kLseSlots + 16 * kQueue + 4 * kQueue);
 
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -175,6 +250,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     // an accumulator buffer is free when the 8 warps of its sub-tile's group have read it
     for (int i = 0; i < kAccBufs; ++i) { mbar_init(bar_sfull + 8 * i, 1); mbar_init(bar_sempty + 8 * i, 8); }
     for (int i = 0; i < kLseSlots; ++i) mbar_init(bar_lse + 8 * i, 1);
+    // a queue slot is free again when the MMA warp and the 16 epilogue warps have read it
+    for (int i = 0; i < kQueue; ++i) { mbar_init(bar_qfull + 8 * i, 1); mbar_init(bar_qempty + 8 * i, 17); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
@@ -186,106 +263,149 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
 
+  // PERSISTENT CTA: one per SM, all rings (shared-memory stages, accumulators, lse tiles) and their phases run on across
+  // work items.  The producer warp draws item indices from a global counter and announces them through a two-slot queue;
+  // it runs ahead of the consumers by up to kStages tiles, so the next item's stationary and first streamed tiles are in
+  // shared memory before the epilogue has finished the current item.
+  int qi = 0, qph = 0;      // consumer side of the item queue
+  auto next_item = [&]() -> int {
+    mbar_wait(bar_qfull + 8 * qi, qph);
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(sQueue + 4 * qi) : "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_qempty + 8 * qi);
+    if (++qi == kQueue) { qi = 0; qph ^= 1; }
+    return uniform((int)v);
+  };
+
+  if (warp < 4) {
   if (warp == 0) {
-    // ===================== TMA producer (streamed operand only; the stationary one lives in TMEM) =====================
-    int it = kPass == 2 ? w.seq0 : 0, g = 0, stage = 0, sph = 1, slot = 0;   // pass 2: query tile / group member of tile j, kept incrementally
-    // the stationary sub-tiles go through the same ring: the MMA warp copies them on into tensor memory (tcgen05.cp).
-    // Rows past the end of the tensor are zero-filled by the TMA unit; rows n .. cache_cap of a cache tile are stale, which
-    // only reaches the (unpublished) results of those rows' own threads.
-    for (int s = 0; s < 2; ++s) {
-      if (!w.sub_valid[s]) continue;
-      mbar_wait(bar_empty + 8 * stage, sph);
-      if (elect_one()) {
-        const CUtensorMap* mA = kPass == 1 ? &mapQ : (w.a_chunk ? &mapKn : &mapKc);
-        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
-        for (int kb = 0; kb < 2; ++kb)
-          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mA, kb * kKBlock, w.rowA0 + s * kTile, w.lhA, bar_full + 8 * stage);
+    // ===================== TMA producer: stationary sub-tiles, then the streamed operand =====================
+    int stage = 0, sph = 1, slot = 0, pq = 0, pqph = 1;
+    for (;;) {
+      mbar_wait(bar_qempty + 8 * pq, pqph);
+      int item = 0;
+      if (lane == 0) {
+        item = atomicAdd(a.counter, 1);
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(sQueue + 4 * pq), "r"(item) : "memory");
+        mbar_arrive(bar_qfull + 8 * pq);
       }
-      __syncwarp();
-      if (++stage == kStages) { stage = 0; sph ^= 1; }
-    }
-    for (int j = 0; j < w.ntiles; ++j) {
-      mbar_wait(bar_empty + 8 * stage, sph);
-      const CUtensorMap* mB;
-      int row0, lh;
-      if (kPass == 1) {
-        const bool cache = j < w.n_cache_tiles;
-        mB = cache ? &mapKc : &mapKn;
-        row0 = (cache ? j : j - w.n_cache_tiles) * kTile;
-        lh = w.l * p.Hkv + w.h;
-      } else {
-        mB = &mapQ;
-        row0 = it * kTile;
-        lh = w.hq0 + g;
-        if (++it == w.seq0 + w.tiles_per_g) { it = w.seq0; ++g; }
-      }
-      if (elect_one()) {
-        mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
-        if (kPass == 2) {
-          // lse2 of these 128 queries: its own ring + barrier.  Slot j % 16 was last read for tile j - 16; this load is
-          // issued only after the MMAs of tile j - kStages completed, which needed the accumulator of a batch at most 3
-          // batches (<= 3 tiles) older to be released, and an epilogue thread releases a batch only after it finished
-          // computing all earlier ones: tile j - 16 is long done.
-          mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
-          bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
+      item = uniform(item);
+      if (++pq == kQueue) { pq = 0; pqph ^= 1; }
+      if (item >= a.n_items) break;
+      Work w;
+      if (!make_work<kPass>(a, w, item)) continue;
+      int it = kPass == 2 ? w.seq0 : 0, g = 0;   // pass 2: query tile / group member of tile j, kept incrementally
+      stage = uniform(stage); sph = uniform(sph); slot = uniform(slot);   // see the epilogue
+      // the stationary sub-tiles go through the same ring: the MMA warp copies them on into tensor memory (tcgen05.cp).
+      // Rows past the end of the tensor are zero-filled by the TMA unit; rows n .. cache_cap of a cache tile are stale,
+      // which only reaches the (unpublished) results of those rows' own threads.
+      for (int s = 0; s < 2; ++s) {
+        if (!w.sub_valid[s]) continue;
+        mbar_wait(bar_empty + 8 * stage, sph);
+        if (elect_one()) {
+          const CUtensorMap* mA = kPass == 1 ? &mapQ : (w.a_chunk ? &mapKn : &mapKc);
+          mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
+          for (int kb = 0; kb < 2; ++kb)
+            tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mA, kb * kKBlock, w.rowA0 + s * kTile, w.lhA, bar_full + 8 * stage);
         }
-        for (int kb = 0; kb < 2; ++kb)
-          tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; sph ^= 1; }
       }
-      __syncwarp();
-      if (++stage == kStages) { stage = 0; sph ^= 1; }
-      if (++slot == kLseSlots) slot = 0;
+      for (int j = 0; j < w.ntiles; ++j) {
+        mbar_wait(bar_empty + 8 * stage, sph);
+        const CUtensorMap* mB;
+        int row0, lh;
+        if (kPass == 1) {
+          const bool cache = j < w.n_cache_tiles;
+          mB = cache ? &mapKc : &mapKn;
+          row0 = (cache ? j : j - w.n_cache_tiles) * kTile;
+          lh = w.l * p.Hkv + w.h;
+        } else {
+          mB = &mapQ;
+          row0 = it * kTile;
+          lh = w.hq0 + g;
+          if (++it == w.seq0 + w.tiles_per_g) { it = w.seq0; ++g; }
+        }
+        if (elect_one()) {
+          mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
+          if (kPass == 2) {
+            // lse2 of these 128 queries: its own ring + barrier, slot = (streamed tiles so far) % 16.  The slot was last
+            // read 16 streamed tiles ago; this load is issued only after the ring entry kStages back (a streamed tile at
+            // most kStages + 2 tiles back, the stationary tiles of an item boundary included) was consumed by its MMAs,
+            // which needed accumulators that the epilogue releases only after it finished computing every earlier batch:
+            // everything more than kStages + 2 + 3 = 11 tiles back is done.
+            mbar_expect_tx(bar_lse + 8 * slot, kTile * 4);
+            bulk_load(sLse + slot * kTile * 4, a.lse2 + (long long)lh * a.lse_stride + row0, kTile * 4, bar_lse + 8 * slot);
+          }
+          for (int kb = 0; kb < 2; ++kb)
+            tma_load_3d(sB + stage * kTileBytes + kb * kKBlockBytes, mB, kb * kKBlock, row0, lh, bar_full + 8 * stage);
+        }
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; sph ^= 1; }
+        if (++slot == kLseSlots) slot = 0;
+      }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     int buf = 0, ph = 0;  // accumulator ring position of the next batch
-    int it = kPass == 2 ? w.seq0 : 0, stage = 0, sph = 0;
-    // stationary sub-tiles: shared memory -> tensor memory columns kTmemA + 64 s (lane = row, word c = elements 2c, 2c+1:
-    // the A-operand layout of a TS-mode tcgen05.mma), 8 columns per K16 step.  The copies run in issue order with the MMAs.
-    for (int s = 0; s < 2; ++s) {
-      if (!w.validp[s]) continue;
-      mbar_wait(bar_full + 8 * stage, sph);
-      tc_fence_after();
-      if (elect_one()) {
-        const uint64_t a_desc = umma_desc_sw128(sB + stage * kTileBytes);
-#pragma unroll
-        for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-          const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
-          tc_cp_128x256b(tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2) + kk * 8), a_desc + koff);
-        }
-        tc_commit(bar_empty + 8 * stage);
-      }
-      __syncwarp();
-      if (++stage == kStages) { stage = 0; sph ^= 1; }
-    }
-    for (int j = 0; j < w.ntiles; ++j) {
-      mbar_wait(bar_full + 8 * stage, sph);
-      tc_fence_after();
+    int stage = 0, sph = 0;
+    for (;;) {
+      const int item = next_item();
+      if (item >= a.n_items) break;
+      Work w;
+      if (!make_work<kPass>(a, w, item)) continue;
+      int it = kPass == 2 ? w.seq0 : 0;
+      buf = uniform(buf); ph = uniform(ph); stage = uniform(stage); sph = uniform(sph);   // see the epilogue
+      // stationary sub-tiles: shared memory -> tensor memory columns kTmemA + 64 s (lane = row, word c = elements 2c,
+      // 2c+1: the A-operand layout of a TS-mode tcgen05.mma), 8 columns per K16 step.  The copies run in issue order with
+      // the MMAs: after the previous item's last MMAs (which read these columns), before this item's first.
       for (int s = 0; s < 2; ++s) {
-        if (!(kPass == 1 ? j < w.ntp[s] : (w.validp[s] && it >= w.it0p[s]))) continue;
-        mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
+        if (!w.validp[s]) continue;
+        mbar_wait(bar_full + 8 * stage, sph);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
-        const uint32_t a_tmem = tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2));
-        const uint64_t b_desc = umma_desc_sw128(sB + stage * kTileBytes);
         if (elect_one()) {
+          const uint64_t a_desc = umma_desc_sw128(sB + stage * kTileBytes);
 #pragma unroll
           for (int kk = 0; kk < kHeadDim / 16; ++kk) {
-            // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
             const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
-            tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, kk > 0 ? 1u : 0u);
+            tc_cp_128x256b(tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2) + kk * 8), a_desc + koff);
           }
-          tc_commit(bar_sfull + 8 * buf);
+          tc_commit(bar_empty + 8 * stage);
         }
         __syncwarp();
-        if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+        if (++stage == kStages) { stage = 0; sph ^= 1; }
       }
-      if (elect_one()) tc_commit(bar_empty + 8 * stage);
-      __syncwarp();
-      if (++stage == kStages) { stage = 0; sph ^= 1; }
-      if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
+      for (int j = 0; j < w.ntiles; ++j) {
+        mbar_wait(bar_full + 8 * stage, sph);
+        tc_fence_after();
+        for (int s = 0; s < 2; ++s) {
+          if (!(kPass == 1 ? j < w.ntp[s] : (w.validp[s] && it >= w.it0p[s]))) continue;
+          mbar_wait(bar_sempty + 8 * buf, ph ^ 1);
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)(buf * kTile);
+          const uint32_t a_tmem = tmem_base + (uint32_t)(kTmemA + s * (kHeadDim / 2));
+          const uint64_t b_desc = umma_desc_sw128(sB + stage * kTileBytes);
+          if (elect_one()) {
+#pragma unroll
+            for (int kk = 0; kk < kHeadDim / 16; ++kk) {
+              // advancing the start-address field (bytes >> 4) walks K inside / across the two 64-element swizzle blocks
+              const uint64_t koff = (uint64_t)(((kk >> 2) * kKBlockBytes + (kk & 3) * 32) >> 4);
+              tc_mma_bf16_ts(d_tmem, a_tmem + kk * 8, b_desc + koff, kIdesc, kk > 0 ? 1u : 0u);
+            }
+            tc_commit(bar_sfull + 8 * buf);
+          }
+          __syncwarp();
+          if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
+        }
+        if (elect_one()) tc_commit(bar_empty + 8 * stage);
+        __syncwarp();
+        if (++stage == kStages) { stage = 0; sph ^= 1; }
+        if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
+      }
     }
-  } else if (warp >= 4) {
+  }
+  } else {
     // ===================== epilogue groups =====================
     const int grp = (warp - 4) >> 2;     // 0..3
     const int s = grp >> 1;              // sub-tile
@@ -298,10 +418,32 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     auto release = [&](int b) {
       if (lane == 0) mbar_arrive(bar_sempty + 8 * b);
     };
-    if (w.sub_valid[s]) {
-      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
-      const uint32_t t_col = t_lane + (uint32_t)col0;
-      int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile
+    const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+    const uint32_t t_col = t_lane + (uint32_t)col0;
+    int buf = 0, ph = 0;  // accumulator ring position, advanced for every batch of either sub-tile, across work items
+    int jt = 0;           // pass 2: streamed tiles of the earlier items, modulo the lse ring (slot and parity of tile j)
+    int mpar = 0;         // merge buffer of this item (double-buffered: the partner reads while the next item's halves write)
+    for (;;) {
+    const int item = next_item();
+    if (item >= a.n_items) break;
+    Work w;
+    if (!make_work<kPass>(a, w, item)) continue;
+    if (!w.sub_valid[s]) {
+      // This group has no rows in the item (ragged last block of a head): keep the ring positions in step, and do NOT run
+      // ahead: the mbarrier waits compare phase parities, which is only sound while a waiter is less than one ring
+      // revolution away from the phase it waits for.  The groups of sub-tile 0 arrive here when they are done with the item.
+      for (int b = w.nbatch % (2 * kAccBufs); b > 0; --b) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }
+      jt = (jt + w.ntiles) & (2 * kLseSlots - 1);
+      named_bar_sync(3, 512);
+      continue;
+    }
+    const bool idle_partner = !w.sub_valid[1];   // (sub-tile 0 is valid in every item that is worked on)
+    // loop-carried ring positions: re-derived from a shuffle at every item so that ptxas keeps them (and the barrier /
+    // tensor-memory addresses computed from them) on the uniform datapath inside the tile loops
+    buf = uniform(buf); ph = uniform(ph); jt = uniform(jt);
+    {
+      float4* sMg = sMerge + mpar * 2 * kTile;
+      mpar ^= 1;
       if (kPass == 1) {
         const int i = w.rowA0 + s * kTile + r;  // query index in the chunk
         const int n = p.n[w.l];
@@ -455,10 +597,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           row_update(v0, v1, limit);
         }
         // merge the two column halves of each row (online-softmax partials), then publish
-        if (half == 1) sMerge[s * kTile + r] = make_float4(m_run, Z, W, 0.f);
+        if (half == 1) sMg[s * kTile + r] = make_float4(m_run, Z, W, 0.f);
         named_bar_sync(1 + s, 256);
         if (half == 0) {
-          const float4 o = sMerge[s * kTile + r];
+          const float4 o = sMg[s * kTile + r];
           const float m = fmaxf(m_run, o.x);
           const float r0 = ex2(m_run - m), r1 = ex2(o.x - m);
           Z = Z * r0 + o.y * r1;
@@ -505,25 +647,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           }
         };
         if (w.sub_valid[0] && w.sub_valid[1] && !(p.causal && w.a_chunk)) {
-          // Steady state (cached keys, or no causal mask): both sub-tiles take every tile of the sequence and nothing is
-          // masked; the ring position advances by two batches per tile.
-          for (int j = 0; j < w.ntiles; ++j) {
-            int own = buf + s, oph = ph;
-            if (own >= kAccBufs) { own -= kAccBufs; oph ^= 1; }
-            uint32_t v0[32], v1[32];
-            load_tile(own, oph, v0, v1);
-            buf += 2;
-            if (buf >= kAccBufs) { buf -= kAccBufs; ph ^= 1; }
-            const int slot = j % kLseSlots;
-            mbar_wait(bar_lse + 8 * slot, (j / kLseSlots) & 1);
-            col_update(v0, v1, sLse + (uint32_t)(slot * kTile + col0) * 4);
-          }
+          const SteadyState st = colsum_steady(w.ntiles, s, half, jt, t_col, c2, buf, ph, acc01, acc23);
+          buf = st.buf; ph = st.ph; acc01 = st.acc01; acc23 = st.acc23;
         } else {
         int it_next = it_first;
         const int it0p_mine = uniform(s == 0 ? w.it0p[0] : w.it0p[1]), it0p_other = uniform(s == 0 ? w.it0p[1] : w.it0p[0]);
         const bool validp_mine = uniform(s == 0 ? w.validp[0] : w.validp[1]) != 0, validp_other = uniform(s == 0 ? w.validp[1] : w.validp[0]) != 0;
         for (int j = 0; j < w.ntiles; ++j) {
-          const int it = it_next, slot = j % kLseSlots, lse_parity = (j / kLseSlots) & 1;   // kLseSlots is a power of two
+          const int it = it_next, slot = (jt + j) & (kLseSlots - 1), lse_parity = ((jt + j) / kLseSlots) & 1;   // kLseSlots is a power of two
           if (++it_next == it_end) it_next = it_first;                                       // no division in the tile loop
           const bool tk_mine = validp_mine && it >= it0p_mine, tk_other = validp_other && it >= it0p_other;   // pair level
           const bool tk0 = s == 0 ? tk_mine : tk_other, tk1 = s == 0 ? tk_other : tk_mine;
@@ -537,7 +668,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           if (++buf == kAccBufs) { buf = 0; ph ^= 1; }
           if (s == 0 && other) { if (++buf == kAccBufs) { buf = 0; ph ^= 1; } }   // sub-tile 1's batch of tile j
           mbar_wait(bar_lse + 8 * slot, lse_parity);
-          const uint32_t l_addr = sLse + (uint32_t)(slot * kTile + col0) * 4;
+          // one uniform register for the whole address (taken before the per-thread branch below): left to itself ptxas
+          // keeps it as a sum of two uniform parts and materialises a vector copy of one of them for each of the 16 loads
+          const uint32_t l_addr = (uint32_t)uniform((int)(sLse + (uint32_t)(slot * kTile + col0) * 4));
           if (first <= 0) {
             col_update(v0, v1, l_addr);
           } else {
@@ -559,7 +692,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         unpack2(acc01, q0, q1);
         unpack2(acc23, q2, q3);
         const float part = ((acc[0] + acc[1]) + (acc[2] + acc[3])) + ((q0 + q1) + (q2 + q3));
-        if (half == 1) sMerge[s * kTile + r].x = part;
+        if (half == 1) sMg[s * kTile + r].x = part;
         named_bar_sync(1 + s, 256);
         const int n_v = p.n_v[w.l], n = p.n[w.l];
         const bool valid = w.a_chunk ? krow < p.Nn : krow < n;
@@ -567,10 +700,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           int m, t;
           if (w.a_chunk) chunk_row_to_seg(p, n_v, n, krow, m, t); else cache_row_to_seg(n_v, krow, m, t);
           float* out = m == 0 ? a.a_v + (long long)w.lhA * p.seg_cap_v : a.a_a + (long long)w.lhA * p.seg_cap_a;
-          out[t] = part + sMerge[s * kTile + r].x;
+          out[t] = part + sMg[s * kTile + r].x;
         }
+        jt = (jt + w.ntiles) & (2 * kLseSlots - 1);
       }
     }
+    if (idle_partner) named_bar_sync(3, 512);
+    }  // work items
   }
   tc_fence_before();
   __syncthreads();
@@ -641,17 +777,22 @@ static TcArgs make_args(const StepParams& p, const StepBuffers& b) {
   a.a_v = b.a_v;
   a.a_a = b.a_a;
   a.n_cache_pairs = (p.cache_cap + 2 * kTile - 1) / (2 * kTile);
-  a.q = (const __nv_bfloat16*)b.Q;
-  a.kc = (const __nv_bfloat16*)b.cacheK;
-  a.kn = (const __nv_bfloat16*)b.chunkK;
   return a;
 }
 
-// One launch of a scoring kernel: 211 KB of dynamic shared memory, one CTA per SM.
+// One launch of a scoring kernel: persistent CTAs (one per SM, 210 KB of dynamic shared memory each) that draw the
+// nx * ny * nz work items from a device counter, which is zeroed on the stream right before the launch.
 typedef void (*ScoreKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const TcArgs);
-static cudaError_t launch_score(ScoreKernel k, dim3 grid, cudaStream_t st, const Maps& m, const TcArgs& a) {
+static cudaError_t launch_score(const omnimem_ctx* ctx, ScoreKernel k, dim3 items, int which, cudaStream_t st, const Maps& m, TcArgs a) {
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
+  a.nx = (int)items.x;
+  a.ny = (int)items.y;
+  a.n_items = (int)(items.x * items.y * items.z);
+  a.counter = ctx->sched + which;
+  if ((e = cudaMemsetAsync(a.counter, 0, sizeof(int), st)) != cudaSuccess) return e;
+  const int ctas = ctx->cfg.score_ctas > 0 && ctx->cfg.score_ctas < ctx->sm_count ? ctx->cfg.score_ctas : ctx->sm_count;
+  const int grid = a.n_items < ctas ? a.n_items : ctas;
   k<<<grid, kThreads, kSmemBytes, st>>>(m.q, m.kc, m.kn, a);
   return cudaGetLastError();
 }
@@ -664,8 +805,8 @@ cudaError_t launch_lse_tc(const omnimem_ctx* ctx, const StepParams& p, const Ste
   const TcArgs a = make_args(p, b);
   dim3 grid((p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hq, p.L);
   ++*launches;
-  if (b.row_entropy) return launch_score(score_tc_kernel<1, true>, grid, st, m, a);
-  return launch_score(score_tc_kernel<1, false>, grid, st, m, a);
+  if (b.row_entropy) return launch_score(ctx, score_tc_kernel<1, true>, grid, 0, st, m, a);
+  return launch_score(ctx, score_tc_kernel<1, false>, grid, 0, st, m, a);
 }
 
 cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
@@ -685,7 +826,7 @@ cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const 
   }
   dim3 grid(a.n_cache_pairs + (p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hkv, p.L);
   ++*launches;
-  return launch_score(score_tc_kernel<2, false>, grid, st, m, a);
+  return launch_score(ctx, score_tc_kernel<2, false>, grid, 1, st, m, a);
 }
 
 }  // namespace omnimem

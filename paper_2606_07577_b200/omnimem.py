@@ -35,7 +35,7 @@ class omnimem_config(C.Structure):
                 ("softmax_scale", C.c_float), ("lam", C.c_float), ("ratio_r", C.c_float), ("temperature", C.c_float),
                 ("budget_min", C.c_int32), ("budget_max", C.c_int32), ("causal", C.c_int32), ("sim_source", C.c_int32),
                 ("sim_stride_v", C.c_int32), ("sim_stride_a", C.c_int32), ("score_path", C.c_int32),
-                ("select_scope", C.c_int32), ("d_model", C.c_int32)]
+                ("select_scope", C.c_int32), ("d_model", C.c_int32), ("score_ctas", C.c_int32)]
 
 
 class omnimem_cache(C.Structure):
@@ -162,7 +162,8 @@ class OmniMem:
     def __init__(self, L: int, Hq: int, Hkv: int, D: int, dtype: str, cache_cap: int, max_chunk_v: int, max_chunk_a: int,
                  lam: float = 0.02, ratio_r: float = 5.0, temperature: float = 0.2, softmax_scale: float = 0.0,
                  budget_min: int = 0, budget_max: int = 0, causal: int = 1, sim_source: int = 0, sim_stride_v: int = 1,
-                 sim_stride_a: int = 1, score_path: int = 0, select_scope: int = 0, d_model: int = 0, device: str = "cuda:0"):
+                 sim_stride_a: int = 1, score_path: int = 0, select_scope: int = 0, d_model: int = 0, score_ctas: int = 0,
+                 device: str = "cuda:0"):
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise OmniMemError("no CUDA device: the OmniMem path has no CPU fallback")
@@ -173,7 +174,7 @@ class OmniMem:
         self.torch_dtype = torch.float32 if dtype == "fp32" else torch.bfloat16
         self.cfg = omnimem_config(L, Hq, Hkv, D, OMNIMEM_FP32 if dtype == "fp32" else OMNIMEM_BF16, cache_cap, max_chunk_v,
                                   max_chunk_a, softmax_scale, lam, ratio_r, temperature, budget_min, budget_max, causal,
-                                  sim_source, sim_stride_v, sim_stride_a, score_path, select_scope, d_model)
+                                  sim_source, sim_stride_v, sim_stride_a, score_path, select_scope, d_model, score_ctas)
         self.ctx = C.c_void_p()
         with torch.cuda.device(self.device):
             self._check(self.lib.omnimem_create(C.byref(self.cfg), C.byref(self.ctx)), "omnimem_create")

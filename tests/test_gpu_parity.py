@@ -153,6 +153,21 @@ def test_bf16_tcgen05_small(wl):
     check_step(wl)
 
 
+@pytest.mark.parametrize("ctas", [1, 2, 3, 7])
+def test_persistent_ctas_walk_several_items(ctas):
+    """The tcgen05 scoring kernels are persistent: with `score_ctas` CTAs instead of one per SM, every CTA of these small
+    shapes walks several work items, so ring positions and barrier phases carry across items, across skipped items
+    (cache blocks beyond n), across ragged last blocks where one sub-tile's warps have nothing to do (they must not run
+    ahead of the ring), the lse ring wraps inside and between items, and an empty cache leaves only chunk items.
+    Results must not depend on the number of CTAs: rules (a)-(c) as everywhere."""
+    for wl in (SMALL2, SMALL3, SMALL4):
+        for n_v in (wl.n_v, wl.n_v - 37, 300, 0):
+            check_step(wl.replace(n_v=n_v), eng_kw=dict(score_ctas=ctas), check_rowH=(n_v == 300))
+    check_step(SMALL2, eng_kw=dict(score_ctas=ctas, causal=0), ref_kw=dict(causal=0))
+    check_step(SMALL3.replace(Hq=14, Hkv=2), eng_kw=dict(score_ctas=ctas))          # G = 7: 35 query tiles per key block
+    check_step(SMALL3, eng_kw=dict(score_ctas=ctas), modality=I.modality_pattern(SMALL3, 5))
+
+
 @pytest.mark.parametrize("wl", [SMALL2, SMALL4], ids=lambda w: w.name)
 def test_bf16_simt_path_small(wl):
     check_step(wl, eng_kw=dict(score_path=1))
@@ -684,7 +699,8 @@ def test_random_shapes_fuzz(seed):
         causal = int(g.integers(0, 2))
         scope = int(g.integers(0, 2))
         mod = I.modality_pattern(wl, int(g.integers(1, 12))) if g.integers(0, 2) and Nn_v and Nn_a else None
-        check_step(wl, eng_kw=dict(causal=causal), ref_kw=dict(causal=causal), select_scope=scope, modality=mod,
+        ctas = int(g.choice([0, 0, 1, 2, 5]))              # persistent scoring CTAs (0 = one per SM)
+        check_step(wl, eng_kw=dict(causal=causal, score_ctas=ctas), ref_kw=dict(causal=causal), select_scope=scope, modality=mod,
                    check_rowH=bool(g.integers(0, 2)))
 
 
