@@ -425,7 +425,8 @@ def measure_stream(args, wl: I.Workload, local_rank: int):
     }
 
 
-NCU_CAPTURES = {"cfg2_qwen25omni7b": "profiles/r02_score_tc_full_cfg2.csv"}   # committed `ncu --set full` summaries
+NCU_CAPTURES = {"cfg2_qwen25omni7b": "profiles/r02_score_tc_full_cfg2.csv",    # committed `ncu --set full` summaries
+                "cfg3_8b": "profiles/r02_score_tc_full_cfg3.csv"}
 
 
 def ncu_traffic(workload: str, pass_no: int):
@@ -444,7 +445,10 @@ def ncu_traffic(workload: str, pass_no: int):
     tot = 0.0
     for r in rows:
         if r and r[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
-            tot += float(r[col]) * unit[r[1]]
+            v = float(r[col])
+            if not np.isfinite(v):
+                return None, f"{rel}: counter not captured for this launch"
+            tot += v * unit[r[1]]
     return (tot or None), rel
 
 

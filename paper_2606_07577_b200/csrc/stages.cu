@@ -44,10 +44,13 @@ template <> struct Vec16<__nv_bfloat16> {
 };
 
 // kTPR = 4 threads cover one row, kVec 16-byte vectors each (vector j of the row goes to thread j % 4, so a warp's load
-// instruction touches 8 rows x 64 contiguous bytes).  One block = kUnroll * 64 consecutive items of one (layer, KV
-// head); every thread first issues all of its 2 * kUnroll * kVec loads (row t and its partner t + sigma, which a
-// neighbouring block reads again out of L2), then reduces: enough bytes in flight per SM to run at HBM speed, and
-// ~25 instructions per 16 bytes instead of ~115 (the first version was instruction-bound: ncu, profiles/).
+// instruction touches 8 rows x 64 contiguous bytes).  One block works on kUnroll * 64 consecutive items of one (layer, KV
+// head) at a time; every thread first issues all of its 2 * kUnroll * kVec loads (row t and its partner t + sigma, which
+// comes out of L1 / L2), then reduces: enough bytes in flight per SM to run at HBM speed, and ~25 instructions per 16 bytes
+// instead of ~115 (the first version was instruction-bound: ncu, profiles/).
+// Items are numbered DENSELY over the rows that exist (K_v visual, then K_a audio: device counts), and a fixed number of
+// blocks per (layer, KV head) strides over them: sized by capacity, 43 % of the blocks of config 2 had no row to read and
+// their launch overhead alone was a quarter of the kernel's time.
 template <typename T, int kVec, int kUnroll>
 __global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __restrict__ cacheX,
                                                      const T* __restrict__ chunkX, float* __restrict__ cosn) {
@@ -57,42 +60,46 @@ __global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __re
   if (layer_skips_scoring(p, l)) return;
   const int sub = threadIdx.x % kTPR;
   const int n_v = p.n_v[l], n = p.n[l];
+  const int Kv = seg_len(p, n_v, n, 0), Ka = seg_len(p, n_v, n, 1);
   const uint4* cbase = reinterpret_cast<const uint4*>(cacheX + (long long)lh * p.cache_cap * p.D) + sub;
   const uint4* kbase = reinterpret_cast<const uint4*>(chunkX + (long long)lh * p.Nn * p.D) + sub;
   const int row_vecs = kVec * kTPR;
-  uint4 xv[kUnroll][kVec], yv[kUnroll][kVec];
-  bool active[kUnroll];
-  int it[kUnroll];
+  for (int d0 = blockIdx.x * (kUnroll * kRows); d0 < Kv + Ka; d0 += gridDim.x * (kUnroll * kRows)) {
+    uint4 xv[kUnroll][kVec], yv[kUnroll][kVec];
+    bool active[kUnroll];
+    int out[kUnroll];
 #pragma unroll
-  for (int u = 0; u < kUnroll; ++u) {
-    it[u] = (blockIdx.x * kUnroll + u) * kRows + threadIdx.x / kTPR;
-    const int m = it[u] < p.seg_cap_v ? 0 : 1;
-    const int t = m == 0 ? it[u] : it[u] - p.seg_cap_v;
-    const int sg = m == 0 ? p.stride_v : p.stride_a;
-    active[u] = it[u] < items && t + sg < seg_len(p, n_v, n, m);
-    if (active[u]) {
-      bool cx, cy;
-      const int rx = seg_row(p, n_v, n, m, t, cx), ry = seg_row(p, n_v, n, m, t + sg, cy);
-      const uint4* x = (cx ? kbase : cbase) + (long long)rx * row_vecs;
-      const uint4* y = (cy ? kbase : cbase) + (long long)ry * row_vecs;
+    for (int u = 0; u < kUnroll; ++u) {
+      const int d = d0 + u * kRows + threadIdx.x / kTPR;      // dense item: visual rows, then audio rows
+      const int m = d < Kv ? 0 : 1;
+      const int t = m == 0 ? d : d - Kv;
+      const int sg = m == 0 ? p.stride_v : p.stride_a;
+      out[u] = m == 0 ? t : p.seg_cap_v + t;
+      active[u] = d < Kv + Ka && t + sg < (m == 0 ? Kv : Ka);
+      if (active[u]) {
+        bool cx, cy;
+        const int rx = seg_row(p, n_v, n, m, t, cx), ry = seg_row(p, n_v, n, m, t + sg, cy);
+        const uint4* x = (cx ? kbase : cbase) + (long long)rx * row_vecs;
+        const uint4* y = (cy ? kbase : cbase) + (long long)ry * row_vecs;
 #pragma unroll
-      for (int i = 0; i < kVec; ++i) { xv[u][i] = __ldg(x + i * kTPR); yv[u][i] = __ldg(y + i * kTPR); }
-    }
-  }
-#pragma unroll
-  for (int u = 0; u < kUnroll; ++u) {
-    float dot = 0.f, nx = 0.f, ny = 0.f;
-    if (active[u]) {
-#pragma unroll
-      for (int i = 0; i < kVec; ++i) Vec16<T>::acc(xv[u][i], yv[u][i], dot, nx, ny);
+        for (int i = 0; i < kVec; ++i) { xv[u][i] = __ldg(x + i * kTPR); yv[u][i] = __ldg(y + i * kTPR); }
+      }
     }
 #pragma unroll
-    for (int o = kTPR / 2; o; o >>= 1) {
-      dot += __shfl_xor_sync(0xffffffffu, dot, o);
-      nx += __shfl_xor_sync(0xffffffffu, nx, o);
-      ny += __shfl_xor_sync(0xffffffffu, ny, o);
+    for (int u = 0; u < kUnroll; ++u) {
+      float dot = 0.f, nx = 0.f, ny = 0.f;
+      if (active[u]) {
+#pragma unroll
+        for (int i = 0; i < kVec; ++i) Vec16<T>::acc(xv[u][i], yv[u][i], dot, nx, ny);
+      }
+#pragma unroll
+      for (int o = kTPR / 2; o; o >>= 1) {
+        dot += __shfl_xor_sync(0xffffffffu, dot, o);
+        nx += __shfl_xor_sync(0xffffffffu, nx, o);
+        ny += __shfl_xor_sync(0xffffffffu, ny, o);
+      }
+      if (active[u] && sub == 0) cosn[(long long)lh * items + out[u]] = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
     }
-    if (active[u] && sub == 0) cosn[(long long)lh * items + it[u]] = dot / fmaxf(sqrtf(nx) * sqrtf(ny), 1e-8f);  // R12
   }
 }
 
@@ -161,7 +168,14 @@ cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const Ste
   const int vec = row_bytes / 64;                      // 16-byte vectors per thread (4 threads per row): 2, 4 or 8
   const int unroll = vec == 8 ? 1 : 2;
   const int rows_per_block = unroll * 64;
-  const dim3 grid((unsigned)((items + rows_per_block - 1) / rows_per_block), (unsigned)(p.L * p.Hkv));
+  // a fixed number of blocks per (layer, KV head) strides over the rows that exist (device counts): just under 8 full
+  // waves of 3 resident blocks per SM (80 registers), so that no wave is left mostly empty and no block finds nothing to do
+  const int lh_count = p.L * p.Hkv;
+  int per_lh = ctx->sm_count * 3 * 8 / lh_count;
+  const int need = (items + rows_per_block - 1) / rows_per_block;
+  if (per_lh > need) per_lh = need;
+  if (per_lh < 1) per_lh = 1;
+  const dim3 grid((unsigned)per_lh, (unsigned)lh_count);
   ++*launches;
 #define OMNIMEM_COS(T, V, U) cosine_kernel<T, V, U><<<grid, 256, 0, st>>>(p, (const T*)cx, (const T*)kx, b.cosn)
   if (ctx->cfg.dtype == OMNIMEM_FP32) {
