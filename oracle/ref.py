@@ -37,10 +37,31 @@ def build(force: bool = False) -> str:
                    "-fopenmp", "-fPIC", "-shared", "-o", so, _SRC, "-lm"]
             subprocess.run(cmd, check=True)
         return so
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+    # -march=native ties the object to the CPU it was built on, and the built file travels with the tree to other
+    # machines: a stamp records source and CPU flags, and anything else triggers a rebuild
+    stamp, want = _SO + ".stamp", _machine_stamp()
+    have = open(stamp).read() if os.path.exists(stamp) else ""
+    if force or not os.path.exists(_SO) or have != want:
         cmd = ["gcc", "-O2", "-march=native", "-fopenmp", "-fPIC", "-shared", "-o", _SO, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
+        with open(stamp, "w") as f:
+            f.write(want)
     return _SO
+
+
+def _machine_stamp() -> str:
+    import hashlib
+    flags = ""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    flags = line
+                    break
+    except OSError:
+        pass
+    with open(_SRC, "rb") as f:
+        return hashlib.sha256(f.read() + flags.encode()).hexdigest()
 
 
 class _Params(C.Structure):
