@@ -213,10 +213,13 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
     stage_sum = {}
     launches = 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     with ClockSampler(local_rank) as clk:
         ev0.record()
-        for _ in range(args.steps):
+        step_ev[0].record()
+        for i in range(args.steps):
             eng.compress_chunk(src, chunk, B, dst)
+            step_ev[i + 1].record()
             ms, nl = eng.stage_ms()                      # waits on this step's own events (adds ~us per 10s of ms)
             launches += nl
             for k, v in ms.items():
@@ -224,6 +227,7 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
         ev1.record()
         barrier()
     t_total = ev0.elapsed_time(ev1) / 1e3
+    per_step = [step_ev[i].elapsed_time(step_ev[i + 1]) for i in range(args.steps)]   # min / median too
     clocks = clk.summary()
     eng.set_profiling(False)
 
@@ -315,6 +319,7 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
     out = {
         "metric": "kv_tokens_per_s", "value": job_value(world, work["Nk"], t_step), "unit": "KV tok/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
+        "ms_per_step_min": float(np.min(per_step)), "ms_per_step_median": float(np.median(per_step)),
         "scaling": "weak", "vs_baseline": None, "dtype": wl.dtype, "data": "synthetic",
         "config": {"workload": wl.name, "L": wl.L, "Hq": wl.Hq, "Hkv": wl.Hkv, "D": wl.D, "cache_rows": wl.n_v + wl.n_a,
                    "chunk_rows": wl.Nn, "budget": wl.budget, "parallelism": f"replicas x{world}",
