@@ -3,7 +3,11 @@
 // It is the step BEFORE the compression path: the LSE it writes is what Eq.6's column sums
 // need, so a caller that runs this forward passes `lse` to omnimem_compress_chunk and score pass 1 disappears.
 //
-// One CTA = 256 queries of one query head = two 128-row sub-tiles that take turns on the tensor pipe:
+// PERSISTENT CTAs (one per SM; cfg.score_ctas overrides) draw work items from a device counter through a two-slot
+// shared-memory queue, as in score_tc.cu; the K / V ring, the S / P / O barriers of each sub-tile and all their phases run on
+// across items; the next item's Q tiles are loaded as soon as the current item's last S product has been issued, and its
+// first S products run under the current item's epilogue.
+// One item = 256 queries of one query head = two 128-row sub-tiles that take turns on the tensor pipe:
 //   S_s = Q_s K_j^T   (SS mode: Q from shared memory, staged once; K tiles stream through a 4-slot ring shared with V)
 //   softmax threads (one per query row): P = 2^(c2 S - m) in fp32, row sum l in fp32, P rounded to bf16 and written
 //   back into tensor memory ON TOP of S_s (columns [0, 64) of its 128)
@@ -13,7 +17,8 @@
 // The running reference m is LAZY, as in score pass 1: a tile's exponentials are taken against m as it stands; only if
 // that could overflow (tile sum not below 2^100) the thread takes the exact path: tile maximum, new reference, and a
 // rescale of its O row in tensor memory (possible because nothing of this sub-tile is in flight at that point).
-// Warp roles: 0 = TMA producer, 1 = MMA issuer, 2 = TMEM allocator, 4-11 = softmax / epilogue (sub-tile x lane quarter).
+// Warp roles: 0 = TMA producer + item scheduler, 1 = MMA issuer, 2 = TMEM allocator, 4-11 = softmax / epilogue (sub-tile x
+// lane quarter).
 #include <cuda.h>
 #include <math.h>
 
@@ -33,7 +38,7 @@ constexpr int kThr = 384;             // 4 control warps + 8 softmax warps
 constexpr int kOffQ = 0;                          // [2 sub][32 KB]
 constexpr int kOffKV = 2 * kTileB;                // [kSlots][32 KB]
 constexpr int kOffBar = kOffKV + kSlots * kTileB;
-constexpr size_t kSmem = 1024 + kOffBar + 256;
+constexpr size_t kSmem = 1024 + kOffBar + 256;   // barriers, item queue and the tensor-memory slot: 180 bytes
 constexpr uint32_t kColS = 0, kColO = 256;        // tensor-memory columns
 #ifndef OMNIMEM_ATT_POLY_NUM
 #define OMNIMEM_ATT_POLY_NUM 2
@@ -48,7 +53,32 @@ struct AttendArgs {
   StepParams p;
   __nv_bfloat16* y;   // [L, Hq, Nn, 128]
   float* lse_nat;     // [L, Hq, Nn]
+  int nx, ny, n_items;   // item grid (x = 256-query block, y = query head, z = layer), x fastest
+  int* counter;          // zeroed by the launcher
 };
+
+// What one item is, computed identically by every role.
+struct AItem {
+  int l, jh, h, row0, n, nct, nnt, ntiles;
+  int nt[2];
+};
+__device__ __forceinline__ void make_item(const AttendArgs& a, int item, AItem& w) {
+  const StepParams& p = a.p;
+  const int bx = a.nx - 1 - item % a.nx;          // the longest items (most visible chunk tiles) of a head first
+  const int yz = item / a.nx;
+  w.jh = yz % a.ny;
+  w.l = yz / a.ny;
+  w.h = w.jh / p.G;
+  w.n = uniform(p.n[w.l]);
+  w.row0 = bx * 2 * kT;                           // first query of this item
+  w.nct = (w.n + kT - 1) / kT;                    // cache tiles
+  w.nnt = (p.Nn + kT - 1) / kT;                   // chunk tiles
+  for (int s = 0; s < 2; ++s) {
+    const int r0 = w.row0 + s * kT;
+    w.nt[s] = r0 < p.Nn ? w.nct + (p.causal ? min(w.nnt, r0 / kT + 1) : w.nnt) : 0;   // R3: chunk key t visible iff t <= i
+  }
+  w.ntiles = max(w.nt[0], w.nt[1]);
+}
 
 __device__ __forceinline__ void tc_ld32x(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile(
@@ -77,17 +107,6 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
                  const __grid_constant__ CUtensorMap mapVn, const AttendArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const StepParams& p = a.p;
-  const int l = blockIdx.z, jh = blockIdx.y, h = jh / p.G;
-  const int n = uniform(p.n[l]);
-  const int row0 = blockIdx.x * 2 * kT;                         // first query of this CTA
-  const int nct = (n + kT - 1) / kT, nnt = (p.Nn + kT - 1) / kT;  // cache tiles, chunk tiles
-  int nt[2];
-  for (int s = 0; s < 2; ++s) {
-    const int r0 = row0 + s * kT;
-    nt[s] = r0 < p.Nn ? nct + (p.causal ? min(nnt, r0 / kT + 1) : nnt) : 0;   // R3: chunk key t visible iff t <= i
-  }
-  const int ntiles = max(nt[0], nt[1]);
-  if (ntiles == 0) return;
 
   const uint32_t s_raw = smem_u32(smem_raw);
   const uint32_t sBase = (s_raw + 1023u) & ~1023u;
@@ -95,12 +114,18 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
   const uint32_t sQ = sBase + kOffQ, sKV = sBase + kOffKV, bars = sBase + kOffBar;
   const uint32_t bar_q = bars, bar_full = bars + 8, bar_empty = bar_full + 8 * kSlots;
   const uint32_t bar_s = bar_empty + 8 * kSlots, bar_p = bar_s + 16, bar_o = bar_p + 16;
-  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBar + 8 + 16 * kSlots + 48);
+  const uint32_t bar_qfree = bar_o + 16, bar_ofree = bar_qfree + 8;                 // Q tiles / O accumulators of the last item consumed
+  const uint32_t bar_qfull = bar_ofree + 16, bar_qempty = bar_qfull + 16, sQueue = bar_qempty + 16;   // item queue [2]
+  uint32_t* tmem_slot = (uint32_t*)(smem + kOffBar + 8 + 16 * kSlots + 48 + 8 + 16 + 32 + 8);
   const int warp = uniform(threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     mbar_init(bar_q, 1);
+    mbar_init(bar_qfree, 1);
     for (int i = 0; i < kSlots; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(bar_s + 8 * s, 1); mbar_init(bar_p + 8 * s, 4); mbar_init(bar_o + 8 * s, 1); }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(bar_s + 8 * s, 1); mbar_init(bar_p + 8 * s, 4); mbar_init(bar_o + 8 * s, 1); mbar_init(bar_ofree + 8 * s, 4);
+      mbar_init(bar_qfull + 8 * s, 1); mbar_init(bar_qempty + 8 * s, 9);     // consumers: the MMA warp + 8 softmax warps
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
@@ -111,109 +136,160 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)uniform((int)*tmem_slot);
-  const int lhq = l * p.Hq + jh, lhk = l * p.Hkv + h;
+
+  int qi = 0, qph = 0;      // consumer side of the item queue
+  auto next_item = [&]() -> int {
+    mbar_wait(bar_qfull + 8 * qi, qph);
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(sQueue + 4 * qi) : "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_qempty + 8 * qi);
+    if (++qi == 2) { qi = 0; qph ^= 1; }
+    return uniform((int)v);
+  };
 
   if (warp == 0) {
-    // ===================== TMA producer: Q once, then K_0, V_0, K_1, V_1, ... through the ring =====================
-    if (elect_one()) {
-      mbar_expect_tx(bar_q, (nt[1] > 0 ? 2 : 1) * kTileB);
-      for (int s = 0; s < 2; ++s)
-        if (nt[s] > 0)
-          for (int kb = 0; kb < 2; ++kb) tma_load_3d(sQ + s * kTileB + kb * (kTileB / 2), &mapQ, kb * 64, row0 + s * kT, lhq, bar_q);
-    }
-    __syncwarp();
-    int slot = 0, ph = 1;
-    for (int j = 0; j < ntiles; ++j) {
-      const bool cache = j < nct;
-      const int r0 = (cache ? j : j - nct) * kT;
-      for (int t = 0; t < 2; ++t) {   // t = 0: K tile, t = 1: V tile
-        mbar_wait(bar_empty + 8 * slot, ph);
-        if (elect_one()) {
-          mbar_expect_tx(bar_full + 8 * slot, kTileB);
-          const CUtensorMap* m = t == 0 ? (cache ? &mapKc : &mapKn) : (cache ? &mapVc : &mapVn);
-          for (int kb = 0; kb < 2; ++kb) tma_load_3d(sKV + slot * kTileB + kb * (kTileB / 2), m, kb * 64, r0, lhk, bar_full + 8 * slot);
+    // ===================== TMA producer: per item Q (once the last item's S products are through), then K_0, V_0, K_1, ... =====================
+    int slot = 0, ph = 1, pq = 0, pqph = 1, qfph = 1;
+    for (;;) {
+      mbar_wait(bar_qempty + 8 * pq, pqph);
+      int item = 0;
+      if (lane == 0) {
+        item = atomicAdd(a.counter, 1);
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(sQueue + 4 * pq), "r"(item) : "memory");
+        mbar_arrive(bar_qfull + 8 * pq);
+      }
+      item = uniform(item);
+      if (++pq == 2) { pq = 0; pqph ^= 1; }
+      if (item >= a.n_items) break;
+      AItem w;
+      make_item(a, item, w);
+      const int lhq = w.l * p.Hq + w.jh, lhk = w.l * p.Hkv + w.h;
+      mbar_wait(bar_qfree, qfph);       // every S product of the previous item has read its Q tiles
+      qfph ^= 1;
+      if (elect_one()) {
+        mbar_expect_tx(bar_q, (w.nt[1] > 0 ? 2 : 1) * kTileB);
+        for (int s = 0; s < 2; ++s)
+          if (w.nt[s] > 0)
+            for (int kb = 0; kb < 2; ++kb) tma_load_3d(sQ + s * kTileB + kb * (kTileB / 2), &mapQ, kb * 64, w.row0 + s * kT, lhq, bar_q);
+      }
+      __syncwarp();
+      for (int j = 0; j < w.ntiles; ++j) {
+        const bool cache = j < w.nct;
+        const int r0 = (cache ? j : j - w.nct) * kT;
+        for (int t = 0; t < 2; ++t) {   // t = 0: K tile, t = 1: V tile
+          mbar_wait(bar_empty + 8 * slot, ph);
+          if (elect_one()) {
+            mbar_expect_tx(bar_full + 8 * slot, kTileB);
+            const CUtensorMap* m = t == 0 ? (cache ? &mapKc : &mapKn) : (cache ? &mapVc : &mapVn);
+            for (int kb = 0; kb < 2; ++kb) tma_load_3d(sKV + slot * kTileB + kb * (kTileB / 2), m, kb * 64, r0, lhk, bar_full + 8 * slot);
+          }
+          __syncwarp();
+          if (++slot == kSlots) { slot = 0; ph ^= 1; }
         }
-        __syncwarp();
-        if (++slot == kSlots) { slot = 0; ph ^= 1; }
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     int slot = 0, ph = 0;             // ring position of the next tile to consume (K_0, V_0, K_1, ...)
+    int done[2] = {0, 0};             // tiles of sub-tile s completed in earlier items: phase of its S / P / O barriers
+    int items_s[2] = {0, 0};          // items in which sub-tile s had rows: phase of its O-free barrier
+    int qph_mma = 0;
     auto advance = [&]() { if (++slot == kSlots) { slot = 0; ph ^= 1; } };
-    auto issue_s = [&](int s, int kslot) {   // S_s = Q_s K^T
-      if (elect_one()) {
-        const uint64_t a_desc = umma_desc_sw128(sQ + s * kTileB), b_desc = umma_desc_sw128(sKV + kslot * kTileB);
+    for (;;) {
+      const int item = next_item();
+      if (item >= a.n_items) break;
+      AItem w;
+      make_item(a, item, w);
+      const int n = w.n, nct = w.nct, ntiles = w.ntiles;
+      auto issue_s = [&](int s, int kslot) {   // S_s = Q_s K^T
+        if (elect_one()) {
+          const uint64_t a_desc = umma_desc_sw128(sQ + s * kTileB), b_desc = umma_desc_sw128(sKV + kslot * kTileB);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-          const uint64_t koff = (uint64_t)(((kk >> 2) * (kTileB / 2) + (kk & 3) * 32) >> 4);
-          tc_mma_bf16(tmem_base + kColS + s * kT, a_desc + koff, b_desc + koff, kIdescQK, kk > 0 ? 1u : 0u);
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint64_t koff = (uint64_t)(((kk >> 2) * (kTileB / 2) + (kk & 3) * 32) >> 4);
+            tc_mma_bf16(tmem_base + kColS + s * kT, a_desc + koff, b_desc + koff, kIdescQK, kk > 0 ? 1u : 0u);
+          }
+          tc_commit(bar_s + 8 * s);
         }
-        tc_commit(bar_s + 8 * s);
-      }
-      __syncwarp();
-    };
-    auto issue_o = [&](int s, int vslot, int j) {   // O_s += P_s V
-      mbar_wait(bar_p + 8 * s, j & 1);
-      tc_fence_after();
-      if (elect_one()) {
-        const uint64_t b_desc = umma_desc_sw128_mn(sKV + vslot * kTileB, kTileB / 2);
+        __syncwarp();
+      };
+      auto issue_o = [&](int s, int vslot, int j) {   // O_s += P_s V
+        mbar_wait(bar_p + 8 * s, (done[s] + j) & 1);
+        if (j == 0) mbar_wait(bar_ofree + 8 * s, (items_s[s] & 1) ^ 1);   // the last item's epilogue has read O_s
+        tc_fence_after();
+        if (elect_one()) {
+          const uint64_t b_desc = umma_desc_sw128_mn(sKV + vslot * kTileB, kTileB / 2);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)   // 16 keys per step: 8 TMEM columns of P, 16 rows (2048 B) of the V tile
-          tc_mma_bf16_ts(tmem_base + kColO + s * kT, tmem_base + kColS + s * kT + kk * 8, b_desc + (uint64_t)((kk * 2048) >> 4),
-                         kIdescPV, (j > 0 || kk > 0) ? 1u : 0u);
-        tc_commit(bar_o + 8 * s);
-      }
+          for (int kk = 0; kk < 8; ++kk)   // 16 keys per step: 8 TMEM columns of P, 16 rows (2048 B) of the V tile
+            tc_mma_bf16_ts(tmem_base + kColO + s * kT, tmem_base + kColS + s * kT + kk * 8, b_desc + (uint64_t)((kk * 2048) >> 4),
+                           kIdescPV, (j > 0 || kk > 0) ? 1u : 0u);
+          tc_commit(bar_o + 8 * s);
+        }
+        __syncwarp();
+      };
+      mbar_wait(bar_q, qph_mma);
+      qph_mma ^= 1;
+      mbar_wait(bar_full + 8 * slot, ph);   // K_0
+      tc_fence_after();
+      for (int s = 0; s < 2; ++s) if (w.nt[s] > 0) issue_s(s, slot);
+      if (ntiles == 1) { if (elect_one()) tc_commit(bar_qfree); __syncwarp(); }   // (no further S product in this item)
+      if (elect_one()) tc_commit(bar_empty + 8 * slot);
       __syncwarp();
-    };
-    mbar_wait(bar_q, 0);
-    mbar_wait(bar_full + 8 * slot, ph);   // K_0
-    tc_fence_after();
-    for (int s = 0; s < 2; ++s) if (nt[s] > 0) issue_s(s, slot);
-    if (elect_one()) tc_commit(bar_empty + 8 * slot);
-    __syncwarp();
-    advance();
-    for (int j = 0; j < ntiles; ++j) {
-      const int vslot = slot, vph = ph;
       advance();
-      const int kslot = slot;
-      mbar_wait(bar_full + 8 * vslot, vph);   // V_j
-      if (j == nct - 1 && (n & (kT - 1)) != 0) {
-        // the last cache tile is ragged: rows >= n of the V tile are stale cache rows.  Their P columns are zero, but
-        // 0 * (Inf or NaN bits) would poison O: zero those rows in shared memory (a row is one 128-byte line per K-block)
-        const int first = n - j * kT;
-        for (int idx = lane; idx < (kT - first) * 16; idx += 32) {
-          const int r = first + (idx >> 4), c = idx & 15;
-          const uint32_t addr = sKV + vslot * kTileB + (c >> 3) * (kTileB / 2) + r * 128 + (c & 7) * 16;
-          asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0) : "memory");
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncwarp();
-      }
-      tc_fence_after();
-      if (j < nt[0]) issue_o(0, vslot, j);
-      if (j + 1 < ntiles) { mbar_wait(bar_full + 8 * kslot, ph); tc_fence_after(); }   // K_{j+1}
-      if (j + 1 < nt[0]) issue_s(0, kslot);
-      if (j < nt[1]) issue_o(1, vslot, j);
-      if (elect_one()) tc_commit(bar_empty + 8 * vslot);
-      __syncwarp();
-      if (j + 1 < nt[1]) issue_s(1, kslot);
-      if (j + 1 < ntiles) {
-        if (elect_one()) tc_commit(bar_empty + 8 * kslot);
-        __syncwarp();
+      for (int j = 0; j < ntiles; ++j) {
+        const int vslot = slot, vph = ph;
         advance();
+        const int kslot = slot;
+        mbar_wait(bar_full + 8 * vslot, vph);   // V_j
+        if (j == nct - 1 && (n & (kT - 1)) != 0) {
+          // the last cache tile is ragged: rows >= n of the V tile are stale cache rows.  Their P columns are zero, but
+          // 0 * (Inf or NaN bits) would poison O: zero those rows in shared memory (a row is one 128-byte line per K-block)
+          const int first = n - j * kT;
+          for (int idx = lane; idx < (kT - first) * 16; idx += 32) {
+            const int r = first + (idx >> 4), c = idx & 15;
+            const uint32_t addr = sKV + vslot * kTileB + (c >> 3) * (kTileB / 2) + r * 128 + (c & 7) * 16;
+            asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0) : "memory");
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+        }
+        tc_fence_after();
+        if (j < w.nt[0]) issue_o(0, vslot, j);
+        if (j + 1 < ntiles) { mbar_wait(bar_full + 8 * kslot, ph); tc_fence_after(); }   // K_{j+1}
+        if (j + 1 < w.nt[0]) issue_s(0, kslot);
+        if (j < w.nt[1]) issue_o(1, vslot, j);
+        if (elect_one()) tc_commit(bar_empty + 8 * vslot);
+        __syncwarp();
+        if (j + 1 < w.nt[1]) issue_s(1, kslot);
+        if (j + 2 == ntiles) { if (elect_one()) tc_commit(bar_qfree); __syncwarp(); }   // the item's last S products are issued
+        if (j + 1 < ntiles) {
+          if (elect_one()) tc_commit(bar_empty + 8 * kslot);
+          __syncwarp();
+          advance();
+        }
       }
+      for (int s = 0; s < 2; ++s) { done[s] += w.nt[s]; items_s[s] += w.nt[s] > 0 ? 1 : 0; }
     }
   } else if (warp >= 4) {
     // ===================== softmax / epilogue: thread = one query row of sub-tile s =====================
     const int s = (warp - 4) >> 2, q4 = warp & 3;
-    const int r = q4 * 32 + lane, i = row0 + s * kT + r;
-    if (nt[s] > 0) {
-      const float c2 = p.scale_log2e;
-      const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
-      const uint32_t tS = t_lane + kColS + s * kT, tO = t_lane + kColO + s * kT;
+    const int r = q4 * 32 + lane;
+    const float c2 = p.scale_log2e;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(q4 * 32) << 16);
+    const uint32_t tS = t_lane + kColS + s * kT, tO = t_lane + kColO + s * kT;
+    int done = 0;                     // tiles of this sub-tile completed in earlier items: phase of its S / P / O barriers
+    for (;;) {
+    const int item = next_item();
+    if (item >= a.n_items) break;
+    AItem w;
+    make_item(a, item, w);
+    const int n = w.n, nct = w.nct, i = w.row0 + s * kT + r;
+    const int lhq = w.l * p.Hq + w.jh;
+    const int nts = uniform(s == 0 ? w.nt[0] : w.nt[1]);
+    if (nts > 0) {
       float m_ref = -INFINITY, lsum = 0.f;
-      for (int j = 0; j < nt[s]; ++j) {
+      for (int j = 0; j < nts; ++j) {
         int limit;                               // visible key columns of this tile for this row
         if (j < nct) limit = n - j * kT;
         else {
@@ -221,7 +297,7 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
           limit = p.Nn - t0;
           if (p.causal) limit = min(limit, i - t0 + 1);
         }
-        mbar_wait(bar_s + 8 * s, j & 1);
+        mbar_wait(bar_s + 8 * s, (done + j) & 1);
         tc_fence_after();
         uint32_t pk[64];                         // the tile's P row, bf16 pairs
         float tsum, pmax;
@@ -293,7 +369,7 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
             // O_s(j) waits for this thread: the O row can be rescaled in place
             const float sc = ex2(m_ref - m_new);
             lsum *= sc;
-            mbar_wait(bar_o + 8 * s, (j - 1) & 1);
+            mbar_wait(bar_o + 8 * s, (done + j - 1) & 1);
             tc_fence_after();
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -317,7 +393,7 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
         if (lane == 0) mbar_arrive(bar_p + 8 * s);
       }
       // epilogue: Y = O / l (bf16), lse = ln 2 (m + log2 l)
-      mbar_wait(bar_o + 8 * s, (nt[s] - 1) & 1);
+      mbar_wait(bar_o + 8 * s, (done + nts - 1) & 1);
       tc_fence_after();
       const float inv = 1.f / lsum;
       const bool valid = i < p.Nn;
@@ -327,6 +403,11 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
         uint32_t v[32];
         tc_ld32x(tO + c * 32, v);
         tc_wait_ld();
+        if (c == 3) {                            // O_s is in registers: the next item's first P V product may overwrite it
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_ofree + 8 * s);
+        }
         if (valid) {
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
@@ -340,7 +421,9 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
         }
       }
       if (valid) a.lse_nat[(long long)lhq * p.Nn + i] = (m_ref + log2f(lsum)) * 0.6931471805599453f;
+      done += nts;
     }
+    }  // work items
   }
   tc_fence_before();
   __syncthreads();
@@ -393,11 +476,16 @@ cudaError_t launch_attend_tc(const omnimem_ctx* ctx, const StepParams& p, const 
   a.p = p;
   a.y = (__nv_bfloat16*)y;
   a.lse_nat = lse_nat;
+  a.nx = (p.Nn + 2 * kT - 1) / (2 * kT);
+  a.ny = p.Hq;
+  a.n_items = a.nx * p.Hq * p.L;
+  a.counter = ctx->sched + 2;
   e = cudaFuncSetAttribute(attend_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
   if (e != cudaSuccess) return e;
-  const dim3 grid((p.Nn + 2 * kT - 1) / (2 * kT), p.Hq, p.L);
+  if ((e = cudaMemsetAsync(a.counter, 0, sizeof(int), st)) != cudaSuccess) return e;
+  const int ctas = ctx->cfg.score_ctas > 0 && ctx->cfg.score_ctas < ctx->sm_count ? ctx->cfg.score_ctas : ctx->sm_count;
   ++*launches;
-  attend_tc_kernel<<<grid, kThr, kSmem, st>>>(mq, mkc, mkn, mvc, mvn, a);
+  attend_tc_kernel<<<a.n_items < ctas ? a.n_items : ctas, kThr, kSmem, st>>>(mq, mkc, mkn, mvc, mvn, a);
   return cudaGetLastError();
 }
 

@@ -87,6 +87,19 @@ def test_attend_bf16_tcgen05_small(wl):
     check_attend(wl, eng_kw=dict(causal=0), ref_kw=dict(causal=0))
 
 
+@pytest.mark.parametrize("ctas", [1, 2, 5])
+def test_attend_persistent_ctas_walk_several_items(ctas):
+    """The tcgen05 forward is persistent: with `score_ctas` CTAs every CTA of these small shapes walks several items, so the
+    K / V ring, the S / P / O barrier phases of each sub-tile, the Q-free and O-free hand-overs and the item queue carry
+    across items, including ragged last blocks (one sub-tile without rows) and an empty cache."""
+    for wl in (SMALL2, SMALL3, SMALL4):
+        for n_v in (wl.n_v, wl.n_v - 37, 0):
+            check_attend(wl.replace(n_v=n_v), eng_kw=dict(score_ctas=ctas), also_compress=(n_v == wl.n_v))
+    check_attend(SMALL2, eng_kw=dict(score_ctas=ctas, causal=0), ref_kw=dict(causal=0), also_compress=False)
+    check_attend(SMALL3.replace(n_v=1, n_a=0, Nn_v=257, Nn_a=0, cache_cap=300, budget=258), eng_kw=dict(score_ctas=ctas),
+                 also_compress=False)
+
+
 def test_attend_bf16_simt_paths():
     check_attend(SMALL2, eng_kw=dict(score_path=1))
     check_attend(SMALL2.replace(D=64))
