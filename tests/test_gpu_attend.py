@@ -7,6 +7,8 @@ above a power of two, 2^-9 just below) and rounds Y once to bf16 (<= 2^-8 |Y|), 
 it is attained when one key takes the whole row (p ~ 1, Y ~ v).  fp32 inputs: 1e-5 of the same magnitude.
 Then the point of the row: attend -> compress_chunk(lse = ...) must keep what the two-pass step keeps.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -98,6 +100,26 @@ def test_attend_persistent_ctas_walk_several_items(ctas):
     check_attend(SMALL2, eng_kw=dict(score_ctas=ctas, causal=0), ref_kw=dict(causal=0), also_compress=False)
     check_attend(SMALL3.replace(n_v=1, n_a=0, Nn_v=257, Nn_a=0, cache_cap=300, budget=258), eng_kw=dict(score_ctas=ctas),
                  also_compress=False)
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("OMNIMEM_FUZZ_SEEDS", "6"))))
+def test_attend_random_shapes_fuzz(seed):
+    """Seeded random shapes around the tile edges (128-row tiles, 256-row items, ragged caches, GQA widths), causal or not,
+    with 1-5 persistent CTAs or one per SM: Y and LSE against the oracle."""
+    g = np.random.default_rng(7000 + seed)
+    for rep in range(3):
+        Hkv = int(g.integers(1, 3))
+        G = int(g.choice([1, 2, 4, 7]))
+        Nn_v, Nn_a = int(g.integers(0, 700)), int(g.integers(0, 150))
+        if Nn_v + Nn_a == 0:
+            Nn_v = 1
+        n_v, n_a = int(g.integers(0, 1200)), int(g.integers(0, 200))
+        cap = n_v + n_a + int(g.integers(1, 64))
+        wl = SMALL3.replace(L=int(g.integers(1, 3)), Hq=Hkv * G, Hkv=Hkv, n_v=n_v, n_a=n_a, Nn_v=Nn_v, Nn_a=Nn_a,
+                            budget=max(1, cap // 2), cache_cap=cap)
+        causal = int(g.integers(0, 2))
+        check_attend(wl, eng_kw=dict(causal=causal, score_ctas=int(g.choice([0, 1, 2, 5]))), ref_kw=dict(causal=causal),
+                     also_compress=False)
 
 
 def test_attend_bf16_simt_paths():
