@@ -62,3 +62,25 @@ def test_reference_arm_only_rank0_works():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["n_gpus"] == 2
+
+
+def test_bench_accounting_matches_the_survey_tables():
+    """bench.py's algorithmic work: causal pairs, two-pass flops and minimum bytes of
+    configs 2-4, and the committed ncu summaries the `roofline.traffic` key is read from at run time."""
+    import bench
+    from paper_2606_07577_b200 import inputs as I
+    want = {2: (107.35e6, 43.09e12, 6.12e9), 3: (429.38e6, 253.26e12, 26.47e9), 4: (31.59e6, 18.63e12, 6.16e9)}
+    for cfg, (pairs, flops, nbytes) in want.items():
+        wl = I.CONFIGS[cfg]
+        w = bench.algorithmic_work(wl, wl.n_v, wl.n_a)
+        assert abs(w["pairs"] - pairs) < 0.01e6 * 1.5 and abs(2 * w["f_pass"] - flops) < 0.01e12 and abs(w["bytes"]["total"] - nbytes) < 0.01e9
+        assert w["exps_pass"] == w["pairs"] * wl.Hq * wl.L and w["Nk"] == wl.n_v + wl.n_a + wl.Nn
+    # DRAM traffic per launch of the two scoring passes, read from profiles/: within 5 % of the algorithmic Q + K bytes
+    for name, cfg in (("cfg2_qwen25omni7b", 2), ("cfg3_8b", 3)):
+        wl = I.CONFIGS[cfg]
+        qk = (wl.L * wl.Hq * wl.Nn + wl.L * wl.Hkv * (wl.n_v + wl.n_a + wl.Nn)) * wl.D * 2
+        for pass_no in (1, 2):
+            traffic, src = bench.ncu_traffic(name, pass_no)
+            assert traffic is not None and src.startswith("profiles/"), src
+            assert 1.0 <= traffic / qk < 1.05, (name, pass_no, traffic / qk)
+    assert bench.ncu_traffic("cfg4_4b_tight", 1)[0] is None      # no capture committed: null, with the reason as source
