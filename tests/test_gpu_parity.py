@@ -164,6 +164,15 @@ def test_persistent_ctas_walk_several_items(ctas):
         for n_v in (wl.n_v, wl.n_v - 37, 300, 0):
             check_step(wl.replace(n_v=n_v), eng_kw=dict(score_ctas=ctas), check_rowH=(n_v == 300))
     check_step(SMALL2, eng_kw=dict(score_ctas=ctas, causal=0), ref_kw=dict(causal=0))
+    # layers of different length in one launch (what a ragged budget table leaves behind): full, 137 rows short, nearly empty, empty
+    wl = SMALL3.replace(L=4)
+    x = I.full_inputs(wl)
+    x["n_v"] = x["n_v"].clone()
+    x["n"] = x["n"].clone()
+    for l, (dv, dn) in enumerate(((0, 0), (100, 137), (wl.n_v - 3, wl.n_v + wl.n_a - 5), (wl.n_v, wl.n_v + wl.n_a))):
+        x["n_v"][l] -= dv
+        x["n"][l] -= dn
+    check_step(wl, x=x, eng_kw=dict(score_ctas=ctas))
     check_step(SMALL3.replace(Hq=14, Hkv=2), eng_kw=dict(score_ctas=ctas))          # G = 7: 35 query tiles per key block
     check_step(SMALL3, eng_kw=dict(score_ctas=ctas), modality=I.modality_pattern(SMALL3, 5))
 
