@@ -60,7 +60,9 @@ typedef enum {
   OMNIMEM_UNSUPPORTED = -2,        /* dtype / head_dim / device architecture not supported                        */
   OMNIMEM_WORKSPACE_TOO_SMALL = -3,
   OMNIMEM_CUDA_ERROR = -4,         /* details: omnimem_last_cuda_error                                           */
-  OMNIMEM_CAPACITY = -5            /* chunk larger than max_chunk_v / max_chunk_a (host-visible sizes only)       */
+  OMNIMEM_CAPACITY = -5,           /* chunk larger than max_chunk_v / max_chunk_a (host-visible sizes only)       */
+  OMNIMEM_STATIC_SCRATCH_EXCEEDED = -6 /* omnimem_redundancy_static only: the problem needs more pair cosines than the
+                                      library's built-in array holds (OMNIMEM_STATIC_SCRATCH_FLOATS)              */
 } omnimem_status;
 
 enum { OMNIMEM_FP32 = 0, OMNIMEM_BF16 = 1 };
@@ -233,6 +235,49 @@ OMNIMEM_API int omnimem_compress_chunk_host(omnimem_ctx* ctx, const omnimem_cach
                                 const omnimem_chunk* dev_chunk, const int32_t* layer_budget, omnimem_cache* dst,
                                 int32_t* host_M_v, int32_t* host_M_a, int64_t* h2d_bytes, int64_t* d2h_bytes,
                                 void* ws, size_t ws_bytes, void* stream);
+
+/* ---- Eq.7 redundancy without any allocation ------------------------------------------------------ */
+/* Who this is for.  Everything above assumes the caller can obtain device memory: omnimem_create itself calls cudaMalloc
+ * (work counters, interleaving maps) and every stage wants a workspace of omnimem_workspace_bytes.  Some users of this
+ * library cannot do that at the point where they need the scores.  Two we know of: (1) a serving engine that handed all
+ * of HBM to its own paged KV-cache pool at start-up, so a later cudaMalloc either fails outright or, when it succeeds,
+ * stalls every stream of the device while the driver maps memory in the middle of serving; (2) an operator body that runs
+ * inside a host runtime's callback, is given its input and output tensors and nothing else, and is forbidden to allocate
+ * there.  For them this ONE call computes the redundancy term of the score with no context, no workspace and no
+ * cudaMalloc / cudaFree / allocating library routine on any path: the intermediate pair cosines live in an array that is
+ * part of the library image.
+ *
+ * What it computes: s_m[l, h, t] = mean over the neighbours t +- sim_stride_m that exist inside the appended sequence of
+ * modality m (Eq.3) of cos(x_t, x_neighbour), clamped to [-1, 1], 0 when there is no neighbour -- the same numbers
+ * omnimem_score writes to omnimem_scores.s_v / .s_a.  x are the rows of cache_x [L, Hkv, cache_cap, D] and chunk_x
+ * [L, Hkv, Nn, D] (pass the value buffers for the paper's default, or the key buffers), dtype OMNIMEM_FP32 or
+ * OMNIMEM_BF16, D in {64, 128}, segment conventions as at the top of this header, chunk modality-blocked (visual rows
+ * first).  n_v, n: DEVICE int32 [L].  Nn_v, Nn_a: HOST ints, Nn_m <= max_chunk_m.  s_v, s_a: DEVICE float
+ * [L, Hkv, cache_cap + max_chunk_m], caller-owned like every input; entries at t >= K_m are left untouched.
+ * All work is enqueued on `stream`, which must belong to the CURRENT device; the call does not wait for it.
+ *
+ * The limit.  The built-in array holds OMNIMEM_STATIC_SCRATCH_FLOATS = 2^20 floats (4 MiB; every GPU that loads the
+ * library carries it until the process exits).  One float is needed per (layer, KV head, row at full capacity):
+ *     n_layers * n_kv_heads * (2 * cache_cap + max_chunk_v + max_chunk_a)  <=  OMNIMEM_STATIC_SCRATCH_FLOATS,
+ * else OMNIMEM_STATIC_SCRATCH_EXCEEDED is returned before anything is launched.  Layers are independent, so a larger
+ * model is served by one call per group of layers (config 2's shape: 6 layers per call) with the pointers advanced.
+ *
+ * Sharing.  There is one array per device and every call on that device uses it.  Calls issued to the same stream run one
+ * after the other and are safe.  Two calls that can be on the GPU at the same time (different streams, different host
+ * threads) overwrite each other's intermediates: serialise them yourself (one stream, or an event between them).  The
+ * array keeps the previous call's contents; nothing has to be cleared, because every entry a call reads it has written
+ * first.
+ *
+ * First call.  The first call on each device looks up where the array lives on that device (cudaGetSymbolAddress, once,
+ * under a lock, with that device current) and may make the CUDA runtime load this library's device code.  Make that first
+ * call during start-up, before any stream capture begins; later calls only launch two kernels.
+ * Errors: INVALID_ARG (NULL pointer, non-positive size, stride < 1), UNSUPPORTED (dtype, head_dim, device is not compute
+ * capability 10.x), CAPACITY (Nn_m > max_chunk_m), STATIC_SCRATCH_EXCEEDED, CUDA_ERROR (a runtime call or launch failed). */
+#define OMNIMEM_STATIC_SCRATCH_FLOATS (1 << 20)
+OMNIMEM_API int omnimem_redundancy_static(int32_t dtype, int32_t n_layers, int32_t n_kv_heads, int32_t head_dim,
+                              int32_t cache_cap, int32_t max_chunk_v, int32_t max_chunk_a, int32_t sim_stride_v,
+                              int32_t sim_stride_a, const void* cache_x, const int32_t* n_v, const int32_t* n,
+                              const void* chunk_x, int32_t Nn_v, int32_t Nn_a, float* s_v, float* s_a, void* stream);
 
 /* ---- per-stage device timing (CUDA events on `stream`, recorded inside the calls above when enabled) ---------- */
 enum {

@@ -19,7 +19,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libomnimem.so")
 OBJDIR = os.path.join(HERE, "build")
 STAMP = os.path.join(OBJDIR, "stamp.json")
-SOURCES = ["api.cu", "score_simt.cu", "score_tc.cu", "attend_tc.cu", "stages.cu"]
+SOURCES = ["api.cu", "score_simt.cu", "score_tc.cu", "attend_tc.cu", "stages.cu", "redundancy_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fvisibility=hidden"]

@@ -273,6 +273,9 @@ const char* omnimem_strerror(int status) {
     case OMNIMEM_WORKSPACE_TOO_SMALL: return "workspace too small (see omnimem_workspace_bytes)";
     case OMNIMEM_CUDA_ERROR: return "CUDA error (see omnimem_last_cuda_error)";
     case OMNIMEM_CAPACITY: return "chunk exceeds the context capacities (max_chunk_v / max_chunk_a)";
+    case OMNIMEM_STATIC_SCRATCH_EXCEEDED:
+      return "omnimem_redundancy_static: n_layers * n_kv_heads * (2 * cache_cap + max_chunk_v + max_chunk_a) exceeds the "
+             "built-in scratch array (OMNIMEM_STATIC_SCRATCH_FLOATS = 2^20 floats); call it per group of layers";
     default: return "unknown status";
   }
 }

@@ -22,7 +22,8 @@ STAT_NAMES = ("Hn_v", "Hn_a", "sbar_v", "sbar_a", "C_v", "C_a", "Hn_all", "sbar_
 EXPORTS = ("omnimem_create", "omnimem_destroy", "omnimem_workspace_bytes", "omnimem_seg_cap", "omnimem_strerror",
            "omnimem_last_cuda_error", "omnimem_score", "omnimem_allocate", "omnimem_select", "omnimem_compact",
            "omnimem_compress_chunk", "omnimem_compress_chunk_host", "omnimem_set_profiling", "omnimem_get_stage_ms",
-           "omnimem_calibrate_accumulate", "omnimem_calibrate_budgets", "omnimem_attend")
+           "omnimem_calibrate_accumulate", "omnimem_calibrate_budgets", "omnimem_attend", "omnimem_redundancy_static")
+STATIC_SCRATCH_FLOATS = 1 << 20      # OMNIMEM_STATIC_SCRATCH_FLOATS of include/omnimem.h
 
 
 class OmniMemError(RuntimeError):
@@ -92,6 +93,7 @@ def load_library() -> C.CDLL:
                                                     C.POINTER(i64), C.POINTER(i64), vp, C.c_size_t, vp]
         lib.omnimem_set_profiling.argtypes = [vp, i32]
         lib.omnimem_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32)]
+        lib.omnimem_redundancy_static.argtypes = [i32] * 9 + [vp, vp, vp, vp, i32, i32, vp, vp, vp]
         _lib = lib
     return _lib
 
@@ -102,6 +104,27 @@ def _ptr(t: Optional[torch.Tensor]):
 
 def _stream() -> C.c_void_p:
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def redundancy_static(cache_x: torch.Tensor, n_v: torch.Tensor, n: torch.Tensor, chunk_x: Optional[torch.Tensor],
+                      Nn_v: int, Nn_a: int, max_chunk_v: int, max_chunk_a: int, s_v: torch.Tensor, s_a: torch.Tensor,
+                      sim_stride_v: int = 1, sim_stride_a: int = 1) -> None:
+    """omnimem_redundancy_static: the Eq.7 redundancy s_v, s_a for callers that must not allocate device memory (a
+    serving engine whose pool already owns all of HBM, an operator body that is handed its tensors and nothing else).
+    No context and no workspace: the C call's intermediates live in a 4 MiB array inside the library, which is why
+    L * Hkv * (2 * cache_cap + max_chunk_v + max_chunk_a) may not exceed STATIC_SCRATCH_FLOATS and why calls that can
+    overlap on the GPU must be serialised by the caller.  This wrapper allocates nothing either: cache_x
+    [L,Hkv,cache_cap,D], chunk_x [L,Hkv,Nn,D] (None when Nn = 0) and the outputs s_m float32 [L,Hkv,cache_cap+max_chunk_m]
+    all come from the caller; work goes to torch's current stream of cache_x's device."""
+    lib = load_library()
+    L, Hkv, cache_cap, D = cache_x.shape
+    dtype = OMNIMEM_FP32 if cache_x.dtype == torch.float32 else OMNIMEM_BF16
+    with torch.cuda.device(cache_x.device):
+        rc = lib.omnimem_redundancy_static(dtype, L, Hkv, D, cache_cap, max_chunk_v, max_chunk_a, sim_stride_v,
+                                           sim_stride_a, _ptr(cache_x), _ptr(n_v), _ptr(n), _ptr(chunk_x), Nn_v, Nn_a,
+                                           _ptr(s_v), _ptr(s_a), _stream())
+    if rc != 0:
+        raise OmniMemError(f"omnimem_redundancy_static failed ({rc}): {lib.omnimem_strerror(rc).decode()}")
 
 
 @dataclass
