@@ -151,12 +151,15 @@ OMNIMEM_API const char* omnimem_last_cuda_error(const omnimem_ctx* ctx); /* cuda
  * KV head j / G, R5), and lse_out[l, j, i] = log sum_k exp(c <q_i, k_k>) (natural log) -- exactly the array
  * omnimem_chunk.lse takes, so that omnimem_compress_chunk on the same chunk skips score pass 1: the forward a model
  * runs anyway (Eq.1) makes Eq.6 a single pass over Q K^T.
- * y: DEVICE [L, Hq, Nn, D] of the context dtype (bf16: fp32 accumulation, P rounded to bf16 before P V, Y rounded once);
+ * y: DEVICE [L, Hq, Nn, D] of the context dtype (bf16: fp32 accumulation, P rounded to bf16 before P V, Y rounded once:
+ * |y - exact| <= 2^-7 sum_k p_k |v_k| element-wise, R32; fp32: 1e-5 of the same magnitude);
  * lse_out: DEVICE float [L, Hq, Nn].  Both required.  chunk->lse, ->h and ->modality are ignored (the mask follows the
  * storage order of the chunk rows, which is the temporal order in both chunk layouts).  bf16 with D = 128 runs on
  * tcgen05 (tensor memory accumulators for S and O, TMA-fed K / V ring); fp32 and D = 64 on a SIMT kernel.
  * Rows n[l] .. cache_cap of the cache buffers are never read into a result.  Nn = 0: nothing is written.
- * Errors: INVALID_ARG, CAPACITY (Nn_v > max_chunk_v, Nn_a > max_chunk_a), WORKSPACE_TOO_SMALL, CUDA_ERROR. */
+ * The forward uses no workspace: ws may be NULL and ws_bytes 0 (a model that only wants Y and the LSE need not allocate
+ * the compression workspace); whatever is passed is ignored.
+ * Errors: INVALID_ARG, CAPACITY (Nn_v > max_chunk_v, Nn_a > max_chunk_a), CUDA_ERROR. */
 OMNIMEM_API int omnimem_attend(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, void* y, float* lse_out,
                    void* ws, size_t ws_bytes, void* stream);
 

@@ -40,7 +40,10 @@ def _headers():
 
 
 def _want_stamp() -> dict:
-    srcs = [os.path.join(CSRC, s) for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
+    srcs = [os.path.join(CSRC, s) for s in SOURCES]
+    missing = [p for p in srcs if not os.path.exists(p)]
+    if missing:   # a dropped entry would only show up later as an unresolved symbol at link or load time
+        raise FileNotFoundError("sources listed in build.SOURCES are missing: " + ", ".join(missing))
     return {"flags": NVCC_FLAGS + LINK_FLAGS, "sources": {os.path.basename(p): _sha(p) for p in srcs},
             "headers": {os.path.basename(p): _sha(p) for p in _headers()}}
 

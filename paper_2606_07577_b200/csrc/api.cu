@@ -12,7 +12,7 @@ using namespace omnimem;
 namespace {
 
 struct WsLayout {
-  size_t lse, cosn, partials, a_v, a_a, la_v, la_a, s_v, s_a, psi_v, psi_a, stats, M_v, M_a, idx_v, idx_a, total;
+  size_t lse, cosn, partials, a_v, a_a, la_v, la_a, s_v, s_a, psi_v, psi_a, stats, M_v, M_a, idx_v, idx_a, rescue_items, total;
 };
 
 size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
@@ -40,6 +40,8 @@ WsLayout ws_layout(const omnimem_ctx* c) {
   w.M_a = take(L * sizeof(int32_t));
   w.idx_v = take(L * Hkv * (size_t)g.cache_cap * sizeof(int32_t));
   w.idx_a = take(L * Hkv * (size_t)g.cache_cap * sizeof(int32_t));
+  // count + list of pass 2's 256-key items that the log-domain rescue redoes (consumed inside the call that writes it)
+  w.rescue_items = take((1 + L * Hkv * (((size_t)g.cache_cap + 255) / 256 + (Nn + 255) / 256)) * sizeof(int32_t));
   w.total = off;
   return w;
 }
@@ -146,6 +148,7 @@ void fill_buffers(const omnimem_ctx* c, const omnimem_cache* src, const omnimem_
   b.psi_a = out ? out->psi_a : (float*)(ws + w.psi_a);
   b.la_v = (float*)(ws + w.la_v);
   b.la_a = (float*)(ws + w.la_a);
+  b.rescue_items = (int32_t*)(ws + w.rescue_items);
   b.cosn = (float*)(ws + w.cosn);
   b.partials = (double*)(ws + w.partials);
   b.stats = out ? out->stats : (double*)(ws + w.stats);
@@ -404,12 +407,12 @@ int omnimem_score(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chun
 
 int omnimem_attend(omnimem_ctx* ctx, const omnimem_cache* src, const omnimem_chunk* chunk, void* y, float* lse_out, void* ws,
                    size_t ws_bytes, void* stream) {
-  if (!ctx || !y || !lse_out || !ws) return OMNIMEM_INVALID_ARG;
+  (void)ws; (void)ws_bytes;   // the forward needs no scratch: NULL / 0 are accepted (the arguments stay for ABI stability)
+  if (!ctx || !y || !lse_out) return OMNIMEM_INVALID_ARG;
   int rc = check_cache(src);
   if (rc) return rc;
   rc = check_chunk(ctx, chunk, true);
   if (rc) return rc;
-  if (ws_bytes < ws_layout(ctx).total) return OMNIMEM_WORKSPACE_TOO_SMALL;
   begin_call(ctx);
   cudaStream_t st = (cudaStream_t)stream;
   StepParams p = make_params(ctx, chunk->Nn_v, chunk->Nn_a, src->n_v, src->n, nullptr);

@@ -40,10 +40,7 @@ constexpr int kOffKV = 2 * kTileB;                // [kSlots][32 KB]
 constexpr int kOffBar = kOffKV + kSlots * kTileB;
 constexpr size_t kSmem = 1024 + kOffBar + 256;   // barriers, item queue and the tensor-memory slot: 180 bytes
 constexpr uint32_t kColS = 0, kColO = 256;        // tensor-memory columns
-#ifndef OMNIMEM_ATT_POLY_NUM
-#define OMNIMEM_ATT_POLY_NUM 2
-#endif
-constexpr int kPolyNum = OMNIMEM_ATT_POLY_NUM, kPolyDen = 8;   // exponential pairs on the FMA-pipe polynomial, of every 8
+constexpr int kPolyNum = 2, kPolyDen = 8;   // exponential pairs on the FMA-pipe polynomial, of every 8
 
 // D = f32, A = B = bf16, N = 128, M = 128; bit 16: B is MN-major (the V tile: rows = keys, head_dim contiguous)
 constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kT >> 3) << 17) | ((uint32_t)(kT >> 4) << 24);
@@ -255,6 +252,11 @@ attend_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant
           __syncwarp();
         }
         tc_fence_after();
+        // ORDERING ASSUMPTION: S_s(j+1) below overwrites the tensor-memory columns that hold P_s(j), which the O_s(j) product
+        // issued just before it reads as its A operand -- two tcgen05.mma on DIFFERENT accumulators with a write-after-read
+        // between them, nothing waiting in between.  It relies on the tensor pipe executing one thread's tcgen05 stream in
+        // issue order (see the note at the stationary copies in score_tc.cu; the PTX ISA guarantees the order only for a
+        // shared accumulator).  Guarded by the multi-item attend tests (distinct P per tile, 1-5 persistent CTAs).
         if (j < w.nt[0]) issue_o(0, vslot, j);
         if (j + 1 < ntiles) { mbar_wait(bar_full + 8 * kslot, ph); tc_fence_after(); }   // K_{j+1}
         if (j + 1 < w.nt[0]) issue_s(0, kslot);

@@ -82,6 +82,7 @@ struct StepBuffers {
   float* row_entropy;    // or nullptr
   float *a_v, *a_a, *s_v, *s_a, *psi_v, *psi_a;
   float *la_v, *la_a;    // internal: log2 of the importance of the keys whose fp32 sum is below 2^-100 (R31), [L,Hkv,seg_cap_m]
+  int32_t* rescue_items; // tcgen05 path: [1 + items of pass 2] count + list of the items redone in the log domain (R31)
   float* cosn;           // [L,Hkv,seg_cap_v+seg_cap_a]: cos(x_t, x_{t+sigma})
   double* partials;      // [L][2][nblk][3]
   double* stats;         // [L,8]
@@ -126,6 +127,7 @@ cudaError_t launch_attend_tc(const omnimem_ctx* ctx, const StepParams& p, const 
 cudaError_t launch_attend_simt(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, void* y, float* lse_nat,
                                cudaStream_t st, int* launches);
 cudaError_t launch_colsum_rescue(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
+cudaError_t launch_colsum_rescue_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_finalize(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches);
 cudaError_t launch_allocate(const omnimem_ctx* ctx, const StepParams& p, const double* stats, const int32_t* layer_budget,

@@ -337,17 +337,20 @@ cudaError_t launch_colsum_simt(const omnimem_ctx* ctx, const StepParams& p, cons
 
 namespace omnimem {
 
-// tcgen05 path: lse_arr = the internal NEGATED log2-domain LSE (row stride padded to 128); SIMT path: the natural-log LSE.
+// SIMT path: per-key recompute against the natural-log LSE.  tcgen05 path: launch_colsum_rescue_tc (score_tc.cu).
 cudaError_t launch_colsum_rescue(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st,
                                  int* launches) {
   if (p.Nn == 0) return cudaSuccess;     // no queries: a = 0 everywhere by definition, psi = 0^lambda (1 - s)
+  // tensor-core path: the flagged 256-key items go through the scoring kernel once more (bounded by one more pass 2); the
+  // per-key kernel below costs a flagged key as much as the SIMT pass 2 does, which is the right bound only on the SIMT path
+  if (ctx->use_tc) return launch_colsum_rescue_tc(ctx, p, b, st, launches);
   const int groups = (p.cache_cap + p.Nn + 31) / 32;
   const long long items = (long long)p.L * p.Hkv * groups;
   const unsigned grid = (unsigned)((items + 3) / 4);
   const size_t smem = 4 * p.D * sizeof(float);
-  const float* lse_arr = ctx->use_tc ? b.lse2 : b.lse;
-  const int stride = ctx->use_tc ? (p.Nn + 127) / 128 * 128 : p.Nn;
-  const float coef = ctx->use_tc ? 1.f : -1.4426950408889634f;
+  const float* lse_arr = b.lse;          // the natural-log LSE of the SIMT passes
+  const int stride = p.Nn;
+  const float coef = -1.4426950408889634f;
   ++*launches;
   if (ctx->cfg.dtype == OMNIMEM_FP32)
     colsum_rescue_kernel<float><<<grid, 128, smem, st>>>(p, (const float*)b.cacheK, (const float*)b.chunkK, (const float*)b.Q,

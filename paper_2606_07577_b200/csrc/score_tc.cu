@@ -5,6 +5,10 @@
 //                        accumulator, keeps an online max / sum and writes lse2 = log2 sum_k 2^(c2 s_k).
 //   pass 2 (kPass == 2)  S^T = K Q^T, M = 128 keys per sub-tile: each thread owns one KEY row, the sum over
 //                        queries is thread-local: a_k = sum_{g,i} 2^(c2 s - lse2_i).  No atomics, no shuffles.
+//   rescue (kPass == 3) pass 2's tiles once more, in the LOG domain, for the items (256 keys of one head and layer) that hold
+//                        a key whose fp32 sum came out below 2^-100 (R31): each thread keeps a running maximum
+//                        with its sum, la_k = log2 sum_{g,i} 2^(c2 s - lse2_i).  The items come from a device-built list, so
+//                        the cost is bounded by one more pass 2 however many keys are flagged, and is ~0 when none is.
 // Both kernels are PERSISTENT: one CTA per SM (cfg.score_ctas overrides the count) draws work items (256 stationary rows
 // of one head and layer x their whole streamed sequence) from a device counter; the TMA stage ring, the accumulator ring,
 // the lse ring and all their barrier phases run on across items, and the producer warp prefetches the next item's tiles
@@ -47,20 +51,11 @@ constexpr int kQueue = 2;           // work items announced ahead by the produce
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + kOffBars + 512 /*barriers + tmem slot*/;
 
 constexpr int kKBlockBytes = kTile * 128;   // one 64-element K-block of a streamed tile (16 KB)
-#ifndef OMNIMEM_LAZY_MAX
-#define OMNIMEM_LAZY_MAX 1
-#endif
-constexpr bool kLazyMax = OMNIMEM_LAZY_MAX != 0;   // pass 1: running reference instead of a per-tile maximum (see the loop)
+constexpr bool kLazyMax = true;   // pass 1: running reference instead of a per-tile maximum (see the loop)
 
-#ifndef OMNIMEM_POLY_NUM
-#define OMNIMEM_POLY_NUM 2
-#endif
-#ifndef OMNIMEM_POLY_DEN
-#define OMNIMEM_POLY_DEN 8
-#endif
 // share of the exponential PAIRS of a row that run as the fp32x2 polynomial on the FMA pipe instead of on the MUFU
 // (tc_ptx.cuh; measured optimum of both scoring passes under the 1000 W cap: 2 of 8, degree 3)
-constexpr int kPolyNum = OMNIMEM_POLY_NUM, kPolyDen = OMNIMEM_POLY_DEN;
+constexpr int kPolyNum = 2, kPolyDen = 8;
 __device__ __forceinline__ constexpr bool pair_is_poly(int pi) { return pair_is_poly_t<kPolyNum, kPolyDen>(pi); }
 __device__ __forceinline__ uint64_t ex2_pair(uint64_t X, int pi) { return ex2_pair_t<kPolyNum, kPolyDen>(X, pi); }
 
@@ -79,7 +74,14 @@ struct TcArgs {
   // persistent CTAs: work item = (x, y, z) of the nx * ny * nz item grid, x fastest; handed out through *counter
   int nx, ny, n_items;
   int* counter;        // zeroed by the launcher
+  // rescue (kPass == 3): the items to work on are item_list[0 .. *item_count) (device data, written by rescue_items_kernel)
+  const int* item_list;
+  const int* item_count;
+  float* la_v;         // rescue outputs: log2 of the importance, [L, Hkv, seg_cap_m]
+  float* la_a;
 };
+
+constexpr float kTinyImportance = 7.888609052210118e-31f;   // 2^-100: below it the fp32 column sum is not trusted (R31)
 
 // What one CTA works on, computed identically by every role.
 struct Work {
@@ -103,6 +105,7 @@ struct Work {
 template <int kPass>
 __device__ __forceinline__ bool make_work(const TcArgs& a, Work& w, int item) {   // item: index in the (x, y, z) item grid
   const StepParams& p = a.p;
+  if (kPass == 3) item = uniform(a.item_list[item]);   // position in the list of flagged items -> pass 2's item index
   int bx = item % a.nx;
   const int yz = item / a.nx, by = yz % a.ny;
   w.l = yz / a.ny;
@@ -228,6 +231,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
                 const __grid_constant__ CUtensorMap mapKn, const TcArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const StepParams& p = a.p;
+  const int n_items = kPass == 3 ? uniform(*a.item_count) : a.n_items;
 
   // 1024-byte alignment (128B swizzle) computed on the 32-bit shared-window address: the window offset of the dynamic
   // array is a link-time constant, so every barrier / stage address below folds into an immediate
@@ -292,10 +296,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
       }
       item = uniform(item);
       if (++pq == kQueue) { pq = 0; pqph ^= 1; }
-      if (item >= a.n_items) break;
+      if (item >= n_items) break;
       Work w;
       if (!make_work<kPass>(a, w, item)) continue;
-      int it = kPass == 2 ? w.seq0 : 0, g = 0;   // pass 2: query tile / group member of tile j, kept incrementally
+      int it = kPass != 1 ? w.seq0 : 0, g = 0;   // pass 2: query tile / group member of tile j, kept incrementally
       stage = uniform(stage); sph = uniform(sph); slot = uniform(slot);   // see the epilogue
       // the stationary sub-tiles go through the same ring: the MMA warp copies them on into tensor memory (tcgen05.cp).
       // Rows past the end of the tensor are zero-filled by the TMA unit; rows n .. cache_cap of a cache tile are stale,
@@ -329,7 +333,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         }
         if (elect_one()) {
           mbar_expect_tx(bar_full + 8 * stage, kTileBytes);
-          if (kPass == 2) {
+          if (kPass != 1) {
             // lse2 of these 128 queries: its own ring + barrier, slot = (streamed tiles so far) % 16.  The slot was last
             // read 16 streamed tiles ago; this load is issued only after the ring entry kStages back (a streamed tile at
             // most kStages + 2 tiles back, the stationary tiles of an item boundary included) was consumed by its MMAs,
@@ -352,14 +356,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     int stage = 0, sph = 0;
     for (;;) {
       const int item = next_item();
-      if (item >= a.n_items) break;
+      if (item >= n_items) break;
       Work w;
       if (!make_work<kPass>(a, w, item)) continue;
-      int it = kPass == 2 ? w.seq0 : 0;
+      int it = kPass != 1 ? w.seq0 : 0;
       buf = uniform(buf); ph = uniform(ph); stage = uniform(stage); sph = uniform(sph);   // see the epilogue
       // stationary sub-tiles: shared memory -> tensor memory columns kTmemA + 64 s (lane = row, word c = elements 2c,
       // 2c+1: the A-operand layout of a TS-mode tcgen05.mma), 8 columns per K16 step.  The copies run in issue order with
       // the MMAs: after the previous item's last MMAs (which read these columns), before this item's first.
+      // ORDERING ASSUMPTION (write-after-read on the A columns): nothing waits between the previous item's last TS-mode
+      // MMAs and these copies.  The PTX ISA states that tcgen05.cp -> tcgen05.mma and tcgen05.mma -> tcgen05.mma issued by
+      // one thread execute in issue order; for tcgen05.mma -> tcgen05.cp it makes no such statement.  This kernel relies on
+      // the tensor pipe executing one thread's tcgen05.cp / .mma stream in order (what sm_100 does: block-scaled GEMM
+      // mainloops in the vendor's template library refill their scale-factor columns with tcgen05.cp behind the MMAs
+      // that read them in the same way).  Regression guard: test_persistent_ctas_walk_several_items and the rescue test
+      // with 3 CTAs give every CTA many consecutive items with distinct stationary tiles; a reordering would corrupt the
+      // second item's rows.  If a future part relaxes the order: commit the item's last MMA to a barrier of its own and
+      // wait on it here before the first copy (the stage-full wait above hides most of that latency).
       for (int s = 0; s < 2; ++s) {
         if (!w.validp[s]) continue;
         mbar_wait(bar_full + 8 * stage, sph);
@@ -401,7 +414,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         if (elect_one()) tc_commit(bar_empty + 8 * stage);
         __syncwarp();
         if (++stage == kStages) { stage = 0; sph ^= 1; }
-        if (kPass == 2 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
+        if (kPass != 1 && ++it == w.seq0 + w.tiles_per_g) it = w.seq0;
       }
     }
   }
@@ -425,7 +438,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
     int mpar = 0;         // merge buffer of this item (double-buffered: the partner reads while the next item's halves write)
     for (;;) {
     const int item = next_item();
-    if (item >= a.n_items) break;
+    if (item >= n_items) break;
     Work w;
     if (!make_work<kPass>(a, w, item)) continue;
     if (!w.sub_valid[s]) {
@@ -646,7 +659,34 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
             acc23 = add2z(acc23, ex2_pair(x3, 4 * e4 + 3));
           }
         };
-        if (w.sub_valid[0] && w.sub_valid[1] && !(p.causal && w.a_chunk)) {
+        // rescue: running reference mx and sum zl of 2^(x - mx) over this thread's columns, x = c2 s - lse2.  Masked columns
+        // drop out, and so do weights below 2^-1074: fp64, the oracle's type, ends there (its psi jumps to 0 at that point).
+        [[maybe_unused]] float mx = -1e30f, zl = 0.f;
+        [[maybe_unused]] auto log_update = [&](const uint32_t (&v0)[32], const uint32_t (&v1)[32], uint32_t l_addr, int first) {
+          float x[kHalf];
+#pragma unroll
+          for (int e4 = 0; e4 < 8; ++e4) {
+            const float4 la = lds128(l_addr + e4 * 16), lb = lds128(l_addr + 128 + e4 * 16);
+            const float le[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const float xa = fmaf(__uint_as_float(v0[4 * e4 + u]), c2, le[u]);
+              const float xb = fmaf(__uint_as_float(v1[4 * e4 + u]), c2, le[4 + u]);
+              x[4 * e4 + u] = (4 * e4 + u >= first && xa >= -1074.f) ? xa : -INFINITY;
+              x[32 + 4 * e4 + u] = (32 + 4 * e4 + u >= first && xb >= -1074.f) ? xb : -INFINITY;
+            }
+          }
+          float tm[4] = {x[0], x[1], x[2], x[3]};
+#pragma unroll
+          for (int e = 4; e < kHalf; ++e) tm[e & 3] = fmaxf(tm[e & 3], x[e]);
+          const float m_new = fmaxf(mx, fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3])));
+          float zs[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int e = 0; e < kHalf; ++e) zs[e & 3] += ex2(x[e] - m_new);
+          zl = fmaf(zl, ex2(mx - m_new), (zs[0] + zs[1]) + (zs[2] + zs[3]));
+          mx = m_new;
+        };
+        if (kPass == 2 && w.sub_valid[0] && w.sub_valid[1] && !(p.causal && w.a_chunk)) {
           const SteadyState st = colsum_steady(w.ntiles, s, half, jt, t_col, c2, buf, ph, acc01, acc23);
           buf = st.buf; ph = st.ph; acc01 = st.acc01; acc23 = st.acc23;
         } else {
@@ -671,7 +711,9 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           // one uniform register for the whole address (taken before the per-thread branch below): left to itself ptxas
           // keeps it as a sum of two uniform parts and materialises a vector copy of one of them for each of the 16 loads
           const uint32_t l_addr = (uint32_t)uniform((int)(sLse + (uint32_t)(slot * kTile + col0) * 4));
-          if (first <= 0) {
+          if constexpr (kPass == 3) {
+            log_update(v0, v1, l_addr, first);
+          } else if (first <= 0) {
             col_update(v0, v1, l_addr);
           } else {
 #pragma unroll
@@ -692,7 +734,10 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
         unpack2(acc01, q0, q1);
         unpack2(acc23, q2, q3);
         const float part = ((acc[0] + acc[1]) + (acc[2] + acc[3])) + ((q0 + q1) + (q2 + q3));
-        if (half == 1) sMg[s * kTile + r].x = part;
+        if (half == 1) {
+          if constexpr (kPass == 3) sMg[s * kTile + r] = make_float4(mx, zl, 0.f, 0.f);
+          else sMg[s * kTile + r].x = part;
+        }
         named_bar_sync(1 + s, 256);
         const int n_v = p.n_v[w.l], n = p.n[w.l];
         const bool valid = w.a_chunk ? krow < p.Nn : krow < n;
@@ -700,7 +745,19 @@ score_tc_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant_
           int m, t;
           if (w.a_chunk) chunk_row_to_seg(p, n_v, n, krow, m, t); else cache_row_to_seg(n_v, krow, m, t);
           float* out = m == 0 ? a.a_v + (long long)w.lhA * p.seg_cap_v : a.a_a + (long long)w.lhA * p.seg_cap_a;
-          out[t] = part + sMg[s * kTile + r].x;
+          if constexpr (kPass == 3) {
+            // only the keys pass 2 could not hold are replaced; finalize reads la for exactly those
+            if (!(out[t] >= kTinyImportance)) {
+              const float4 o = sMg[s * kTile + r];
+              const float M = fmaxf(mx, o.x);
+              const float Z = zl * ex2(mx - M) + o.y * ex2(o.x - M);
+              const float la = Z > 0.f ? M + log2f(Z) : -INFINITY;
+              (m == 0 ? a.la_v + (long long)w.lhA * p.seg_cap_v : a.la_a + (long long)w.lhA * p.seg_cap_a)[t] = la;
+              out[t] = exp2f(la);   // what fp32 can hold of it (usually 0)
+            }
+          } else {
+            out[t] = part + sMg[s * kTile + r].x;
+          }
         }
         jt = (jt + w.ntiles) & (2 * kLseSlots - 1);
       }
@@ -723,6 +780,28 @@ __global__ void lse_to_log2_kernel(const float* __restrict__ lse_nat, float* __r
   const int i = (int)(idx % stride);
   const long long r = idx / stride;
   lse2[idx] = i < Nn ? -lse_nat[r * Nn + i] * 1.4426950408889634f : -INFINITY;
+}
+
+// Rescue, step 1: which of pass 2's items (256 stationary key rows of one (layer, KV head); same numbering as its item
+// grid) hold a key that exists and whose fp32 column sum is below 2^-100.  One block per item, one thread per key row;
+// flagged items are appended to `list` (order is irrelevant: every item's results are its own).
+__global__ void __launch_bounds__(2 * kTile) rescue_items_kernel(const TcArgs a, int* __restrict__ list, int* __restrict__ count) {
+  const StepParams& p = a.p;
+  const int item = blockIdx.x;
+  const int bx = item % a.nx, yz = item / a.nx, h = yz % a.ny, l = yz / a.ny;
+  bool flag = false;
+  if (!layer_skips_scoring(p, l)) {
+    const int n_v = p.n_v[l], n = p.n[l];
+    const bool in_chunk = bx >= a.n_cache_pairs;
+    const int krow = (in_chunk ? bx - a.n_cache_pairs : bx) * 2 * kTile + threadIdx.x;
+    if (krow < (in_chunk ? p.Nn : n)) {
+      int m, t;
+      if (in_chunk) chunk_row_to_seg(p, n_v, n, krow, m, t); else cache_row_to_seg(n_v, krow, m, t);
+      const long long lh = (long long)l * p.Hkv + h;
+      flag = !((m == 0 ? a.a_v + lh * p.seg_cap_v : a.a_a + lh * p.seg_cap_a)[t] >= kTinyImportance);
+    }
+  }
+  if (__syncthreads_or(flag) && threadIdx.x == 0) list[atomicAdd(count, 1)] = item;
 }
 
 // ---- host side -------------------------------------------------------------------------------------------------
@@ -827,6 +906,32 @@ cudaError_t launch_colsum_tc(const omnimem_ctx* ctx, const StepParams& p, const 
   dim3 grid(a.n_cache_pairs + (p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hkv, p.L);
   ++*launches;
   return launch_score(ctx, score_tc_kernel<2, false>, grid, 1, st, m, a);
+}
+
+// Eq.6 below fp32's range on the tensor-core path (R31): flag the items, then redo exactly those in the log domain.
+// rescue_items: [1 + items] ints of scratch (count, then the list).  Worst case (every item flagged) = one more pass over
+// Q K^T on the tensor cores; nothing flagged = one sweep over a and a kernel whose CTAs find an empty list.
+cudaError_t launch_colsum_rescue_tc(const omnimem_ctx* ctx, const StepParams& p, const StepBuffers& b, cudaStream_t st, int* launches) {
+  if (p.Nn == 0) return cudaSuccess;
+  Maps m;
+  cudaError_t e = make_maps(ctx, p, b, &m);
+  if (e != cudaSuccess) return e;
+  TcArgs a = make_args(p, b);
+  a.la_v = b.la_v;
+  a.la_a = b.la_a;
+  const dim3 grid(a.n_cache_pairs + (p.Nn + 2 * kTile - 1) / (2 * kTile), p.Hkv, p.L);   // pass 2's item grid
+  a.nx = (int)grid.x;
+  a.ny = (int)grid.y;
+  a.n_items = (int)(grid.x * grid.y * grid.z);
+  int* count = b.rescue_items;
+  int* list = b.rescue_items + 1;
+  if ((e = cudaMemsetAsync(count, 0, sizeof(int), st)) != cudaSuccess) return e;
+  rescue_items_kernel<<<a.n_items, 2 * kTile, 0, st>>>(a, list, count);
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  a.item_list = list;
+  a.item_count = count;
+  *launches += 2;
+  return launch_score(ctx, score_tc_kernel<3, false>, grid, 3, st, m, a);
 }
 
 }  // namespace omnimem

@@ -17,14 +17,14 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Blocks until the phase of `bar` with the given parity has completed.  One try_wait per trip: the instruction itself parks
+// the thread for a hardware-chosen time before it reports "not yet", so the C++ loop around it does not spin hot.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");  // suspend-time hint: sleep, do not spin
+  uint32_t done;
+  do {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
   asm volatile(
@@ -140,16 +140,13 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
 // Cody-Waite split + minimax polynomial on [-0.5, 0.5], two lanes per instruction (fp32x2).  The MUFU ex2 pipe
 // (16 / clk / SM) limits every softmax epilogue here (ncu: xu pipe 82-89 %), so a share of the exponential PAIRS of a row
 // is evaluated with this instead.  Degree 3: max relative error 7.5e-5, equi-oscillating in the fractional part (the error
-// of a sum of many terms averages out); degree 4: 2.7e-6.  Coefficients fitted for this repository (Lawson iteration on
+// of a sum of many terms averages out).  Coefficients fitted for this repository (Lawson iteration on
 // the relative error).
 __device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
   uint64_t d;
   asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
 }
-#ifndef OMNIMEM_POLY_DEG
-#define OMNIMEM_POLY_DEG 3
-#endif
 __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
   float x0, x1;
   unpack2(X, x0, x1);
@@ -159,16 +156,9 @@ __device__ __forceinline__ uint64_t ex2_poly2(uint64_t X) {
   const uint64_t MG = pack2(12582912.f, 12582912.f);  // 1.5 * 2^23: the low mantissa bits of T hold round(x)
   const uint64_t T = add2(X, MG);
   const uint64_t F = sub2(X, sub2(T, MG));
-#if OMNIMEM_POLY_DEG == 4
-  uint64_t Q = fma2(pack2(0.009570102207362652f, 0.009570102207362652f), F, pack2(0.05591785907745361f, 0.05591785907745361f));
-  Q = fma2(Q, F, pack2(0.240247443318367f, 0.240247443318367f));
-  Q = fma2(Q, F, pack2(0.6931217908859253f, 0.6931217908859253f));
-  Q = fma2(Q, F, pack2(0.9999992847442627f, 0.9999992847442627f));
-#else
   uint64_t Q = fma2(pack2(0.0551716685295105f, 0.0551716685295105f), F, pack2(0.2426111251115799f, 0.2426111251115799f));
   Q = fma2(Q, F, pack2(0.6932609677314758f, 0.6932609677314758f));
   Q = fma2(Q, F, pack2(0.9999280571937561f, 0.9999280571937561f));
-#endif
   float q0, q1, t0, t1;
   unpack2(Q, q0, q1);
   unpack2(T, t0, t1);

@@ -136,6 +136,25 @@ def test_attend_edge_shapes():
     check_attend(SMALL3.replace(n_v=700, n_a=100, Nn_v=600, Nn_a=170, cache_cap=1700, budget=1000, Hq=14, Hkv=2))  # G = 7
 
 
+def test_attend_needs_no_workspace():
+    """omnimem_attend uses no scratch: NULL / 0 for ws is accepted (a model that only wants the forward and its LSE need not
+    allocate the compression workspace) and gives bit-identical results to a call that passes one."""
+    import ctypes as C
+    for wl, kw in ((SMALL2, {}), (I.CFG1, {})):                 # tcgen05 and SIMT forward
+        x = I.full_inputs(wl)
+        eng = engine_for(wl, **kw)
+        src, chunk = dev_objs(x, wl)
+        y0, lse0 = eng.attend(src, chunk)
+        y1, lse1 = torch.full_like(y0, float("nan")), torch.full_like(lse0, float("nan"))
+        cs, cc = src.c(), chunk.c()
+        rc = eng.lib.omnimem_attend(eng.ctx, C.byref(cs), C.byref(cc), C.c_void_p(y1.data_ptr()), C.c_void_p(lse1.data_ptr()),
+                                    None, 0, C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        torch.cuda.synchronize()
+        assert rc == 0
+        assert torch.equal(y0, y1) and torch.equal(lse0, lse1)
+        eng.close()
+
+
 def test_attend_ignores_rows_beyond_n():
     """Rows n .. cache_cap of the cache buffers may hold anything (stale rows, NaN bit patterns): masked key columns are
     selected away and the value rows of the ragged last cache tile are zeroed in shared memory before P V."""
@@ -205,10 +224,13 @@ def test_attend_full_size(wl, samples):
     torch.cuda.synchronize()
     assert float((sc.lse - lse).abs().max()) < 2 * 7.5e-5 + 1e-5
     G = wl.G
+    worst = 0.0
     for l, h in samples:
         Y_ref, lse_ref, absY = oracle_one_kv_head(wl, x, l, h)
-        compare_attend(wl, y[l:l + 1, h * G:(h + 1) * G].float().cpu().numpy(), lse[l:l + 1, h * G:(h + 1) * G].cpu().numpy(),
-                       Y_ref, lse_ref, absY, f"{wl.name} layer {l} kv head {h}")
+        worst = max(worst, compare_attend(wl, y[l:l + 1, h * G:(h + 1) * G].float().cpu().numpy(),
+                                          lse[l:l + 1, h * G:(h + 1) * G].cpu().numpy(), Y_ref, lse_ref, absY,
+                                          f"{wl.name} layer {l} kv head {h}"))
+    print(f"{wl.name}: worst |dY| / sum_k p_k |v_k| = {worst * Y_TOL[wl.dtype]:.3e} (bound {Y_TOL[wl.dtype]:.3e})")
     # the point of the row at full size: forward + one-pass compression keeps what the two-pass step keeps, on EVERY layer
     # (the two LSEs differ by up to 1.5e-4, i.e. psi by lambda x that = 3e-6 relative: only exact near-ties at the threshold
     # can flip, and rule (c) allows those)

@@ -81,3 +81,11 @@ def test_product_does_not_import_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2606_07577_b200" not in text and "from paper_2606_07577_b200" not in text
             assert "csrc" not in text.replace("paper_2606_07577_b200/csrc", "") or f.endswith(".c")
+
+
+def test_build_refuses_a_source_list_with_a_missing_file(monkeypatch):
+    """A SOURCES entry that is not on disk is an error at build time, not an unresolved symbol at load time."""
+    from paper_2606_07577_b200 import build
+    monkeypatch.setattr(build, "SOURCES", build.SOURCES + ["no_such_file.cu"])
+    with pytest.raises(FileNotFoundError, match="no_such_file.cu"):
+        build.build()

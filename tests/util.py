@@ -59,6 +59,7 @@ def compare_scores(wl, n_v, n, gpu: dict, orc: dict, tol: float, stats_tol=None)
 
 def kept_sets_rule_c(name, idx_gpu, idx_ref, M, psi_ref_seg, tol):
     """Rule (c): index sets identical except where the oracle's score is within tol of the M-th largest score."""
+    assert np.all(np.diff(idx_gpu[:M]) > 0), f"{name}: indices not ascending"      # the order is part of the contract
     g, r = set(idx_gpu[:M].tolist()), set(idx_ref[:M].tolist())
     diff = g ^ r
     if not diff:
@@ -68,7 +69,6 @@ def kept_sets_rule_c(name, idx_gpu, idx_ref, M, psi_ref_seg, tol):
     for t in diff:
         if abs(float(psi_ref_seg[t]) - tau) > tol * max(abs(tau), 1e-30):
             raise AssertionError(f"{name}: index {t} differs and psi {psi_ref_seg[t]!r} is not within {tol} of tau {tau!r}")
-    assert np.all(np.diff(idx_gpu[:M]) > 0), f"{name}: indices not ascending"
     return len(diff)
 
 
