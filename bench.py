@@ -5,7 +5,9 @@ A "step" is one `omnimem_compress_chunk` call: all five stages (score, AVBA budg
 layer of one synthetic chunk.  BASELINE.json's `metric` names no config, so the line of record is the LARGEST
 single-GPU config, configs[2] (8B-shaped, 253 TFLOP per step); the same run also times configs[1] (the
 Qwen2.5-Omni-7B-shaped step, object "cfg2", same keys) and the 60-chunk stream of configs[4] (object "stream":
-p50 / p99 per chunk, total ingest tok/s), so that the driver records all three.  `--config N` runs one config only.
+p50 / p99 per chunk, total ingest tok/s), configs[3] and configs[0] (objects "cfg4", "cfg1") and the worst case of the
+log-domain rescue (object "rescue_worst": config 2 with peaky logits, R31) and the step under an offline ragged
+per-layer table (object "ragged", NEXT-2), so that the driver records every config.  `--config N` runs one config only.  The defaults (--steps 20 --warmup 5) are the protocol the driver records with.
 `value` = KV tokens processed per second = Nk / t_step (Nk = cached + new rows per layer), whole job over N GPUs.
 Multi-GPU: the path does not shard in this repo (replicas only) -> N independent replicas,
 weak scaling, no data-path collective.
@@ -113,7 +115,8 @@ class ClockSampler:
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(self.samples), "power_w": float(np.median(self.power)) if self.power else None}
+                "samples": len(self.samples), "power_w": float(np.median(self.power)) if self.power else None,
+                "power_w_mean": float(np.mean(self.power)) if self.power else None}
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm
@@ -334,7 +337,14 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
     # P_TC = the measured BURST bf16 peak ("the stricter one"); the sustained figure is printed beside it
     t_roof = max(2 * work["f_pass"] / (peaks["tf_burst"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
     t_roof_sust = max(2 * work["f_pass"] / (peaks["tf_sust"] * 1e12), work["bytes"]["total"] / (peaks["hbm_gbs"] * 1e9))
-    traffic, traffic_src = ncu_traffic(wl.name, 2 if dom == "colsum" else 1)
+    traffic, traffic_src = ncu_traffic(wl.name, f"score_tc_kernel<{2 if dom == 'colsum' else 1}")
+    fwd_traffic, fwd_traffic_src = ncu_traffic(wl.name, "attend_tc_kernel")
+    # algorithmic bytes of one launch of the dominant kernel, counted live from this run's shapes: Q + K read once, the LSE
+    # written (pass 1) or read (pass 2), the column sums written (pass 2)
+    es = wl.elem_bytes
+    dom_bytes = (wl.L * wl.Hq * wl.Nn * wl.D * es + wl.L * wl.Hkv * work["Nk"] * wl.D * es + wl.L * wl.Hq * wl.Nn * 4 +
+                 (wl.L * wl.Hkv * work["Nk"] * 4 if dom == "colsum" else 0))
+    power = clocks.get("power_w_mean") if isinstance(clocks, dict) else None
     out = {
         "metric": "kv_tokens_per_s", "value": job_value(world, work["Nk"], t_step), "unit": "KV tok/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
@@ -345,8 +355,15 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
                    "l2": "inputs larger than L2 (Q+K+V per step >> 126 MB); no flush", "gen_s": round(t_gen, 1)},
         "clocks": clocks,
         "e2e": {"value": job_value(world, work["Nk"], t_e2e / args.steps), "unit": "KV tok/s", "ms_per_step": t_e2e / args.steps * 1e3,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "note": "omnimem_compress_chunk_host: the chunk (K, V, Q) is copied in from pinned host memory and the per-layer "
+                        "budgets M_v, M_a are read back; the compacted cache stays on the device by design (it is the next "
+                        "step's input), so d2h is not a read-back of the result rows"},
         "gpu_launches": launches,
+        "energy": None if not power else {
+            "board_w_mean": power, "j_per_step": power * t_step,
+            "j_per_scoring_pass": {k: power * stage_ms[k] / 1e3 for k in ("lse", "colsum") if k in stage_ms},
+            "note": "mean NVML board power over the timed loop x CUDA-event time (a whole-loop mean, not per-kernel metering)"},
         "stage_ms": stage_ms,
         "roofline": {"bound": "tensor", "kernel": f"score_tc_kernel<{2 if dom == 'colsum' else 1}> ({dom})",
                      "achieved": achieved, "peak": peaks["tf_burst"], "unit": "TFLOP/s", "frac": achieved / peaks["tf_burst"],
@@ -354,6 +371,9 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
                      "peak_burst": peaks["tf_burst"], "peak_sustained": peaks["tf_sust"],
                      "frac_of_sustained": achieved / peaks["tf_sust"], "frac_of_burst": achieved / peaks["tf_burst"],
                      "traffic": traffic, "traffic_source": traffic_src,
+                     "traffic_kind": "OFFLINE: DRAM bytes per launch from the committed ncu capture named in traffic_source "
+                                     "(another run of the same kernel and shapes), not measured by this run",
+                     "algorithmic_bytes_per_launch": dom_bytes,
                      "algorithmic_flops_per_launch": work["f_pass"], "exps_per_launch": work["exps_pass"]},
         "step_roofline": {"t_roof_ms": t_roof * 1e3, "frac_two_pass": t_roof / t_step,
                           "frac_two_pass_of_sustained": t_roof_sust / t_step,
@@ -379,7 +399,10 @@ def measure_config(args, wl: I.Workload, rank: int, local_rank: int, world: int,
                     "roofline": {"bound": "tensor", "kernel": "attend_tc_kernel", "achieved": f_fwd / t_fwd / 1e12, "unit": "TFLOP/s",
                                  "peak": peaks["tf_burst"], "frac": f_fwd / t_fwd / 1e12 / peaks["tf_burst"],
                                  "frac_of_sustained": f_fwd / t_fwd / 1e12 / peaks["tf_sust"], "algorithmic_flops_per_launch": f_fwd,
-                                 "traffic": None},
+                                 "traffic": fwd_traffic, "traffic_source": fwd_traffic_src,
+                                 "traffic_kind": "OFFLINE (committed ncu capture), not measured by this run",
+                                 "algorithmic_bytes_per_launch": 2 * wl.L * wl.Hq * wl.Nn * wl.D * es + 2 * wl.L * wl.Hkv * work["Nk"] * wl.D * es
+                                 + wl.L * wl.Hq * wl.Nn * 4},
                     "note": "omnimem_attend (Eq.1: Y and the row LSE) then omnimem_compress_chunk(lse=...): a model that runs this "
                             "forward anyway pays forward_plus_compress instead of forward + two-pass"}
     out["derived"] = {"ingest_tok_per_s": world * wl.Nn / t_step, "layer_entries_per_s": world * wl.L * work["Nk"] / t_step,
@@ -456,20 +479,127 @@ def measure_stream(args, wl: I.Workload, local_rank: int):
     }
 
 
-NCU_CAPTURES = {"cfg2_qwen25omni7b": "profiles/r02_score_tc_full_cfg2.csv",    # committed `ncu --set full` summaries
-                "cfg3_8b": "profiles/r02_score_tc_full_cfg3.csv"}
+# committed ncu summaries (profiles/r02_README.md, r03_README.md name the commands): (workload, kernel-name prefix) -> file
+def measure_ragged(args, wl: I.Workload, local_rank: int):
+    """NEXT-2 (Eq.13-14; "determined offline"): the step under an offline, non-uniform per-layer table.
+    Config 2's shape with cache buffers sized for B_max; the layers' queries get different scales so that the table is far
+    from uniform.  Three calibration steps (uniform budget, statistics accumulated on the device), the table
+    B^(l) = Softmax(C/T) x L x 16384 clamped to [8192, 24576], free-running steps until every layer holds B^(l) rows, then
+    the timed steps (ping-pong caches).  Flops are counted for the rows each layer actually holds."""
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    Bmin, Bmax = 8192, 24576
+    wl = wl.replace(cache_cap=Bmax)
+    L = wl.L
+    eng = OmniMem.for_workload(wl, device=str(dev), budget_min=Bmin, budget_max=Bmax)
+    x = I.full_inputs(wl)
+    x["Q"] = (x["Q"].float() * torch.linspace(0.5, 2.0, L).view(L, 1, 1, 1)).to(x["Q"].dtype)
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    dst = eng.new_cache()
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)   # the same chunk every step
+    B_uni = torch.full((L,), wl.budget, dtype=torch.int32, device=dev)
+    sc = eng.new_scores(wl.Nn)
+    acc = eng.new_calibration()
+    for _ in range(3):
+        eng.compress_chunk(src, chunk, B_uni, dst, out=sc)
+        eng.calibrate_accumulate(sc.stats, acc)
+        src, dst = dst, src
+    total = L * wl.budget
+    B_dev, _ = eng.calibrate_budgets(acc, total)
+    for _ in range(4):                                         # until n[l] = B^(l) on every layer
+        eng.compress_chunk(src, chunk, B_dev, dst)
+        src, dst = dst, src
+    torch.cuda.synchronize(dev)
+    B, n = B_dev.cpu().numpy().astype(np.int64), src.n.cpu().numpy().astype(np.int64)
+    steps = max(3, min(args.steps, 10))
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(steps):
+        eng.compress_chunk(src, chunk, B_dev, dst)
+        src, dst = dst, src
+    ev1.record()
+    torch.cuda.synchronize(dev)
+    t = ev0.elapsed_time(ev1) / 1e3 / steps
+    pairs = int((wl.Nn * n + wl.Nn * (wl.Nn + 1) // 2).sum())                # visible (q, k) pairs per query head, all layers
+    flops = 2 * 2.0 * wl.D * wl.Hq * pairs                                   # two scoring passes
+    peaks = measured_peaks()
+    eng.close()
+    return {"workload": wl.name, "ms_per_step": t * 1e3, "steps": steps, "kv_tok_per_s": float((n + wl.Nn).mean()) / t,
+            "table": {"min": int(B.min()), "max": int(B.max()), "sum": int(B.sum()), "budget_min": Bmin, "budget_max": Bmax,
+                      "distinct": int(len(set(B.tolist())))},
+            "rows_cached_steady": {"min": int(n.min()), "max": int(n.max()), "equal_to_table": bool((n == B).all())},
+            "flops_two_pass": flops, "tflops": flops / t / 1e12, "frac_of_burst": flops / t / 1e12 / peaks["tf_burst"],
+            "frac_of_sustained": flops / t / 1e12 / peaks["tf_sust"],
+            "hbm_rows": {"allocated_per_kv_head": int(L * Bmax), "needed_per_kv_head": int(B.sum()),
+                         "note": "the cache buffers are [L, Hkv, cache_cap, D] with one cache_cap >= B_max for every layer; "
+                                 "per-layer capacities (sum of B^(l) rows) are not built"},
+            "note": "config 2's shape under an offline Eq.13-14 table (per-layer query scales 0.5-2.0 make it non-uniform); "
+                    "steady state (every layer holds B^(l) rows); the same chunk is fed every step"}
 
 
-def ncu_traffic(workload: str, pass_no: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of score_tc_kernel<pass_no> from the committed ncu capture
-    of this workload (profiles/), read at run time.  Returns (bytes or None, source)."""
-    rel = NCU_CAPTURES.get(workload)
+def measure_rescue_worst(args, wl: I.Workload, local_rank: int):
+    """DESIGN.md R31, the cost cliff ADVICE r2 named: the softmax scale x 40 makes the logits so peaky that most keys get
+    less than 2^-100 from all queries together, so most of pass 2's 256-key items are redone in the log domain
+    (score_tc_kernel<3>).  Reports the step and its column-sum stage (pass 2 + rescue) next to the same shapes with the
+    default scale, and the share of keys that were flagged."""
+    from paper_2606_07577_b200.omnimem import Cache, Chunk, OmniMem
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    x = I.full_inputs(wl)
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+    B = torch.full((wl.L,), wl.budget, dtype=torch.int32, device=dev)
+    steps = max(3, min(args.steps, 10))
+    res = {}
+    for name, scale in (("default_scale", 0.0), ("peaky", 40.0 / float(np.sqrt(wl.D)))):
+        eng = OmniMem.for_workload(wl, device=str(dev), softmax_scale=scale)
+        dst = eng.new_cache()
+        sc = eng.new_scores(wl.Nn)
+        eng.set_profiling(True)
+        for _ in range(3):
+            eng.compress_chunk(src, chunk, B, dst, out=sc)
+        torch.cuda.synchronize(dev)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        colsum = 0.0
+        ev0.record()
+        for _ in range(steps):
+            eng.compress_chunk(src, chunk, B, dst, out=sc)
+            colsum += eng.stage_ms()[0]["colsum"]
+        ev1.record()
+        torch.cuda.synchronize(dev)
+        Kv, Ka = wl.n_v + wl.Nn_v, wl.n_a + wl.Nn_a
+        tiny = int((sc.a_v[:, :, :Kv] < 2.0 ** -100).sum()) + int((sc.a_a[:, :, :Ka] < 2.0 ** -100).sum())
+        res[name] = {"ms_per_step": ev0.elapsed_time(ev1) / steps, "colsum_stage_ms": colsum / steps,
+                     "keys_below_2^-100": tiny / float(wl.L * wl.Hkv * (Kv + Ka))}
+        eng.close()
+        del dst, sc
+    res["workload"] = wl.name
+    res["steps"] = steps
+    res["note"] = ("peaky = softmax scale x 40: the flagged 256-key items go through the tensor-core scoring kernel once more in the "
+                   "log domain (at about twice the cost of a pass-2 tile), so the column-sum stage is bounded by about three times its "
+                   "ordinary time however many keys are flagged")
+    return res
+
+
+NCU_CAPTURES = {("cfg2_qwen25omni7b", "score_tc_kernel"): "profiles/r02_score_tc_full_cfg2.csv",
+                ("cfg3_8b", "score_tc_kernel"): "profiles/r03_score_tc_metrics_cfg3.csv",
+                ("cfg4_4b_tight", "score_tc_kernel"): "profiles/r03_score_tc_metrics_cfg4.csv",
+                ("cfg2_qwen25omni7b", "attend_tc_kernel"): "profiles/r02_attend_tc_full_cfg2.csv"}
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel whose name starts with `kernel` (e.g.
+    "score_tc_kernel<2") from the committed ncu capture of this workload (profiles/).  An OFFLINE figure: it comes from an
+    earlier profiled run of the same kernel on the same shapes, not from the run being reported (the line says so).
+    Returns (bytes or None, source)."""
+    rel = NCU_CAPTURES.get((workload, kernel.split("<")[0]))
     path = os.path.join(ROOT, rel) if rel else None
     if not path or not os.path.exists(path):
         return None, "no ncu --set full capture committed for this workload"
     import csv
     rows = list(csv.reader(open(path)))
-    col = next((i for i, c in enumerate(rows[0]) if f"score_tc_kernel<{pass_no}" in c), None)
+    col = next((i for i, c in enumerate(rows[0]) if kernel in c), None)
     if col is None:
         return None, f"{rel}: kernel column not found"
     unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
@@ -486,10 +616,11 @@ def ncu_traffic(workload: str, pass_no: int):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=20)      # the driver's protocol: --steps 20 --warmup 5
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=0,
-                    help="BASELINE.json configs[i-1]; 0 (default) = the line of record: config 3 (largest) + objects cfg2 and stream (config 5)")
+                    help="BASELINE.json configs[i-1]; 0 (default) = the line of record: config 3 (largest) + objects cfg2, cfg4, cfg1, "
+                         "stream (config 5) and rescue_worst")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunks", type=int, default=0, help="config 5 only: chunks in the stream (default: the config's 60)")
@@ -513,9 +644,16 @@ def main():
             # the other two workloads BASELINE.json singles out, in the same line so that the driver records them
             torch.cuda.empty_cache()
             cfg2 = measure_config(args, I.CFG2, rank, local_rank, world, cpu_baseline=False)
+            torch.cuda.empty_cache()
+            cfg4 = measure_config(args, I.CFG4, rank, local_rank, world, cpu_baseline=False)
+            cfg1 = measure_config(args, I.CFG1, rank, local_rank, world, cpu_baseline=False)
             if rank == 0:
-                out["cfg2"] = cfg2
+                out["cfg2"], out["cfg4"], out["cfg1"] = cfg2, cfg4, cfg1
             if world == 1:
+                torch.cuda.empty_cache()
+                out["rescue_worst"] = measure_rescue_worst(args, I.CFG2, local_rank)
+                torch.cuda.empty_cache()
+                out["ragged"] = measure_ragged(args, I.CFG2, local_rank)
                 torch.cuda.empty_cache()
                 st = measure_stream(args, I.CFG5, local_rank)
                 out["stream"] = {"workload": I.CFG5.name, "chunks": st["steps"], "ms_per_step_mean": st["ms_per_step"],

@@ -76,11 +76,11 @@ def test_bench_accounting_matches_the_survey_tables():
         assert abs(w["pairs"] - pairs) < 0.01e6 * 1.5 and abs(2 * w["f_pass"] - flops) < 0.01e12 and abs(w["bytes"]["total"] - nbytes) < 0.01e9
         assert w["exps_pass"] == w["pairs"] * wl.Hq * wl.L and w["Nk"] == wl.n_v + wl.n_a + wl.Nn
     # DRAM traffic per launch of the two scoring passes, read from profiles/: within 5 % of the algorithmic Q + K bytes
-    for name, cfg in (("cfg2_qwen25omni7b", 2), ("cfg3_8b", 3)):
+    for name, cfg in (("cfg2_qwen25omni7b", 2), ("cfg3_8b", 3), ("cfg4_4b_tight", 4)):
         wl = I.CONFIGS[cfg]
         qk = (wl.L * wl.Hq * wl.Nn + wl.L * wl.Hkv * (wl.n_v + wl.n_a + wl.Nn)) * wl.D * 2
         for pass_no in (1, 2):
-            traffic, src = bench.ncu_traffic(name, pass_no)
+            traffic, src = bench.ncu_traffic(name, f"score_tc_kernel<{pass_no}")
             assert traffic is not None and src.startswith("profiles/"), src
             assert 1.0 <= traffic / qk < 1.05, (name, pass_no, traffic / qk)
-    assert bench.ncu_traffic("cfg4_4b_tight", 1)[0] is None      # no capture committed: null, with the reason as source
+    assert bench.ncu_traffic("cfg1_tiny_fp32", "score_tc_kernel<1")[0] is None     # no capture committed: null, with the reason as source

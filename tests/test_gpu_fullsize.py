@@ -21,7 +21,8 @@ pytestmark = pytest.mark.gpu
 
 
 def oracle_layer(wl, x, i, n_v, n, cacheK=None, cacheV=None):
-    """The oracle on layer slot `i` of the stacked inputs (L = 1).  cacheK / cacheV override x's cache (teacher forcing)."""
+    """The oracle on layer slot `i` of the stacked inputs (L = 1).  cacheK / cacheV override x's cache (teacher forcing).
+    wl.budget is THIS layer's total B^(l)."""
     p = ref_params(wl, 1)
     cK = x["cacheK"][i:i + 1] if cacheK is None else cacheK
     cV = x["cacheV"][i:i + 1] if cacheV is None else cacheV
@@ -35,19 +36,21 @@ def gpu_layer_scores(sc, l):
                 stats=f(sc.stats), lse=f(sc.lse))
 
 
-def check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n):
+def check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n, budgets=None, scored=None):
     """Properties of the fused step's outputs that need no oracle; every layer, every head; computed with torch ops on
-    the device (an independent gather, not the library's)."""
+    the device (an independent gather, not the library's).  budgets: per-layer totals B^(l) (default: wl.budget for all);
+    scored: per-layer flags, False where the step had nothing to evict and may have skipped scoring (default: all True)."""
     L, tol = wl.L, TOL[wl.dtype]
     Kv, Ka = seg_lens(wl, n_v, n)
     mv, ma = M_v.cpu().numpy(), M_a.cpu().numpy()
-    assert np.array_equal(mv + ma, np.minimum(wl.budget, Kv + Ka)), "budgets do not sum to B"
+    assert np.array_equal(mv + ma, np.minimum(wl.budget if budgets is None else budgets, Kv + Ka)), "budgets do not sum to B"
     assert np.all(mv <= Kv) and np.all(ma <= Ka) and np.all(mv >= 0) and np.all(ma >= 0)
     assert np.array_equal(dst.n_v.cpu().numpy(), mv) and np.array_equal(dst.n.cpu().numpy(), mv + ma)
     for l in range(L):
-        tot = sc.a_v[l, :, :Kv[l]].double().sum(-1) + sc.a_a[l, :, :Ka[l]].double().sum(-1)
-        np.testing.assert_allclose(tot.cpu().numpy(), wl.G * wl.Nn, rtol=10 * tol)
-        assert bool((sc.a_v[l, :, :Kv[l]] >= 0).all()) and bool((sc.psi_v[l, :, :Kv[l]] >= 0).all())
+        if scored is None or scored[l]:
+            tot = sc.a_v[l, :, :Kv[l]].double().sum(-1) + sc.a_a[l, :, :Ka[l]].double().sum(-1)
+            np.testing.assert_allclose(tot.cpu().numpy(), wl.G * wl.Nn, rtol=10 * tol)
+            assert bool((sc.a_v[l, :, :Kv[l]] >= 0).all()) and bool((sc.psi_v[l, :, :Kv[l]] >= 0).all())
         for idx, M, K, off_c, cnt_c, off_n in ((idx_v, mv[l], Kv[l], 0, n_v[l], 0),
                                                (idx_a, ma[l], Ka[l], n_v[l], n[l] - n_v[l], wl.Nn_v)):
             if M == 0:
@@ -129,7 +132,7 @@ def test_cfg4_full_size():
     # indices differ (both inside rule (c)'s band, scores equal to 7 digits)
     n_diff = run_full_step(I.CFG4, sample_layers=(0, 18, 35))
     print(f"cfg4 n_diff = {n_diff}")
-    assert n_diff <= 4
+    assert n_diff <= 2          # what is measured; the kernels are deterministic, so it does not drift
 
 
 def test_cfg3_full_size():
@@ -191,3 +194,108 @@ def test_cfg5_streaming_teacher_forced():
     assert int(src.n.min()) == wl.budget
     assert n_diff == 0
     eng.close()
+
+
+def test_cfg2_offline_ragged_table_full_size():
+    """NEXT-2 at size on the tensor-core path (Eq.13-14, "determined offline ... calibration set"; R28).
+    One stream of config 2's shape (28 layers, 28 / 4 heads, bf16, 16384 cached rows, chunks of 4096 + 1500), cache
+    buffers sized for B_max.  Calibration: three CONSECUTIVE chunks run free under the uniform budget and their statistics
+    are accumulated on the device (omnimem_calibrate_accumulate); omnimem_calibrate_budgets turns the means into the table
+    B^(l) = Softmax(C/T) x 28 x 16384 clamped to [8192, 24576].  The layers' queries get different scales (so their
+    attention entropies, and with them the table, differ).  Then three more chunks run free under that RAGGED table without
+    `out=`-forced scoring: layers whose cache plus chunk still fit (B^(l) = 24576 in the first table step) skip scoring
+    inside the same launches in which others evict, n[l] differs from layer to layer afterwards, and
+      * on every layer of every step: rows out = min(B^(l), rows in + Nn), budgets sum, indices ascending and in range,
+        compacted rows byte-identical to an independent gather;
+      * on the smallest-budget and the largest-budget layer of the last step: the oracle, started from the GPU's own
+        pre-step cache of that layer (teacher forcing), at rules (a), (b), (c)."""
+    from paper_2606_07577_b200.omnimem import Chunk, OmniMem
+    Bmin, Bmax = 8192, 24576
+    wl = I.CFG2.replace(cache_cap=Bmax)
+    L = wl.L
+    total = L * wl.budget
+    eng = OmniMem.for_workload(wl, budget_min=Bmin, budget_max=Bmax)
+    dev = eng.device
+    qscale = torch.linspace(0.5, 2.0, L).view(L, 1, 1, 1)
+
+    def draw(step, with_cache=False):
+        x = I.full_inputs(wl, step=step, with_cache=with_cache)
+        x["Q"] = (x["Q"].float() * qscale).to(x["Q"].dtype)
+        return x
+
+    x = draw(0, with_cache=True)
+    from paper_2606_07577_b200.omnimem import Cache
+    src = Cache(x["cacheK"].to(dev), x["cacheV"].to(dev), x["n_v"].to(dev), x["n"].to(dev))
+    dst = eng.new_cache()
+    sc = eng.new_scores(wl.Nn, want_lse=True)
+    M_v = torch.zeros(L, dtype=torch.int32, device=dev)
+    M_a = torch.zeros_like(M_v)
+    idx_v, idx_a = eng.new_indices()
+    B_uni = torch.full((L,), wl.budget, dtype=torch.int32, device=dev)
+    acc = eng.new_calibration()
+    n_cal, n_run = 3, 3
+    for step in range(n_cal):                                   # calibration chunks: consecutive, free-running, uniform budget
+        if step:
+            x = draw(step)
+        chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+        eng.compress_chunk(src, chunk, B_uni, dst, out=sc, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+        eng.calibrate_accumulate(sc.stats, acc)
+        torch.cuda.synchronize()
+        src, dst = dst, src
+    B_dev, mean_stats = eng.calibrate_budgets(acc, total)
+    torch.cuda.synchronize()
+    B = B_dev.cpu().numpy()
+    C = (mean_stats[:, 6] * (1.0 - mean_stats[:, 7])).cpu().numpy()
+    print(f"table: min {B.min()} max {B.max()} sum {B.sum()}; C^(l) from {C.min():.4f} to {C.max():.4f}")
+    assert B.sum() == total and B.min() >= Bmin and B.max() <= Bmax
+    assert B.max() - B.min() >= 4096, "the calibration inputs should give a visibly non-uniform table"
+    assert np.all(np.diff(B[np.argsort(C, kind="stable")]) >= -1)           # Eq.14: a larger C^(l) never gets fewer rows
+    n_diff = 0
+    for k in range(n_run):                                      # free-running under the ragged table
+        step = n_cal + k
+        x = draw(step)
+        chunk = Chunk(x["chunkK"].to(dev), x["chunkV"].to(dev), x["Q"].to(dev), wl.Nn_v, wl.Nn_a)
+        n_v, n = src.n_v.cpu().numpy(), src.n.cpu().numpy()
+        last = k == n_run - 1
+        # `out=` makes every layer score (needed for the oracle comparison of the last step); the earlier steps run as
+        # bench.py's `ragged` leg does, with the skip of layers that have nothing to evict
+        if last:
+            eng.compress_chunk(src, chunk, B_dev, dst, out=sc, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+        else:
+            eng.compress_chunk(src, chunk, B_dev, dst, idx_v=idx_v, idx_a=idx_a, M_v=M_v, M_a=M_a)
+        torch.cuda.synchronize()
+        n_out = dst.n.cpu().numpy()
+        assert np.array_equal(n_out, np.minimum(B, n + wl.Nn)), f"step {step}: rows out {n_out}"
+        scored = (n + wl.Nn > B) | last
+        if k == 0 and B.max() >= n.max() + wl.Nn:
+            assert (~scored).any()                              # first table step: the B_max layers only append
+        check_any_size_properties(wl, src, chunk, dst, sc, idx_v, idx_a, M_v, M_a, n_v, n, budgets=B,
+                                  scored=scored if last else np.zeros(L, bool))
+        if last:
+            assert len(set(n.tolist())) > 2                     # ragged n[l] went through the tcgen05 kernels
+            for l in (int(np.argmin(B)), int(np.argmax(B))):
+                cK, cV = src.k[l:l + 1].cpu(), src.v[l:l + 1].cpu()
+                wl_l = wl.replace(budget=int(B[l]))
+                orc = oracle_layer(wl_l, x, l, int(n_v[l]), int(n[l]), cacheK=cK, cacheV=cV)
+                assert int(orc["n_out"][0]) == n_out[l]
+                n_diff += check_sampled_layer(wl_l, eng, x, l, l, src, chunk, sc, idx_v, idx_a, M_v, M_a, int(n_v[l]),
+                                              int(n[l]), orc=orc)
+        src, dst = dst, src
+    print(f"ragged table: n_diff = {n_diff}")
+    assert n_diff <= 2
+    eng.close()
+
+
+def test_cfg2_shape_variants_one_layer_each():
+    """The two variants that were parity-checked at <= 1.3 k rows only, on ONE layer of config 2's shape each (21 980 keys,
+    4 KV heads x 7 query heads, the launch geometry of the full step: 86 items per head), all rules against the oracle:
+      * select_scope = 1 (R29, the paper-literal one index set per layer): psi from the head-summed importance and the
+        head-mean redundancy, identical index rows on every head;
+      * sim_source = 2, d_model = 3584 (R30, Eq.7 on retained hidden states, Qwen2.5-Omni-7B's width): the hidden sweep and
+        the K / V / H compaction, H rows byte-exact."""
+    from tests.test_gpu_parity import check_hidden_variant, check_step
+    wl = I.CFG2.replace(L=1)
+    n1 = check_step(wl, select_scope=1, check_rowH=False)
+    n2 = check_hidden_variant(wl, 3584, steps=1)
+    print(f"cfg2-shape variants: select_scope=1 n_diff = {n1}, hidden states n_diff = {n2}")
+    assert (n1 or 0) <= 2 and n2 <= 2
