@@ -46,13 +46,18 @@ template <> struct Vec16<__nv_bfloat16> {
 // kTPR = 4 threads cover one row, kVec 16-byte vectors each (vector j of the row goes to thread j % 4, so a warp's load
 // instruction touches 8 rows x 64 contiguous bytes).  One block works on kUnroll * 64 consecutive items of one (layer, KV
 // head) at a time; every thread first issues all of its 2 * kUnroll * kVec loads (row t and its partner t + sigma, which
-// comes out of L1 / L2), then reduces: enough bytes in flight per SM to run at HBM speed, and ~25 instructions per 16 bytes
-// instead of ~115 (the first version was instruction-bound: ncu, profiles/).
+// comes out of L1 / L2), then reduces: ~25 instructions per 16 bytes instead of ~115 (the first version was
+// instruction-bound: ncu, profiles/).
+// Round 3: a block alternates a load phase and a reduce phase, so what hides one block's latency is the OTHER resident
+// blocks, not more loads per thread.  With kUnroll = 2 the bf16 kernel took 92 registers = 2 blocks per SM (ncu: 24 % warps
+// active, 56 % of the HBM copy peak); kUnroll = 1 under __launch_bounds__(256, 4) takes 56 registers = 4 blocks per SM with
+// the same bytes in flight per SM: config 2 0.196 -> 0.120 ms (5.35 TB/s, 82 % of the measured copy peak), config 3
+// 0.907 -> 0.573 ms (88 %).  (3 blocks of the kUnroll = 2 form: 0.149 / 0.693 ms.)
 // Items are numbered DENSELY over the rows that exist (K_v visual, then K_a audio: device counts), and a fixed number of
 // blocks per (layer, KV head) strides over them: sized by capacity, 43 % of the blocks of config 2 had no row to read and
 // their launch overhead alone was a quarter of the kernel's time.
 template <typename T, int kVec, int kUnroll>
-__global__ void __launch_bounds__(256) cosine_kernel(StepParams p, const T* __restrict__ cacheX,
+__global__ void __launch_bounds__(256, kVec * kUnroll <= 4 ? 4 : 3) cosine_kernel(StepParams p, const T* __restrict__ cacheX,
                                                      const T* __restrict__ chunkX, float* __restrict__ cosn) {
   constexpr int kTPR = 4, kRows = 256 / kTPR;
   const int items = p.seg_cap_v + p.seg_cap_a;
@@ -166,12 +171,13 @@ cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const Ste
   const void* kx = ctx->cfg.sim_source == 0 ? b.chunkV : b.chunkK;
   const int row_bytes = p.D * (ctx->cfg.dtype == OMNIMEM_FP32 ? 4 : 2);
   const int vec = row_bytes / 64;                      // 16-byte vectors per thread (4 threads per row): 2, 4 or 8
-  const int unroll = vec == 8 ? 1 : 2;
+  const int unroll = 1;
   const int rows_per_block = unroll * 64;
   // a fixed number of blocks per (layer, KV head) strides over the rows that exist (device counts): just under 8 full
-  // waves of 3 resident blocks per SM (80 registers), so that no wave is left mostly empty and no block finds nothing to do
+  // waves of the resident blocks per SM (4; 3 for 512-byte fp32 rows), so that no wave is left mostly empty and no block
+  // finds nothing to do
   const int lh_count = p.L * p.Hkv;
-  int per_lh = ctx->sm_count * 3 * 8 / lh_count;
+  int per_lh = ctx->sm_count * (vec == 8 ? 3 : 4) * 8 / lh_count;
   const int need = (items + rows_per_block - 1) / rows_per_block;
   if (per_lh > need) per_lh = need;
   if (per_lh < 1) per_lh = 1;
@@ -179,9 +185,9 @@ cudaError_t launch_cosine(const omnimem_ctx* ctx, const StepParams& p, const Ste
   ++*launches;
 #define OMNIMEM_COS(T, V, U) cosine_kernel<T, V, U><<<grid, 256, 0, st>>>(p, (const T*)cx, (const T*)kx, b.cosn)
   if (ctx->cfg.dtype == OMNIMEM_FP32) {
-    if (vec == 4) OMNIMEM_COS(float, 4, 2); else OMNIMEM_COS(float, 8, 1);
+    if (vec == 4) OMNIMEM_COS(float, 4, 1); else OMNIMEM_COS(float, 8, 1);
   } else {
-    if (vec == 2) OMNIMEM_COS(__nv_bfloat16, 2, 2); else OMNIMEM_COS(__nv_bfloat16, 4, 2);
+    if (vec == 2) OMNIMEM_COS(__nv_bfloat16, 2, 1); else OMNIMEM_COS(__nv_bfloat16, 4, 1);
   }
 #undef OMNIMEM_COS
   return cudaGetLastError();
